@@ -1,0 +1,28 @@
+"""Builds oracle/libkvr_oracle.so from oracle/kvr_oracle.c with gcc.
+
+ORACLE = test infrastructure (see the header of kvr_oracle.c).  Building the
+checker is not using it: __graft_entry__.build() calls build() here; only
+tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs load the result.
+"""
+import os
+import subprocess
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(HERE, "kvr_oracle.c")
+LIB = os.path.join(HERE, "libkvr_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    if (not force and os.path.exists(LIB)
+            and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
+        return LIB
+    cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-ffp-contract=off", "-fno-fast-math",
+           "-Wall", "-Wextra", "-shared", "-fPIC", SRC, "-o", LIB + ".tmp", "-lm"]
+    subprocess.run(cmd, check=True)
+    os.replace(LIB + ".tmp", LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force=True))

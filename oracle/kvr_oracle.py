@@ -1,0 +1,142 @@
+"""ctypes wrapper around oracle/libkvr_oracle.so -- ORACLE, test infrastructure.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+reference legs may import this module.  It imports nothing from the product
+package and the product package imports nothing from here.  All arrays are
+numpy arrays in HOST memory: uint16 holds bf16 bit patterns, uint8 holds
+e4m3fn bit patterns.  See kvr_oracle.c for the definition and its citations
+(PAPER.md:131, :393, :143).
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+BF16, FP8_E4M3 = 0, 1
+NEOX_HALF, GPTJ_INTERLEAVED = 0, 1
+OK, ERR_INVALID_ARG, ERR_OUT_OF_RANGE = 0, -1, -4
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        _lib = C.CDLL(path)
+        _lib.kvr_oracle_bf16_decode.restype = C.c_double
+        _lib.kvr_oracle_bf16_decode.argtypes = [C.c_uint16]
+        _lib.kvr_oracle_bf16_encode.restype = C.c_uint16
+        _lib.kvr_oracle_bf16_encode.argtypes = [C.c_double]
+        _lib.kvr_oracle_e4m3_decode.restype = C.c_double
+        _lib.kvr_oracle_e4m3_decode.argtypes = [C.c_uint8]
+        _lib.kvr_oracle_e4m3_encode_sat.restype = C.c_uint8
+        _lib.kvr_oracle_e4m3_encode_sat.argtypes = [C.c_double]
+        _lib.kvr_oracle_rotate_f64.restype = C.c_int
+        _lib.kvr_oracle_rotate_f64.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int, C.c_int,
+                                               C.c_int, C.c_void_p, C.c_void_p]
+        _lib.kvr_oracle_reposition_splice.restype = C.c_int
+        _lib.kvr_oracle_reposition_splice.argtypes = (
+            [C.c_int] * 6 + [C.c_void_p] +                      # model
+            [C.c_void_p, C.c_void_p] + [C.c_int64] * 4 + [C.c_int, C.c_int] +
+            [C.c_void_p, C.c_int, C.c_int, C.c_void_p] +          # pool
+            [C.c_void_p, C.c_void_p] + [C.c_int64] * 3 + [C.c_int] * 5 +
+            [C.c_void_p, C.c_void_p] +                            # segment
+            [C.c_int] * 3)                                        # control
+        _lib.kvr_oracle_bytes_moved.restype = C.c_uint64
+        _lib.kvr_oracle_bytes_moved.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int64]
+    return _lib
+
+
+def _ptr(a, dtype=None, writable=False):
+    if a is None:
+        return None
+    assert isinstance(a, np.ndarray), type(a)
+    if dtype is not None:
+        assert a.dtype == dtype, (a.dtype, dtype)
+    assert a.flags["C_CONTIGUOUS"]
+    if writable:
+        assert a.flags["WRITEABLE"]
+    return a.ctypes.data
+
+
+# ---- codecs (scalar, and vectorised by plain loops over the C scalar routine) ----
+
+def bf16_decode(bits):
+    f = lib().kvr_oracle_bf16_decode
+    b = np.asarray(bits, dtype=np.uint16)
+    return np.array([f(int(x)) for x in b.ravel()], dtype=np.float64).reshape(b.shape)
+
+
+def bf16_encode(x):
+    f = lib().kvr_oracle_bf16_encode
+    v = np.asarray(x, dtype=np.float64)
+    return np.array([f(float(t)) for t in v.ravel()], dtype=np.uint16).reshape(v.shape)
+
+
+def e4m3_decode(bits):
+    f = lib().kvr_oracle_e4m3_decode
+    b = np.asarray(bits, dtype=np.uint8)
+    return np.array([f(int(x)) for x in b.ravel()], dtype=np.float64).reshape(b.shape)
+
+
+def e4m3_encode_sat(x):
+    f = lib().kvr_oracle_e4m3_encode_sat
+    v = np.asarray(x, dtype=np.float64)
+    return np.array([f(float(t)) for t in v.ravel()], dtype=np.uint8).reshape(v.shape)
+
+
+# ---- pure fp64 rotation (the arithmetic core; RoPE itself when applied to a pre-RoPE key) ----
+
+def rotate_f64(x, delta, inv_freq, rotary_dim, pairing):
+    """x: [n, head_dim] float64; delta: [n] int64 position shift per row."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    n, head_dim = x.shape
+    delta = np.ascontiguousarray(np.broadcast_to(np.asarray(delta, dtype=np.int64), (n,)))
+    inv_freq = np.ascontiguousarray(inv_freq, dtype=np.float64)
+    assert inv_freq.shape == (rotary_dim // 2,)
+    out = np.empty_like(x)
+    st = lib().kvr_oracle_rotate_f64(_ptr(x), _ptr(out, writable=True), n, head_dim, rotary_dim,
+                                     pairing, _ptr(inv_freq), _ptr(delta))
+    if st != OK:
+        raise ValueError(f"kvr_oracle_rotate_f64 -> {st}")
+    return out
+
+
+# ---- the oracle proper ----
+
+def reposition_splice(*, layers, kv_heads, head_dim, rotary_dim, pairing, dtype, inv_freq,
+                      k_cache, v_cache, stride_layer, stride_block, stride_token, stride_head,
+                      num_blocks, block_size, block_table, k_scale_dst=None,
+                      k_src, v_src, src_stride_layer, src_stride_head, src_stride_token,
+                      len, old_start, new_start, dst_seq, dst_token_start,
+                      pos_map=None, k_scale_src=None,
+                      layer_begin=0, layer_end=None, n_threads=1):
+    """Splices ONE segment into (k_cache, v_cache) in place.  Returns the status code."""
+    edt = np.uint16 if dtype == BF16 else np.uint8
+    inv_freq = np.ascontiguousarray(inv_freq, dtype=np.float64)
+    assert inv_freq.shape == (rotary_dim // 2,)
+    assert block_table.dtype == np.int32 and block_table.ndim == 2
+    num_seqs, max_blocks = block_table.shape
+    if layer_end is None:
+        layer_end = layers
+    return lib().kvr_oracle_reposition_splice(
+        layers, kv_heads, head_dim, rotary_dim, pairing, dtype, _ptr(inv_freq),
+        _ptr(k_cache, edt, True), _ptr(v_cache, edt, True),
+        stride_layer, stride_block, stride_token, stride_head, num_blocks, block_size,
+        _ptr(block_table, np.int32), num_seqs, max_blocks, _ptr(k_scale_dst, np.float32),
+        _ptr(k_src, edt), _ptr(v_src, edt), src_stride_layer, src_stride_head, src_stride_token,
+        len, old_start, new_start, dst_seq, dst_token_start,
+        _ptr(pos_map, np.int32), _ptr(k_scale_src, np.float32),
+        layer_begin, layer_end, n_threads)
+
+
+def bytes_moved(layers, kv_heads, head_dim, dtype, tokens):
+    return int(lib().kvr_oracle_bytes_moved(layers, kv_heads, head_dim, dtype, tokens))
+
+
+def host_threads():
+    """Threads the OpenMP timing variant can use = cores this process may run on."""
+    return len(os.sched_getaffinity(0))
