@@ -1,0 +1,159 @@
+/*
+ * kvr.h -- C ABI of the kvr library: RoPE REPOSITIONING + SPLICE of precompiled
+ * key/value segments into a paged KV cache, on one NVIDIA B200 (sm_100a).
+ *
+ * The operation is the data-parallel hot path behind the "composable" KV cache of
+ * arxiv/paper_2606_17107 ("Models Take Notes at Prefill: KV Cache Can Be Editable and
+ * Composable").  PAPER.md = the paper text; line numbers refer to it.
+ *
+ *   PAPER.md:131 (sec. 5): "we precompile a long skill ... and because the attention library
+ *     caches post-RoPE keys, we re-rotate the chunk's keys from their source positions to the
+ *     target positions (values are position-free) before concatenating (Figure 4b)."
+ *   PAPER.md:393 (App. B): "The skill is prefilled once in isolation (positions 0..L-1), its keys
+ *     re-rotated to the target offset, and spliced after the system prompt".
+ *   PAPER.md:143 (sec. 5): "transplant is O(L) (a re-rotation pass plus the suffix)".
+ *   PAPER.md:528 (App. H): the memory chunk is "RoPE-repositioned ... each turn (an O(L_mem)
+ *     re-rotation, no re-prefill)".
+ *   PAPER.md:209 (sec. 8): the operation is compatible with "paged attention/vLLM, and GQA/MQA".
+ *
+ * For every spliced segment s, layer l, kv head h and token t in [0, len_s):
+ *     Delta_t = new_start - old_start            (or pos_map[t] - (old_start + t) if pos_map)
+ *     for each rotary pair i < rotary_dim/2, with phi = Delta_t * inv_freq[i]:
+ *         (ia, ib) = (i, i + rotary_dim/2)  [KVR_PAIR_NEOX_HALF]  or  (2i, 2i+1)  [KVR_PAIR_GPTJ_INTERLEAVED]
+ *         K'[ia] = K[ia] cos(phi) - K[ib] sin(phi) ;  K'[ib] = K[ib] cos(phi) + K[ia] sin(phi)
+ *     dims [rotary_dim, head_dim) of K and all of V are copied unchanged
+ *     j = dst_token_start + t ; blk = block_table[dst_seq][j / block_size] ; off = j % block_size
+ *     K', V are written at element offset  l*stride_layer + blk*stride_block + off*stride_token + h*stride_head
+ * Delta_t == 0 copies the K row byte for byte.  In KVR_FP8_E4M3 mode K is dequantised with the
+ * source scale, rotated, and requantised (round-to-nearest-even, saturating to +-448) with the
+ * destination scale; V bytes are always copied unchanged.
+ *
+ * Every step above runs in hand-written CUDA kernels; there is no CPU fallback.  All entry points
+ * return kvr_status and never throw.  Nothing here synchronises the device except where stated.
+ */
+#ifndef KVR_H_
+#define KVR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define KVR_API __attribute__((visibility("default")))
+
+typedef struct kvr_ctx kvr_ctx; /* opaque; owned by the library */
+
+typedef enum {
+  KVR_OK = 0,
+  KVR_ERR_INVALID_ARG = -1,  /* NULL pointer, bad enum, odd rotary_dim, len <= 0, dst_seq out of range ... */
+  KVR_ERR_UNSUPPORTED = -2,  /* valid but not implemented on this build / device (e.g. not sm_100)          */
+  KVR_ERR_ALIGNMENT = -3,    /* a base pointer or stride is not a multiple of 16 bytes                     */
+  KVR_ERR_OUT_OF_RANGE = -4, /* segment runs past its block-table row; device: bad block-table entry        */
+  KVR_ERR_CUDA = -5,         /* a CUDA runtime call failed (see kvr_last_cuda_error)                        */
+  KVR_ERR_NOMEM = -6
+} kvr_status;
+
+typedef enum { KVR_BF16 = 0, KVR_FP8_E4M3 = 1 } kvr_dtype;
+typedef enum { KVR_PAIR_NEOX_HALF = 0, KVR_PAIR_GPTJ_INTERLEAVED = 1 } kvr_pairing;
+
+/* Fixed per model.  inv_freq is a HOST array of rotary_dim/2 doubles, copied by kvr_create; the caller
+ * applies any frequency scaling (standard theta^(-2i/R), llama3, YaRN ...; "RoPE [28] and
+ * their extensions [25]").  rotary_dim is even, 2 <= rotary_dim <= head_dim (partial rotary allowed).
+ * head_dim * sizeof(element) must be a multiple of 16 bytes. */
+typedef struct {
+  int32_t layers, kv_heads, head_dim, rotary_dim;
+  int32_t pairing; /* kvr_pairing */
+  int32_t dtype;   /* kvr_dtype   */
+  const double* inv_freq;
+} kvr_model_desc;
+
+/* Destination paged pool: caller-owned DEVICE memory.  K and V pools share the four element strides;
+ * head_dim elements are contiguous.  Covers token-major ("NHD": stride_token = kv_heads*head_dim,
+ * stride_head = head_dim) and head-major ("HND": stride_head = block_size*head_dim, stride_token =
+ * head_dim) block layouts, with the layer dimension outside or inside the block dimension.
+ * block_table is a DEVICE array [num_seqs][max_blocks_per_seq] of physical block ids; an entry the call
+ * touches that is < 0 or >= num_blocks makes the kernel skip that token range and raise the sticky
+ * device status (kvr_last_device_status).  k_scale: DEVICE [layers*kv_heads] fp32 destination K scales,
+ * KVR_FP8_E4M3 only (NULL otherwise). */
+typedef struct {
+  void* k_cache;
+  void* v_cache;
+  int64_t stride_layer, stride_block, stride_token, stride_head; /* elements */
+  int32_t num_blocks, block_size;
+  const int32_t* block_table;
+  int32_t num_seqs, max_blocks_per_seq;
+  const float* k_scale;
+} kvr_paged_dst;
+
+/* One spliced segment.  The ARRAY of segments lives on the HOST and is copied before the call returns.
+ * k_src / v_src: DEVICE, logical [layers][kv_heads][len][head_dim] addressed by the three element
+ * strides (head_dim contiguous).  delta = new_start - old_start (any sign).  Token t is written to logical
+ * token dst_token_start + t of block-table row dst_seq (slots are dense; positions only set angles).
+ * pos_map: DEVICE int32 [len] or NULL; if given, token t moves to position pos_map[t], i.e.
+ * delta_t = pos_map[t] - (old_start + t), and new_start is ignored.
+ * k_scale_src: DEVICE fp32 [layers*kv_heads] source K scales (fp8 only); NULL = same as destination.
+ * Two segments that write the same slot, or a source that aliases the destination, are undefined. */
+typedef struct {
+  const void* k_src;
+  const void* v_src;
+  int64_t src_stride_layer, src_stride_head, src_stride_token; /* elements */
+  int32_t len, old_start, new_start;
+  int32_t dst_seq, dst_token_start;
+  const int32_t* pos_map;
+  const float* k_scale_src;
+} kvr_segment;
+
+/* Optional tuning knobs (0 = library default).  Never changes results, only the launch shape. */
+typedef struct {
+  int32_t path;            /* 0 auto, 1 force the generic kernel, 2 force the TMA-ring kernel */
+  int32_t ctas_per_sm;     /* persistent CTAs per SM for the ring kernel                       */
+  int32_t consumer_warps;  /* consumer warps per CTA                                           */
+  int32_t stages;          /* ring depth (tiles in flight per CTA)                             */
+  int32_t layers_per_unit; /* layers one scheduled unit covers                                  */
+  int32_t v_bulk_store;    /* 0 auto, 1 V leaves shared memory by bulk (TMA) stores, 2 by warps */
+  int32_t reserved[10];
+} kvr_tuning;
+
+/* Creates a context on CUDA device `cuda_device` (must be compute capability 10.x).  Allocates a few
+ * hundred KB of device and pinned host memory (descriptor staging, status word).  Synchronous. */
+KVR_API kvr_status kvr_create(kvr_ctx** out, const kvr_model_desc* model, int cuda_device);
+KVR_API kvr_status kvr_destroy(kvr_ctx* ctx); /* synchronises the device; NULL is a no-op */
+KVR_API kvr_status kvr_set_tuning(kvr_ctx* ctx, const kvr_tuning* t); /* NULL restores defaults */
+
+/* Host-only validation of one call's arguments (no CUDA call is made; usable without a GPU).
+ * Returns the status kvr_reposition_splice would return before launching anything. */
+KVR_API kvr_status kvr_validate(const kvr_model_desc* model, const kvr_paged_dst* dst,
+                                const kvr_segment* segs, int32_t n_segs);
+
+/* THE HOT PATH.  Enqueues, on `cuda_stream` (a cudaStream_t; NULL = the legacy
+ * default stream), the reposition + splice of n_segs segments into dst.  Asynchronous: returns once the
+ * work is enqueued; there is no device synchronisation.  Host-detectable faults are rejected before any
+ * launch and leave the destination untouched.  Calls on one context must be issued to one stream at a
+ * time (the context owns per-call staging).  Every destination byte not addressed keeps its value. */
+KVR_API kvr_status kvr_reposition_splice(kvr_ctx* ctx, const kvr_paged_dst* dst, const kvr_segment* segs,
+                                         int32_t n_segs, void* cuda_stream);
+
+/* Algorithmic bytes of a call: read K, read V, write K, write V = 4 * layers*kv_heads*head_dim*esz * sum(len).
+ * This is the O(L) of PAPER.md:143 and the numerator of every GB/s this repository reports. */
+KVR_API uint64_t kvr_bytes_moved(const kvr_model_desc* model, const kvr_segment* segs, int32_t n_segs);
+
+/* Waits for the stream of the last call, then reports and clears the sticky device status:
+ * KVR_OK, or KVR_ERR_OUT_OF_RANGE with the first offending segment index and token (either may be NULL). */
+KVR_API kvr_status kvr_last_device_status(kvr_ctx* ctx, int32_t* bad_segment, int32_t* bad_token);
+
+/* Introspection for benchmarks: kernels launched by this context so far; the kernel path the last call took
+ * (1 generic, 2 TMA ring); grid size, CTA size and dynamic shared memory of its main kernel. */
+KVR_API uint64_t kvr_launch_count(const kvr_ctx* ctx);
+KVR_API kvr_status kvr_last_launch_info(const kvr_ctx* ctx, int32_t* path, int32_t* grid, int32_t* block,
+                                        int32_t* smem_bytes);
+
+KVR_API const char* kvr_status_string(kvr_status s);
+KVR_API const char* kvr_last_cuda_error(const kvr_ctx* ctx); /* "" if none; valid until the next call */
+KVR_API const char* kvr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KVR_H_ */

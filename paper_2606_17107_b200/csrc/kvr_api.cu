@@ -1,0 +1,376 @@
+// kvr_api.cu -- the C ABI of include/kvr.h: context, host-side validation, work decomposition,
+// descriptor staging and kernel dispatch.  No arithmetic of the method happens on the host.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/kvr.h"
+#include "kvr_common.cuh"
+
+using namespace kvr;
+
+namespace {
+
+constexpr int kSlots = 8;           // descriptor staging ring (calls in flight per context)
+constexpr int kInitialSegCap = 256;
+
+struct Slot {
+  SegDev* host = nullptr;           // pinned
+  SegDev* dev = nullptr;
+  size_t cap = 0;
+  cudaEvent_t ev = nullptr;
+  bool pending = false;
+};
+
+inline int elt_bytes(int dtype) { return dtype == KVR_BF16 ? 2 : 1; }
+
+kvr_status check_model(const kvr_model_desc* m) {
+  if (!m || !m->inv_freq) return KVR_ERR_INVALID_ARG;
+  if (m->layers <= 0 || m->kv_heads <= 0 || m->head_dim <= 0) return KVR_ERR_INVALID_ARG;
+  if (m->rotary_dim < 2 || (m->rotary_dim & 1) || m->rotary_dim > m->head_dim) return KVR_ERR_INVALID_ARG;
+  if (m->pairing != KVR_PAIR_NEOX_HALF && m->pairing != KVR_PAIR_GPTJ_INTERLEAVED) return KVR_ERR_INVALID_ARG;
+  if (m->dtype != KVR_BF16 && m->dtype != KVR_FP8_E4M3) return KVR_ERR_INVALID_ARG;
+  if (((int64_t)m->head_dim * elt_bytes(m->dtype)) % 16 != 0) return KVR_ERR_ALIGNMENT;
+  return KVR_OK;
+}
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+kvr_status check_call(const kvr_model_desc* m, const kvr_paged_dst* d, const kvr_segment* segs, int32_t n) {
+  kvr_status st = check_model(m);
+  if (st != KVR_OK) return st;
+  if (!d || n < 0 || (n > 0 && !segs)) return KVR_ERR_INVALID_ARG;
+  if (!d->k_cache || !d->v_cache || !d->block_table) return KVR_ERR_INVALID_ARG;
+  if (d->num_blocks <= 0 || d->block_size <= 0 || d->num_seqs <= 0 || d->max_blocks_per_seq <= 0)
+    return KVR_ERR_INVALID_ARG;
+  if (d->stride_layer < 0 || d->stride_block <= 0 || (d->stride_token < m->head_dim && d->block_size > 1))
+    return KVR_ERR_INVALID_ARG;
+  if (d->stride_head < m->head_dim && m->kv_heads > 1) return KVR_ERR_INVALID_ARG;
+  if (m->dtype == KVR_FP8_E4M3 && !d->k_scale) return KVR_ERR_INVALID_ARG;
+  const int E = elt_bytes(m->dtype);
+  if (!aligned16(d->k_cache) || !aligned16(d->v_cache)) return KVR_ERR_ALIGNMENT;
+  const int64_t ds[4] = {d->stride_layer, d->stride_block, d->stride_token, d->stride_head};
+  for (int64_t s : ds)
+    if ((s * E) % 16 != 0) return KVR_ERR_ALIGNMENT;
+  const int64_t cap = (int64_t)d->max_blocks_per_seq * d->block_size;
+  for (int32_t i = 0; i < n; ++i) {
+    const kvr_segment& s = segs[i];
+    if (!s.k_src || !s.v_src) return KVR_ERR_INVALID_ARG;
+    if (s.len <= 0 || s.dst_seq < 0 || s.dst_seq >= d->num_seqs || s.dst_token_start < 0)
+      return KVR_ERR_INVALID_ARG;
+    if (s.old_start < 0 || (!s.pos_map && s.new_start < 0)) return KVR_ERR_INVALID_ARG;
+    if (s.src_stride_token < m->head_dim && s.len > 1) return KVR_ERR_INVALID_ARG;
+    if (s.src_stride_layer < 0 || s.src_stride_head < 0) return KVR_ERR_INVALID_ARG;
+    if ((int64_t)s.dst_token_start + s.len > cap) return KVR_ERR_OUT_OF_RANGE;
+    if (!aligned16(s.k_src) || !aligned16(s.v_src)) return KVR_ERR_ALIGNMENT;
+    const int64_t ss[3] = {s.src_stride_layer, s.src_stride_head, s.src_stride_token};
+    for (int64_t x : ss)
+      if ((x * E) % 16 != 0) return KVR_ERR_ALIGNMENT;
+    if (s.pos_map && (reinterpret_cast<uintptr_t>(s.pos_map) & 3u)) return KVR_ERR_ALIGNMENT;
+  }
+  return KVR_OK;
+}
+
+// largest divisor of block_size that is <= limit
+int chunk_granularity(int block_size, int limit) {
+  if (limit < 1) limit = 1;
+  for (int c = (block_size < limit ? block_size : limit); c >= 1; --c)
+    if (block_size % c == 0) return c;
+  return 1;
+}
+
+}  // namespace
+
+struct kvr_ctx {
+  kvr_model_desc model{};
+  std::vector<double> inv_freq;
+  double* d_inv_freq = nullptr;
+  int32_t* d_status = nullptr;
+  int32_t* h_status = nullptr;      // pinned
+  int device = 0, sm_count = 0;
+  Slot slots[kSlots];
+  int next_slot = 0;
+  kvr_tuning tuning{};
+  uint64_t launches = 0;
+  int last_path = 0, last_grid = 0, last_block = 0, last_smem = 0;
+  cudaStream_t last_stream = nullptr;
+  std::string last_err;
+
+  kvr_status cuda_fail(cudaError_t e, const char* what) {
+    last_err = std::string(what) + ": " + cudaGetErrorString(e);
+    (void)cudaGetLastError();
+    return KVR_ERR_CUDA;
+  }
+};
+
+#define KVR_CUDA(ctx, call)                                  \
+  do {                                                       \
+    cudaError_t e_ = (call);                                 \
+    if (e_ != cudaSuccess) return (ctx)->cuda_fail(e_, #call); \
+  } while (0)
+
+static kvr_status slot_reserve(kvr_ctx* c, Slot& s, size_t n) {
+  if (n <= s.cap) return KVR_OK;
+  size_t cap = s.cap ? s.cap : kInitialSegCap;
+  while (cap < n) cap *= 2;
+  if (s.host) cudaFreeHost(s.host);
+  if (s.dev) cudaFree(s.dev);
+  s.host = nullptr; s.dev = nullptr; s.cap = 0;
+  KVR_CUDA(c, cudaMallocHost(&s.host, cap * sizeof(SegDev)));
+  KVR_CUDA(c, cudaMalloc(&s.dev, cap * sizeof(SegDev)));
+  s.cap = cap;
+  return KVR_OK;
+}
+
+extern "C" {
+
+kvr_status kvr_create(kvr_ctx** out, const kvr_model_desc* model, int cuda_device) {
+  if (!out) return KVR_ERR_INVALID_ARG;
+  *out = nullptr;
+  kvr_status st = check_model(model);
+  if (st != KVR_OK) return st;
+  int count = 0;
+  if (cudaGetDeviceCount(&count) != cudaSuccess || cuda_device < 0 || cuda_device >= count) {
+    (void)cudaGetLastError();
+    return KVR_ERR_CUDA;   // no CUDA device: this library has no CPU fallback
+  }
+  cudaDeviceProp prop{};
+  if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) return KVR_ERR_CUDA;
+  if (prop.major != 10) return KVR_ERR_UNSUPPORTED;   // built for sm_100a only
+  kvr_ctx* c = new (std::nothrow) kvr_ctx();
+  if (!c) return KVR_ERR_NOMEM;
+  c->model = *model;
+  c->inv_freq.assign(model->inv_freq, model->inv_freq + model->rotary_dim / 2);
+  c->model.inv_freq = c->inv_freq.data();
+  c->device = cuda_device;
+  c->sm_count = prop.multiProcessorCount;
+  int prev = 0;
+  cudaGetDevice(&prev);
+  cudaError_t e = cudaSetDevice(cuda_device);
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_inv_freq, c->inv_freq.size() * sizeof(double));
+  if (e == cudaSuccess) e = cudaMemcpy(c->d_inv_freq, c->inv_freq.data(), c->inv_freq.size() * sizeof(double),
+                                       cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_status, 4 * sizeof(int32_t));
+  if (e == cudaSuccess) e = cudaMemset(c->d_status, 0, 4 * sizeof(int32_t));
+  if (e == cudaSuccess) e = cudaMallocHost(&c->h_status, 4 * sizeof(int32_t));
+  for (int i = 0; i < kSlots && e == cudaSuccess; ++i)
+    e = cudaEventCreateWithFlags(&c->slots[i].ev, cudaEventDisableTiming);
+  cudaSetDevice(prev);
+  if (e != cudaSuccess) {
+    kvr_destroy(c);
+    (void)cudaGetLastError();
+    return KVR_ERR_CUDA;
+  }
+  *out = c;
+  return KVR_OK;
+}
+
+kvr_status kvr_destroy(kvr_ctx* c) {
+  if (!c) return KVR_OK;
+  int prev = 0;
+  cudaGetDevice(&prev);
+  cudaSetDevice(c->device);
+  cudaDeviceSynchronize();
+  for (Slot& s : c->slots) {
+    if (s.host) cudaFreeHost(s.host);
+    if (s.dev) cudaFree(s.dev);
+    if (s.ev) cudaEventDestroy(s.ev);
+  }
+  if (c->d_inv_freq) cudaFree(c->d_inv_freq);
+  if (c->d_status) cudaFree(c->d_status);
+  if (c->h_status) cudaFreeHost(c->h_status);
+  cudaSetDevice(prev);
+  (void)cudaGetLastError();
+  delete c;
+  return KVR_OK;
+}
+
+kvr_status kvr_set_tuning(kvr_ctx* c, const kvr_tuning* t) {
+  if (!c) return KVR_ERR_INVALID_ARG;
+  if (t) c->tuning = *t; else c->tuning = kvr_tuning{};
+  return KVR_OK;
+}
+
+kvr_status kvr_validate(const kvr_model_desc* model, const kvr_paged_dst* dst, const kvr_segment* segs,
+                        int32_t n_segs) {
+  return check_call(model, dst, segs, n_segs);
+}
+
+uint64_t kvr_bytes_moved(const kvr_model_desc* m, const kvr_segment* segs, int32_t n) {
+  if (!m || (n > 0 && !segs)) return 0;
+  uint64_t tokens = 0;
+  for (int32_t i = 0; i < n; ++i) tokens += segs[i].len > 0 ? (uint64_t)segs[i].len : 0u;
+  return 4ull * (uint64_t)m->layers * (uint64_t)m->kv_heads * (uint64_t)m->head_dim *
+         (uint64_t)elt_bytes(m->dtype) * tokens;
+}
+
+kvr_status kvr_reposition_splice(kvr_ctx* c, const kvr_paged_dst* d, const kvr_segment* segs, int32_t n,
+                                 void* cuda_stream) {
+  if (!c) return KVR_ERR_INVALID_ARG;
+  c->last_err.clear();
+  kvr_status st = check_call(&c->model, d, segs, n);
+  if (st != KVR_OK) return st;
+  if (n == 0) return KVR_OK;
+  for (int32_t i = 0; i < n; ++i) {
+    int64_t delta = (int64_t)segs[i].new_start - (int64_t)segs[i].old_start;
+    if (!segs[i].pos_map && (delta > INT32_MAX || delta < INT32_MIN)) return KVR_ERR_INVALID_ARG;
+  }
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  int prev = 0;
+  cudaGetDevice(&prev);
+  if (prev != c->device) KVR_CUDA(c, cudaSetDevice(c->device));
+  struct Restore { int prev, cur; ~Restore() { if (prev != cur) cudaSetDevice(prev); } } restore{prev, c->device};
+
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  KVR_CUDA(c, cudaStreamIsCapturing(stream, &cap));
+  const bool capturing = cap != cudaStreamCaptureStatusNone;
+
+  Slot& slot = c->slots[c->next_slot];
+  c->next_slot = (c->next_slot + 1) % kSlots;
+  if (slot.pending && !capturing) {
+    KVR_CUDA(c, cudaEventSynchronize(slot.ev));   // the call that used this slot 8 calls ago
+    slot.pending = false;
+  }
+  if ((size_t)n > slot.cap) {
+    if (capturing) return KVR_ERR_UNSUPPORTED;    // cannot allocate under stream capture; warm the context first
+    st = slot_reserve(c, slot, (size_t)n);
+    if (st != KVR_OK) return st;
+  }
+
+  const kvr_model_desc& m = c->model;
+  CallParams P{};
+  P.layers = m.layers; P.heads = m.kv_heads; P.head_dim = m.head_dim; P.rotary_dim = m.rotary_dim;
+  P.pairing = m.pairing; P.dtype = m.dtype; P.inv_freq = c->d_inv_freq;
+  P.k_cache = static_cast<uint8_t*>(d->k_cache); P.v_cache = static_cast<uint8_t*>(d->v_cache);
+  P.d_sl = d->stride_layer; P.d_sb = d->stride_block; P.d_st = d->stride_token; P.d_sh = d->stride_head;
+  P.block_table = d->block_table; P.k_scale_dst = d->k_scale;
+  P.num_blocks = d->num_blocks; P.block_size = d->block_size; P.num_seqs = d->num_seqs;
+  P.max_blocks = d->max_blocks_per_seq;
+  P.segs = slot.dev; P.n_segs = n; P.status = c->d_status;
+
+  bool any_map = false, scales_differ = false;
+  for (int32_t i = 0; i < n; ++i) {
+    any_map |= segs[i].pos_map != nullptr;
+    scales_differ |= (m.dtype == KVR_FP8_E4M3 && segs[i].k_scale_src && segs[i].k_scale_src != d->k_scale);
+  }
+  P.any_pos_map = any_map; P.scales_differ = scales_differ;
+
+  // ---- work decomposition: (segment, chunk of <= cg destination tokens, group of lpu layers) ----
+  auto decompose = [&](int cg, int lpu_request) {
+    P.cg = cg;
+    int64_t chunks_total = 0;
+    for (int32_t i = 0; i < n; ++i) {
+      const kvr_segment& s = segs[i];
+      SegDev& o = slot.host[i];
+      o.k_src = static_cast<const uint8_t*>(s.k_src); o.v_src = static_cast<const uint8_t*>(s.v_src);
+      o.pos_map = s.pos_map;
+      o.k_scale_src = s.k_scale_src ? s.k_scale_src : d->k_scale;
+      o.sl = s.src_stride_layer; o.sh = s.src_stride_head; o.st = s.src_stride_token;
+      o.len = s.len; o.old_start = s.old_start; o.delta = (int32_t)((int64_t)s.new_start - s.old_start);
+      o.dst_seq = s.dst_seq; o.dst_token_start = s.dst_token_start;
+      o.first_q = s.dst_token_start / cg;
+      o.n_chunks = (int32_t)(((int64_t)s.dst_token_start + s.len - 1) / cg - o.first_q + 1);
+      o.index = i; o.pad_ = 0;
+      chunks_total += o.n_chunks;
+    }
+    int lpu = lpu_request;
+    if (lpu <= 0) {
+      if (any_map) lpu = m.layers;   // the per-token angle table is built once per chunk and reused by all layers
+      else {
+        int64_t target = (int64_t)c->sm_count * 32;
+        int64_t v = (chunks_total * m.layers) / target;
+        lpu = (int)(v < 1 ? 1 : (v > m.layers ? m.layers : v));
+      }
+    }
+    if (lpu > m.layers) lpu = m.layers;
+    P.lpu = lpu; P.n_lgroups = (m.layers + lpu - 1) / lpu;
+    int64_t at = 0;
+    for (int32_t i = 0; i < n; ++i) {
+      slot.host[i].unit_begin = at;
+      at += (int64_t)slot.host[i].n_chunks * P.n_lgroups;
+    }
+    P.total_units = at;
+  };
+
+  const kvr_tuning& tu = c->tuning;
+  int path = tu.path;
+  const char* why = nullptr;
+  if (path == 0 || path == 2) {
+    decompose(chunk_granularity(d->block_size, 16), tu.layers_per_unit);
+    bool ok = ring_supported(P, slot.host, &why);
+    if (!ok && path == 2) { c->last_err = std::string("ring kernel unsupported: ") + (why ? why : ""); return KVR_ERR_UNSUPPORTED; }
+    path = ok ? 2 : 1;
+  }
+  if (path == 1) {
+    // generic kernel: chunk table [cg][R/2] float4 must fit 48 KB of static-limit shared memory
+    int limit = (int)(47 * 1024 / ((m.rotary_dim / 2) * 16 + 4));
+    if (limit < 1) return KVR_ERR_UNSUPPORTED;
+    decompose(chunk_granularity(d->block_size, limit < 16 ? limit : 16), tu.layers_per_unit);
+  }
+
+  KVR_CUDA(c, cudaMemcpyAsync(slot.dev, slot.host, (size_t)n * sizeof(SegDev), cudaMemcpyHostToDevice, stream));
+  cudaError_t e;
+  if (path == 2) {
+    RingConfig rc{tu.ctas_per_sm, tu.consumer_warps, tu.stages, tu.v_bulk_store};
+    e = launch_ring(P, rc, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
+  } else {
+    e = launch_generic(P, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
+  }
+  if (e != cudaSuccess) return c->cuda_fail(e, path == 2 ? "launch_ring" : "launch_generic");
+  c->launches += 1;
+  c->last_path = path;
+  c->last_stream = stream;
+  if (!capturing) {
+    KVR_CUDA(c, cudaEventRecord(slot.ev, stream));
+    slot.pending = true;
+  }
+  return KVR_OK;
+}
+
+kvr_status kvr_last_device_status(kvr_ctx* c, int32_t* bad_segment, int32_t* bad_token) {
+  if (!c) return KVR_ERR_INVALID_ARG;
+  int prev = 0;
+  cudaGetDevice(&prev);
+  if (prev != c->device) cudaSetDevice(c->device);
+  cudaError_t e = cudaMemcpyAsync(c->h_status, c->d_status, 4 * sizeof(int32_t), cudaMemcpyDeviceToHost, c->last_stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->d_status, 0, 4 * sizeof(int32_t), c->last_stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->last_stream);
+  if (prev != c->device) cudaSetDevice(prev);
+  if (e != cudaSuccess) return c->cuda_fail(e, "kvr_last_device_status");
+  if (c->h_status[0] == 0) return KVR_OK;
+  if (bad_segment) *bad_segment = c->h_status[1];
+  if (bad_token) *bad_token = c->h_status[2];
+  return KVR_ERR_OUT_OF_RANGE;
+}
+
+uint64_t kvr_launch_count(const kvr_ctx* c) { return c ? c->launches : 0; }
+
+kvr_status kvr_last_launch_info(const kvr_ctx* c, int32_t* path, int32_t* grid, int32_t* block, int32_t* smem) {
+  if (!c) return KVR_ERR_INVALID_ARG;
+  if (path) *path = c->last_path;
+  if (grid) *grid = c->last_grid;
+  if (block) *block = c->last_block;
+  if (smem) *smem = c->last_smem;
+  return KVR_OK;
+}
+
+const char* kvr_status_string(kvr_status s) {
+  switch (s) {
+    case KVR_OK: return "KVR_OK";
+    case KVR_ERR_INVALID_ARG: return "KVR_ERR_INVALID_ARG";
+    case KVR_ERR_UNSUPPORTED: return "KVR_ERR_UNSUPPORTED";
+    case KVR_ERR_ALIGNMENT: return "KVR_ERR_ALIGNMENT";
+    case KVR_ERR_OUT_OF_RANGE: return "KVR_ERR_OUT_OF_RANGE";
+    case KVR_ERR_CUDA: return "KVR_ERR_CUDA";
+    case KVR_ERR_NOMEM: return "KVR_ERR_NOMEM";
+  }
+  return "KVR_ERR_UNKNOWN";
+}
+
+const char* kvr_last_cuda_error(const kvr_ctx* c) { return c ? c->last_err.c_str() : ""; }
+
+const char* kvr_version(void) { return "kvr 0.1 (sm_100a)"; }
+
+}  // extern "C"

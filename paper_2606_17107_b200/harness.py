@@ -1,0 +1,58 @@
+"""Device-side materialisation of a workloads.Workload and its marshalling into the kvr C ABI.
+
+Used by tests/, bench.py and __graft_entry__.smoke().  torch is plumbing here: device memory, streams.
+Nothing in this module computes any part of the method, and nothing here touches oracle/.
+"""
+import numpy as np
+import torch
+
+from . import kvr
+
+_PAIRING = {"neox": kvr.KVR_PAIR_NEOX_HALF, "gptj": kvr.KVR_PAIR_GPTJ_INTERLEAVED}
+_DTYPE = {"bf16": kvr.KVR_BF16, "fp8": kvr.KVR_FP8_E4M3}
+
+
+def model_of(w):
+    return kvr.model_desc(w.layers, w.kv_heads, w.head_dim, w.rotary_dim, _PAIRING[w.pairing],
+                          _DTYPE[w.dtype], w.inv_freq)
+
+
+class DeviceWorkload:
+    """Sources, sentinel-filled pool, block table, position maps and scales of `w` resident on `device`,
+    plus the ctypes structs of one kvr_reposition_splice call over all segments."""
+
+    def __init__(self, w, device="cuda:0", sources=None, make_pool=True):
+        from workloads import make_pool as _make_pool, make_sources
+        self.w = w
+        self.device = torch.device(device)
+        self.model, self._inv_keep = model_of(w)
+        if sources is None:
+            sources = make_sources(w, self.device)
+        self.sources = [(k.to(self.device).contiguous(), v.to(self.device).contiguous()) for k, v in sources]
+        self.block_table = torch.from_numpy(np.ascontiguousarray(w.block_table)).to(self.device)
+        self.k_scale = self.k_scale_src = None
+        if w.k_scale is not None:
+            self.k_scale = torch.from_numpy(w.k_scale).to(self.device)
+        if w.k_scale_src is not None:
+            self.k_scale_src = torch.from_numpy(w.k_scale_src).to(self.device)
+        self.pos_maps = [None if s.pos_map is None else torch.from_numpy(s.pos_map).to(self.device)
+                         for s in w.segments]
+        self.k_cache = self.v_cache = None
+        if make_pool:
+            self.k_cache, self.v_cache = _make_pool(w, self.device)
+        self.segs = kvr.segment_array([
+            kvr.segment(k, v, w.src_strides(s), s.len, s.old_start, s.new_start, s.dst_seq, s.dst_token_start,
+                        pos_map=pm, k_scale_src=self.k_scale_src)
+            for s, (k, v), pm in zip(w.segments, self.sources, self.pos_maps)])
+        self.dst = self.dst_for(self.k_cache, self.v_cache) if make_pool else None
+
+    def dst_for(self, k_cache, v_cache):
+        w = self.w
+        return kvr.paged_dst(k_cache, v_cache, w.dst_strides(), w.num_blocks, w.block_size, self.block_table,
+                             w.block_table.shape[0], w.block_table.shape[1], k_scale=self.k_scale)
+
+    def bytes_moved(self):
+        return kvr.kvr_bytes_moved(self.model, self.segs)
+
+    def run(self, ctx, stream=None, dst=None):
+        return ctx.reposition_splice(dst if dst is not None else self.dst, self.segs, stream=stream)

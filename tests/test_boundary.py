@@ -1,0 +1,106 @@
+"""Host-side checks of the C-ABI boundary that need no GPU: the library loads, exports every symbol
+include/kvr.h declares, validates arguments, counts bytes, and refuses to run without a device."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def kvr():
+    from paper_2606_17107_b200 import build
+    build.build()
+    from paper_2606_17107_b200 import kvr as k
+    return k
+
+
+def test_exports_match_header(kvr):
+    header = open(os.path.join(ROOT, "include", "kvr.h")).read()
+    declared = set(re.findall(r"KVR_API\s+[\w\s\*]+?\b(kvr_\w+)\s*\(", header))
+    assert declared == set(kvr.EXPORTS), declared ^ set(kvr.EXPORTS)
+    for name in declared:
+        assert hasattr(kvr.lib, name), name
+    assert kvr.kvr_version().startswith("kvr ")
+
+
+def test_struct_layouts_match_header(kvr):
+    # sizes implied by the field lists in include/kvr.h on LP64
+    assert C.sizeof(kvr.kvr_model_desc) == 32
+    assert C.sizeof(kvr.kvr_paged_dst) == 16 + 32 + 8 + 8 + 8 + 8
+    assert C.sizeof(kvr.kvr_segment) == 16 + 24 + 20 + 4 + 16
+    assert C.sizeof(kvr.kvr_tuning) == 64
+
+
+def _call(kvr, **over):
+    m, keep = kvr.model_desc(over.get("layers", 2), 2, over.get("head_dim", 64), over.get("rotary_dim", 64),
+                             over.get("pairing", 0), over.get("dtype", 0), [1.0] * (over.get("rotary_dim", 64) // 2))
+    base = 1 << 20
+    d = kvr.paged_dst(base, base * 2, over.get("strides", (16 * 4 * 2 * 64, 4 * 2 * 64, 2 * 64, 64)), 16, 4, base * 3, 1,
+                      over.get("max_blocks", 8), k_scale=over.get("k_scale"))
+    s = kvr.segment(over.get("k_src", base * 4), base * 5, over.get("src_strides", (2 * 10 * 64, 10 * 64, 64)),
+                    over.get("len", 10), 0, over.get("new_start", 7), over.get("dst_seq", 0),
+                    over.get("dst_token_start", 3))
+    return kvr.kvr_validate(m, d, [s]), keep
+
+
+def test_validation(kvr):
+    assert _call(kvr)[0] == kvr.KVR_OK
+    assert _call(kvr, rotary_dim=63)[0] == kvr.KVR_ERR_INVALID_ARG
+    assert _call(kvr, rotary_dim=66)[0] == kvr.KVR_ERR_INVALID_ARG
+    assert _call(kvr, pairing=2)[0] == kvr.KVR_ERR_INVALID_ARG
+    assert _call(kvr, dtype=1)[0] == kvr.KVR_ERR_INVALID_ARG            # fp8 without k_scale
+    assert _call(kvr, dtype=1, k_scale=1 << 22)[0] == kvr.KVR_OK
+    assert _call(kvr, head_dim=60, rotary_dim=60)[0] == kvr.KVR_ERR_ALIGNMENT
+    assert _call(kvr, len=0)[0] == kvr.KVR_ERR_INVALID_ARG
+    assert _call(kvr, dst_seq=1)[0] == kvr.KVR_ERR_INVALID_ARG
+    assert _call(kvr, dst_token_start=23)[0] == kvr.KVR_ERR_OUT_OF_RANGE  # 23 + 10 > 8 * 4
+    assert _call(kvr, dst_token_start=22)[0] == kvr.KVR_OK
+    assert _call(kvr, k_src=(1 << 22) + 8)[0] == kvr.KVR_ERR_ALIGNMENT
+    assert _call(kvr, src_strides=(2 * 10 * 64, 10 * 64, 68))[0] == kvr.KVR_ERR_ALIGNMENT
+    assert _call(kvr, src_strides=(2 * 10 * 64, 10 * 64, 32))[0] == kvr.KVR_ERR_INVALID_ARG
+    assert _call(kvr, strides=(16 * 4 * 2 * 64, 4 * 2 * 64, 2 * 64, 68))[0] == kvr.KVR_ERR_ALIGNMENT
+    assert _call(kvr, new_start=-1)[0] == kvr.KVR_ERR_INVALID_ARG
+
+
+def test_bytes_moved_is_linear(kvr):
+    """O(L) of PAPER.md:143: 4 * layers * kv_heads * head_dim * esz bytes per token."""
+    m, keep = kvr.model_desc(36, 8, 128, 128, 0, 0, [1.0] * 64)
+    seg = lambda n: kvr.segment(16, 16, (0, 0, 128), n, 0, 0, 0, 0)
+    assert kvr.kvr_bytes_moved(m, [seg(4096)]) == 1207959552
+    assert kvr.kvr_bytes_moved(m, [seg(1), seg(2), seg(3)]) == 6 * 294912
+    m8, keep8 = kvr.model_desc(32, 8, 128, 128, 0, 1, [1.0] * 64)
+    assert kvr.kvr_bytes_moved(m8, [seg(1)]) == 131072
+    assert kvr.kvr_bytes_moved(m, []) == 0
+
+
+def test_no_cpu_fallback(kvr):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    m, keep = kvr.model_desc(2, 2, 64, 64, 0, 0, [1.0] * 32)
+    with pytest.raises(kvr.KvrError):
+        kvr.Context(m)
+
+
+def test_status_strings(kvr):
+    names = {0: "KVR_OK", -1: "KVR_ERR_INVALID_ARG", -2: "KVR_ERR_UNSUPPORTED", -3: "KVR_ERR_ALIGNMENT",
+             -4: "KVR_ERR_OUT_OF_RANGE", -5: "KVR_ERR_CUDA", -6: "KVR_ERR_NOMEM"}
+    for k, v in names.items():
+        assert kvr.lib.kvr_status_string(k).decode() == v
+
+
+def test_product_does_not_import_oracle():
+    """The product path must never route through the oracle."""
+    pkg = os.path.join(ROOT, "paper_2606_17107_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle", text, re.M), f
+                assert "kvr_oracle" not in text, f
+    orc = open(os.path.join(ROOT, "oracle", "kvr_oracle.c")).read() + open(os.path.join(ROOT, "oracle", "kvr_oracle.py")).read()
+    assert "kvr.h" not in orc.replace("include/kvr.h)", "") and "paper_2606_17107_b200 import" not in orc
