@@ -1,6 +1,525 @@
-// kvr_ring.cu -- TMA-ring kernel (placeholder until the first GPU parity run of the generic kernel).
+// kvr_ring.cu -- the FAST reposition+splice kernel for sm_100a: a persistent, warp-specialised
+// TMA ring.  HBM-bound by construction (no contraction => no tensor cores).
+//
+//   producer warp   lane 0 walks this CTA's units (segment, chunk of <= cg destination tokens, layer
+//                   group), resolves the block-table entry (step a4), and for every tile
+//                   (layer, head group) of the unit arms an mbarrier with the byte count and issues
+//                   1-D bulk TMA loads  global -> shared  (cp.async.bulk, steps a2/a6-read) of the K
+//                   and V runs into the next ring stage, together with a 32-byte tile descriptor.
+//                   All 32 lanes evaluate the angle table  (fp64 sincos of Delta*inv_freq -> fp32
+//                   hi/lo, step a1)  into a small double-buffered shared table whenever the segment
+//                   (or, with a position map, the chunk) changes.
+//   consumer warps  each owns every NW-th tile: wait on the stage's "full" mbarrier, then
+//                   V: either one bulk TMA store  shared -> global  per destination run (head-major
+//                      pools) or 16-byte warp copies (token-major pools)             (step a6)
+//                   K: 16-byte shared loads, compensated fp32 rotation in registers with the
+//                      segment's cos/sin held in registers, 16-byte global stores to the paged slot
+//                                                                                     (steps a3, a5)
+//                   then release the stage through its "empty" mbarrier.
+//
+// Tiles are uniform, so units are dealt round-robin to the persistent CTAs (grid = SMs x CTAs/SM).
 #include "kvr_common.cuh"
+
 namespace kvr {
-bool ring_supported(const CallParams&, const SegDev*, const char** why) { if (why) *why = "not built yet"; return false; }
-cudaError_t launch_ring(const CallParams&, const RingConfig&, int, cudaStream_t, int*, int*, int*) { return cudaErrorNotSupported; }
+
+struct RingParams {
+  int S, NW, hpt, cg;
+  int rowB, nv, log_nv, sp, log_sp, rpi;  // row bytes; 16-B vectors per row; slots (vector pairs) per row; rows per warp pass
+  int nr;                                 // rotary vectors per row = rotary_dim * E / 16
+  int half_R;                             // rotary pairs per row
+  int NV;                                 // table transposition width (see tab_pos)
+  int tile_bytes;                         // K (or V) region of a stage = hpt * cg * rowB
+  int stage_bytes;                        // 2 * tile_bytes
+  int off_meta, off_scales, off_tab, tab_stride, NTB, off_stage;
+  int v_bulk;                             // V leaves shared memory by bulk stores (needs stride_token == head_dim)
+  int n_scales;                           // fp8: layers * heads destination scales preloaded to shared memory
+};
+
+struct __align__(16) TileMeta {
+  int64_t dst_off;    // element offset of (layer, block, offset-in-block, first head of the tile)
+  int32_t n_tok;
+  int32_t flags;      // bit0 DONE, bit1 ROTATE (segment mode: Delta != 0)
+  int32_t tab;        // table buffer index
+  int32_t gen;        // table generation (changes when the consumer must reload its registers)
+  int32_t scale_idx;  // layer * heads + first head
+  int32_t seg;        // segment (only read when source scales differ)
+};
+static_assert(sizeof(TileMeta) == 32, "TileMeta layout");
+
+constexpr int kFlagDone = 1, kFlagRotate = 2;
+constexpr int kMaxThreads = 32 * 17;
+
+// ------------------------------------------------------------------------------- PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+// global -> shared bulk copy (TMA, 1-D), completion signalled on an mbarrier
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+      ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+}
+// shared -> global bulk copy (TMA, 1-D), tracked by the issuing thread's bulk async-group
+__device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ float4 lds128f(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void stg128(void* p, uint4 v) {
+  asm volatile("st.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+// Position of rotary pair p inside a table row.  Transposed so that the lanes of one row read
+// consecutive 16-byte entries for the same k (bank-conflict free): p = group * PPV + k -> k * NV + group.
+template <int PPV>
+__device__ __forceinline__ int tab_pos(int p, int NV) { return (p % PPV) * NV + p / PPV; }
+
+// ------------------------------------------------------------------------------- word-level math
+template <int DTYPE, int PAIRING> struct Geo;
+template <> struct Geo<0, 0> { static constexpr int EPV = 8, PPV = 8, NT = 8; };    // bf16 NeoX : table regs = 8 pairs
+template <> struct Geo<0, 1> { static constexpr int EPV = 8, PPV = 4, NT = 8; };    // bf16 GPT-J: 4 + 4
+template <> struct Geo<1, 0> { static constexpr int EPV = 16, PPV = 16, NT = 16; }; // fp8 NeoX
+template <> struct Geo<1, 1> { static constexpr int EPV = 16, PPV = 8, NT = 16; };  // fp8 GPT-J: 8 + 8
+
+// bf16, NeoX: A = 8 "a" elements, B = the 8 partner "b" elements; T[j] belongs to element j.
+__device__ __forceinline__ void rot_bf16_neox(uint4& A, uint4& B, const float4* T) {
+  uint32_t* a = reinterpret_cast<uint32_t*>(&A);
+  uint32_t* b = reinterpret_cast<uint32_t*>(&B);
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    float ra0, rb0, ra1, rb1;
+    rotate_comp(__uint_as_float(a[w] << 16), __uint_as_float(b[w] << 16), T[2 * w], ra0, rb0);
+    rotate_comp(__uint_as_float(a[w] & 0xFFFF0000u), __uint_as_float(b[w] & 0xFFFF0000u), T[2 * w + 1], ra1, rb1);
+    a[w] = pack_bf16x2(ra0, ra1);
+    b[w] = pack_bf16x2(rb0, rb1);
+  }
+}
+// bf16, GPT-J: each 32-bit word is one pair (lo = a, hi = b); T[w] belongs to word w.
+__device__ __forceinline__ void rot_bf16_gptj(uint4& A, const float4* T) {
+  uint32_t* a = reinterpret_cast<uint32_t*>(&A);
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    float ra, rb;
+    rotate_comp(__uint_as_float(a[w] << 16), __uint_as_float(a[w] & 0xFFFF0000u), T[w], ra, rb);
+    a[w] = pack_bf16x2(ra, rb);
+  }
+}
+// fp8, NeoX: A = 16 "a" codes, B = 16 "b" codes; T[j] = (cos, sin) of element j.
+__device__ __forceinline__ void rot_fp8_neox(uint4& A, uint4& B, const float2* T, float s_src, float inv_dst, bool rot) {
+  uint32_t* a = reinterpret_cast<uint32_t*>(&A);
+  uint32_t* b = reinterpret_cast<uint32_t*>(&B);
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    float2 a01 = e4m3x2_to_f32x2(a[w] & 0xFFFFu), a23 = e4m3x2_to_f32x2(a[w] >> 16);
+    float2 b01 = e4m3x2_to_f32x2(b[w] & 0xFFFFu), b23 = e4m3x2_to_f32x2(b[w] >> 16);
+    float av[4] = {a01.x, a01.y, a23.x, a23.y}, bv[4] = {b01.x, b01.y, b23.x, b23.y};
+    float ra[4], rb[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      float2 cs = rot ? T[4 * w + j] : make_float2(1.0f, 0.0f);
+      rotate_plain(__fmul_rn(av[j], s_src), __fmul_rn(bv[j], s_src), cs.x, cs.y, ra[j], rb[j]);
+      ra[j] = __fmul_rn(ra[j], inv_dst);
+      rb[j] = __fmul_rn(rb[j], inv_dst);
+    }
+    a[w] = f32x2_to_e4m3x2_sat(ra[0], ra[1]) | (f32x2_to_e4m3x2_sat(ra[2], ra[3]) << 16);
+    b[w] = f32x2_to_e4m3x2_sat(rb[0], rb[1]) | (f32x2_to_e4m3x2_sat(rb[2], rb[3]) << 16);
+  }
+}
+// fp8, GPT-J: word w = codes (a, b, a, b) of pairs 2w, 2w+1.
+__device__ __forceinline__ void rot_fp8_gptj(uint4& A, const float2* T, float s_src, float inv_dst, bool rot) {
+  uint32_t* a = reinterpret_cast<uint32_t*>(&A);
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    float2 p0 = e4m3x2_to_f32x2(a[w] & 0xFFFFu), p1 = e4m3x2_to_f32x2(a[w] >> 16);
+    float2 c0 = rot ? T[2 * w] : make_float2(1.0f, 0.0f), c1 = rot ? T[2 * w + 1] : make_float2(1.0f, 0.0f);
+    float ra0, rb0, ra1, rb1;
+    rotate_plain(__fmul_rn(p0.x, s_src), __fmul_rn(p0.y, s_src), c0.x, c0.y, ra0, rb0);
+    rotate_plain(__fmul_rn(p1.x, s_src), __fmul_rn(p1.y, s_src), c1.x, c1.y, ra1, rb1);
+    a[w] = f32x2_to_e4m3x2_sat(__fmul_rn(ra0, inv_dst), __fmul_rn(rb0, inv_dst)) |
+           (f32x2_to_e4m3x2_sat(__fmul_rn(ra1, inv_dst), __fmul_rn(rb1, inv_dst)) << 16);
+  }
+}
+// fp8 pass-through vector under a scale change: requantise every code
+__device__ __forceinline__ void requant_fp8(uint4& A, float s_src, float inv_dst) {
+  uint32_t* a = reinterpret_cast<uint32_t*>(&A);
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    float2 p0 = e4m3x2_to_f32x2(a[w] & 0xFFFFu), p1 = e4m3x2_to_f32x2(a[w] >> 16);
+    a[w] = f32x2_to_e4m3x2_sat(__fmul_rn(__fmul_rn(p0.x, s_src), inv_dst), __fmul_rn(__fmul_rn(p0.y, s_src), inv_dst)) |
+           (f32x2_to_e4m3x2_sat(__fmul_rn(__fmul_rn(p1.x, s_src), inv_dst), __fmul_rn(__fmul_rn(p1.y, s_src), inv_dst)) << 16);
+  }
+}
+
+// ------------------------------------------------------------------------------- the kernel
+template <int DTYPE, int PAIRING, bool MAP>
+__global__ void __launch_bounds__(kMaxThreads, 1)
+kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ RingParams RP) {
+  using G = Geo<DTYPE, PAIRING>;
+  constexpr int E = (DTYPE == 0) ? 2 : 1;
+  extern __shared__ __align__(128) unsigned char smem[];
+  const uint32_t s_base = smem_u32(smem);
+  const uint32_t s_full = s_base, s_empty = s_base + 8u * RP.S;
+  TileMeta* meta = reinterpret_cast<TileMeta*>(smem + RP.off_meta);
+  float* s_scales = reinterpret_cast<float*>(smem + RP.off_scales);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int S = RP.S, NW = RP.NW;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < S; ++s) { mbar_init(s_full + 8u * s, 1); mbar_init(s_empty + 8u * s, 1); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (DTYPE == 1)
+    for (int i = threadIdx.x; i < RP.n_scales; i += blockDim.x) s_scales[i] = P.k_scale_dst[i];
+  __syncthreads();
+
+  if (warp == NW) {
+    // =========================================================================== PRODUCER
+    const uint64_t pol = policy_evict_first();
+    int64_t i = 0;                 // tiles issued by this CTA
+    int tb = 0, gen = 0;           // current table buffer / generation
+    int64_t cur_key = -1;          // segment (segment mode) or unit (map mode) the current table belongs to
+    int64_t last_use[4] = {-1, -1, -1, -1};
+    const int hgroups = P.heads / RP.hpt;
+
+    for (int64_t unit = blockIdx.x; unit < P.total_units; unit += gridDim.x) {
+      const int si = find_segment(P.segs, P.n_segs, unit);
+      const SegDev& sg = P.segs[si];
+      const int64_t local = unit - sg.unit_begin;
+      const int n_chunks = sg.n_chunks;
+      const int lg = (int)(local / n_chunks);
+      const int c = (int)(local % n_chunks);
+      const Chunk ch = chunk_of(sg, c, RP.cg, P.block_size);
+      const int32_t blk = P.block_table[(int64_t)sg.dst_seq * P.max_blocks + ch.blk_index];
+      if (blk < 0 || blk >= P.num_blocks) {
+        if (lane == 0) report_bad_block(P.status, sg.index, ch.t0);
+        continue;
+      }
+      const int32_t delta_seg = sg.delta;
+      const int32_t* pos_map = sg.pos_map;
+      const bool seg_map = MAP;   // a position-map launch builds per-token rows for every segment
+      // ---- angle table (step a1) ----
+      const int64_t key = seg_map ? (unit | ((int64_t)1 << 62)) : (int64_t)si;
+      if (key != cur_key) {
+        const int nb = (tb + 1) % RP.NTB;
+        if (lane == 0 && last_use[nb] >= 0 && last_use[nb] > i - 1 - S) {
+          const int64_t q = last_use[nb];   // still possibly in flight: wait until its stage was released
+          mbar_wait(s_empty + 8u * (uint32_t)(q % S), (uint32_t)((q / S) & 1));
+        }
+        __syncwarp();
+        float4* tab = reinterpret_cast<float4*>(smem + RP.off_tab + nb * RP.tab_stride);
+        const int rows = seg_map ? ch.n_tok : 1;
+        for (int idx = lane; idx < rows * RP.half_R; idx += 32) {
+          const int t = idx / RP.half_R, p = idx % RP.half_R;
+          const int64_t delta = (seg_map && pos_map) ? (int64_t)pos_map[ch.t0 + t] - ((int64_t)sg.old_start + ch.t0 + t)
+                                                     : (int64_t)delta_seg;
+          tab[t * RP.half_R + tab_pos<G::PPV>(p, RP.NV)] = angle_entry(delta, P.inv_freq[p]);
+          if (MAP && p == 0)
+            reinterpret_cast<int32_t*>(tab + RP.cg * RP.half_R)[t] = (delta == 0);
+        }
+        __syncwarp();
+        tb = nb; gen += 1; cur_key = key;
+      }
+      if (lane == 0) {
+        const int l0 = lg * P.lpu, l1 = min(P.layers, l0 + P.lpu);
+        const int flags = (seg_map || delta_seg != 0) ? kFlagRotate : 0;
+        const uint32_t run_bytes = (uint32_t)(ch.n_tok * RP.rowB);
+        const bool packed_rows = (sg.st == P.head_dim);
+        const int64_t dst_chunk = (int64_t)blk * P.d_sb + (int64_t)ch.off * P.d_st;
+        for (int l = l0; l < l1; ++l) {
+          for (int hg = 0; hg < hgroups; ++hg) {
+            const int stage = (int)(i % S);
+            const uint32_t bar = s_full + 8u * stage;
+            mbar_wait(s_empty + 8u * stage, (uint32_t)(((i / S) & 1) ^ 1));
+            const int h0 = hg * RP.hpt;
+            TileMeta m;
+            m.dst_off = (int64_t)l * P.d_sl + dst_chunk + (int64_t)h0 * P.d_sh;
+            m.n_tok = ch.n_tok; m.flags = flags; m.tab = tb; m.gen = gen;
+            m.scale_idx = l * P.heads + h0; m.seg = si;
+            meta[stage] = m;
+            mbar_arrive_expect_tx(bar, 2u * RP.hpt * run_bytes);
+            const uint32_t sk = s_base + RP.off_stage + (uint32_t)stage * RP.stage_bytes;
+            const uint32_t sv = sk + RP.tile_bytes;
+            for (int hh = 0; hh < RP.hpt; ++hh) {
+              const int64_t src_off = ((int64_t)l * sg.sl + (int64_t)(h0 + hh) * sg.sh + (int64_t)ch.t0 * sg.st) * E;
+              const uint32_t so = (uint32_t)(hh * RP.cg * RP.rowB);
+              if (packed_rows) {
+                bulk_g2s(sk + so, sg.k_src + src_off, run_bytes, bar, pol);
+                bulk_g2s(sv + so, sg.v_src + src_off, run_bytes, bar, pol);
+              } else {
+                for (int t = 0; t < ch.n_tok; ++t) {
+                  bulk_g2s(sk + so + t * RP.rowB, sg.k_src + src_off + (int64_t)t * sg.st * E, RP.rowB, bar, pol);
+                  bulk_g2s(sv + so + t * RP.rowB, sg.v_src + src_off + (int64_t)t * sg.st * E, RP.rowB, bar, pol);
+                }
+              }
+            }
+            last_use[tb] = i;
+            ++i;
+          }
+        }
+      }
+      i = __shfl_sync(0xFFFFFFFFu, i, 0);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) last_use[k] = __shfl_sync(0xFFFFFFFFu, last_use[k], 0);
+    }
+    // one DONE tile per consumer warp, through the same ring
+    if (lane == 0) {
+      for (int w = 0; w < NW; ++w) {
+        const int stage = (int)(i % S);
+        mbar_wait(s_empty + 8u * stage, (uint32_t)(((i / S) & 1) ^ 1));
+        TileMeta m{};
+        m.flags = kFlagDone;
+        meta[stage] = m;
+        mbar_arrive(s_full + 8u * stage);
+        ++i;
+      }
+    }
+    return;
+  }
+
+  // ============================================================================= CONSUMERS
+  const int sp = RP.sp, q = lane & (sp - 1), rsub = lane >> RP.log_sp, rpi = RP.rpi;
+  const int nv = RP.nv, nr = RP.nr;
+  // this lane's slot: two 16-byte vectors (va, vb) of every row it visits
+  int va, vb;
+  bool rot_a, rot_b;
+  int tpos[G::NT];               // table positions of this lane's pairs (only used if rotary)
+  if (PAIRING == 0) {
+    const int half = nr >> 1;
+    if (q < half) { va = q; vb = q + half; rot_a = rot_b = true; }
+    else { va = nr + 2 * (q - half); vb = va + 1; rot_a = rot_b = false; }
+#pragma unroll
+    for (int k = 0; k < G::NT; ++k) tpos[k] = rot_a ? tab_pos<G::PPV>(va * G::EPV + k, RP.NV) : 0;
+  } else {
+    va = q; vb = q + (nv >> 1);
+    rot_a = va < nr; rot_b = vb < nr;
+#pragma unroll
+    for (int k = 0; k < G::NT; ++k) {
+      const int v = (k < G::PPV) ? va : vb;
+      const bool r = (k < G::PPV) ? rot_a : rot_b;
+      tpos[k] = r ? tab_pos<G::PPV>(v * G::PPV + (k % G::PPV), RP.NV) : 0;
+    }
+  }
+  float4 T4[DTYPE == 0 ? G::NT : 1];
+  float2 T2[DTYPE == 1 ? G::NT : 1];
+  int my_gen = -1;
+  const bool dst_rows_packed = (P.d_st == P.head_dim);
+
+  for (int64_t i = warp;; i += NW) {
+    const int stage = (int)(i % S);
+    mbar_wait(s_full + 8u * stage, (uint32_t)((i / S) & 1));
+    const TileMeta m = meta[stage];
+    if (m.flags & kFlagDone) break;
+    const uint32_t sk = s_base + RP.off_stage + (uint32_t)stage * RP.stage_bytes;
+    const uint32_t sv = sk + RP.tile_bytes;
+    const int n_tok = m.n_tok;
+
+    // ---- V (step a6): bytes unchanged ----
+    if (RP.v_bulk) {
+      if (lane == 0) {
+        for (int hh = 0; hh < RP.hpt; ++hh)
+          bulk_s2g(P.v_cache + (m.dst_off + (int64_t)hh * P.d_sh) * E, sv + hh * RP.cg * RP.rowB, (uint32_t)(n_tok * RP.rowB));
+        bulk_commit();
+      }
+    } else {
+      for (int hh = 0; hh < RP.hpt; ++hh) {
+        const uint32_t vs = sv + hh * RP.cg * RP.rowB;
+        uint8_t* vd = P.v_cache + (m.dst_off + (int64_t)hh * P.d_sh) * E;
+        const int total = n_tok * nv;
+#pragma unroll 4
+        for (int idx = lane; idx < total; idx += 32) {
+          const int t = idx >> RP.log_nv, v = idx & (nv - 1);
+          stg128(vd + (int64_t)t * P.d_st * E + v * 16, lds128(vs + idx * 16));
+        }
+      }
+    }
+
+    // ---- K (steps a3, a5) ----
+    const uint32_t tab = s_base + RP.off_tab + m.tab * RP.tab_stride;
+    const bool rotate = (m.flags & kFlagRotate) != 0;
+    if (!MAP && rotate && m.gen != my_gen) {       // new segment: refresh the cos/sin registers
+      my_gen = m.gen;
+      if (rot_a || rot_b) {
+#pragma unroll
+        for (int k = 0; k < G::NT; ++k) {
+          float4 e = lds128f(tab + tpos[k] * 16);
+          if (DTYPE == 0) T4[k] = e; else T2[k] = make_float2(e.x, e.z);
+        }
+      }
+    }
+    for (int hh = 0; hh < RP.hpt; ++hh) {
+      const uint32_t ks = sk + hh * RP.cg * RP.rowB;
+      uint8_t* kd = P.k_cache + (m.dst_off + (int64_t)hh * P.d_sh) * E;
+      float s_src = 1.0f, inv_dst = 1.0f;
+      bool requant = false;
+      if (DTYPE == 1) {
+        const float s_dst = s_scales[m.scale_idx + hh];
+        s_src = P.scales_differ ? P.segs[m.seg].k_scale_src[m.scale_idx + hh] : s_dst;
+        requant = (s_src != s_dst);
+        inv_dst = __frcp_rn(s_dst);
+      }
+      for (int t = rsub; t < n_tok; t += rpi) {
+        uint4 A = lds128(ks + t * RP.rowB + va * 16);
+        uint4 B = lds128(ks + t * RP.rowB + vb * 16);
+        bool rot_row = rotate;
+        if (MAP) {
+          rot_row = reinterpret_cast<const int32_t*>(smem + RP.off_tab + m.tab * RP.tab_stride + RP.cg * RP.half_R * 16)[t] == 0;
+          if (rot_row && (rot_a || rot_b)) {
+            const uint32_t trow = tab + t * RP.half_R * 16;
+#pragma unroll
+            for (int k = 0; k < G::NT; ++k) {
+              float4 e = lds128f(trow + tpos[k] * 16);
+              if (DTYPE == 0) T4[k] = e; else T2[k] = make_float2(e.x, e.z);
+            }
+          }
+        }
+        if constexpr (DTYPE == 0) {
+          if (rot_row) {
+            if constexpr (PAIRING == 0) { if (rot_a) rot_bf16_neox(A, B, T4); }
+            else { if (rot_a) rot_bf16_gptj(A, T4); if (rot_b) rot_bf16_gptj(B, T4 + G::PPV); }
+          }
+        } else if (rot_row || requant) {
+          if constexpr (PAIRING == 0) {
+            if (rot_a) rot_fp8_neox(A, B, T2, s_src, inv_dst, rot_row);
+            else if (requant) { requant_fp8(A, s_src, inv_dst); requant_fp8(B, s_src, inv_dst); }
+          } else {
+            if (rot_a) rot_fp8_gptj(A, T2, s_src, inv_dst, rot_row); else if (requant) requant_fp8(A, s_src, inv_dst);
+            if (rot_b) rot_fp8_gptj(B, T2 + G::PPV, s_src, inv_dst, rot_row); else if (requant) requant_fp8(B, s_src, inv_dst);
+          }
+        }
+        uint8_t* row = kd + (int64_t)t * P.d_st * E;
+        stg128(row + va * 16, A);
+        stg128(row + vb * 16, B);
+      }
+    }
+    if (RP.v_bulk && lane == 0) bulk_wait_read0();   // V bytes have left shared memory
+    __syncwarp();
+    if (lane == 0) mbar_arrive(s_empty + 8u * stage);
+  }
+  if (RP.v_bulk && lane == 0) bulk_wait_all0();
+  (void)dst_rows_packed;
+}
+
+// ------------------------------------------------------------------------------- host side
+static int ilog2(int x) { int l = 0; while ((1 << l) < x) ++l; return l; }
+
+bool ring_supported(const CallParams& P, const SegDev* segs, const char** why) {
+  const int E = P.dtype == 0 ? 2 : 1;
+  const int rowB = P.head_dim * E;
+  const char* w = nullptr;
+  if (rowB < 32 || rowB > 1024 || (rowB & (rowB - 1))) w = "head_dim*esz must be a power of two in [32, 1024] bytes";
+  else if (P.pairing == 0 && (P.rotary_dim * E) % 32) w = "NeoX pairing needs rotary_dim*esz % 32 == 0";
+  else if (P.pairing == 1 && (P.rotary_dim * E) % 16) w = "GPT-J pairing needs rotary_dim*esz % 16 == 0";
+  else if (P.dtype == 1 && (int64_t)P.layers * P.heads > 8192) w = "too many (layer, head) scales for shared memory";
+  else if (P.rotary_dim / 2 > 512) w = "rotary_dim too large for the shared angle table";
+  (void)segs;
+  if (why) *why = w;
+  return w == nullptr;
+}
+
+template <int DTYPE, int PAIRING, bool MAP>
+static cudaError_t launch_inst(const CallParams& P, const RingParams& RP, int grid, int block, int smem, cudaStream_t st) {
+  static int configured = 0;   // per instantiation
+  if (configured < smem) {
+    cudaError_t e = cudaFuncSetAttribute(kvr_ring_kernel<DTYPE, PAIRING, MAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    configured = smem;
+  }
+  kvr_ring_kernel<DTYPE, PAIRING, MAP><<<grid, block, smem, st>>>(P, RP);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_ring(const CallParams& P, const RingConfig& cfg, int sm_count, cudaStream_t stream,
+                        int* grid_out, int* block_out, int* smem_out) {
+  const int E = P.dtype == 0 ? 2 : 1;
+  RingParams RP{};
+  RP.cg = P.cg;
+  RP.rowB = P.head_dim * E;
+  RP.nv = RP.rowB / 16; RP.log_nv = ilog2(RP.nv);
+  RP.sp = RP.nv / 2; RP.log_sp = ilog2(RP.sp); RP.rpi = 32 / RP.sp;
+  RP.nr = P.rotary_dim * E / 16;
+  RP.half_R = P.rotary_dim / 2;
+  const int ppv = (P.pairing == 0) ? 16 / E : 8 / E;
+  RP.NV = RP.half_R / ppv;
+  // heads per tile: smallest divisor of heads whose K run reaches 4 KB
+  int hpt = P.heads;
+  for (int h = 1; h <= P.heads; ++h)
+    if (P.heads % h == 0 && h * RP.cg * RP.rowB >= 4096) { hpt = h; break; }
+  RP.hpt = hpt;
+  RP.tile_bytes = hpt * RP.cg * RP.rowB;
+  RP.stage_bytes = 2 * RP.tile_bytes;
+  const int ctas = cfg.ctas_per_sm > 0 ? cfg.ctas_per_sm : 2;
+  RP.NW = cfg.consumer_warps > 0 ? cfg.consumer_warps : 6;
+  if (RP.NW > 16) RP.NW = 16;
+  RP.NTB = 2;
+  const int tab_rows = P.any_pos_map ? RP.cg : 1;
+  RP.tab_stride = ((tab_rows * RP.half_R * 16 + RP.cg * 4) + 127) & ~127;
+  RP.n_scales = P.dtype == 1 ? P.layers * P.heads : 0;
+  const int budget = (227 * 1024) / ctas - 1024;          // per-CTA dynamic shared memory (1 KB reserved per CTA)
+  auto layout = [&](int S) {
+    int off = 16 * S;
+    off = (off + 31) & ~31; RP.off_meta = off; off += 32 * S;
+    off = (off + 15) & ~15; RP.off_scales = off; off += 4 * RP.n_scales;
+    off = (off + 127) & ~127; RP.off_tab = off; off += RP.NTB * RP.tab_stride;
+    off = (off + 127) & ~127; RP.off_stage = off; off += S * RP.stage_bytes;
+    return off;
+  };
+  int S = cfg.stages > 0 ? cfg.stages : 64;
+  while (S > 2 && layout(S) > budget) --S;
+  if (layout(S) > budget) return cudaErrorInvalidConfiguration;
+  if (S < RP.NW) RP.NW = S;                                // every consumer warp needs a stage to wait on
+  RP.S = S;
+  const int smem = layout(S);
+  RP.v_bulk = cfg.v_bulk_store == 1 ? 1 : (cfg.v_bulk_store == 2 ? 0 : (P.d_st == P.head_dim ? 1 : 0));
+  if (P.d_st != P.head_dim) RP.v_bulk = 0;                 // bulk V stores need one contiguous run per (head, chunk)
+  int64_t g = (int64_t)sm_count * ctas;
+  if (g > P.total_units) g = P.total_units;
+  if (g < 1) g = 1;
+  const int block = (RP.NW + 1) * 32;
+  *grid_out = (int)g; *block_out = block; *smem_out = smem;
+  const bool map = P.any_pos_map != 0;
+#define KVR_LAUNCH(D, PR, M) return launch_inst<D, PR, M>(P, RP, (int)g, block, smem, stream)
+  if (P.dtype == 0) {
+    if (P.pairing == 0) { if (map) KVR_LAUNCH(0, 0, true); else KVR_LAUNCH(0, 0, false); }
+    else { if (map) KVR_LAUNCH(0, 1, true); else KVR_LAUNCH(0, 1, false); }
+  } else {
+    if (P.pairing == 0) { if (map) KVR_LAUNCH(1, 0, true); else KVR_LAUNCH(1, 0, false); }
+    else { if (map) KVR_LAUNCH(1, 1, true); else KVR_LAUNCH(1, 1, false); }
+  }
+#undef KVR_LAUNCH
+}
+
 }  // namespace kvr
