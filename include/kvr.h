@@ -113,7 +113,8 @@ typedef struct {
   int32_t stages;          /* ring depth (tiles in flight per CTA)                             */
   int32_t layers_per_unit; /* layers one scheduled unit covers                                  */
   int32_t v_bulk_store;    /* 0 auto, 1 V leaves shared memory by bulk (TMA) stores, 2 by warps */
-  int32_t reserved[10];
+  int32_t max_ctas;        /* cap on the persistent grid (tests use it to force many tiles per CTA)  */
+  int32_t reserved[9];
 } kvr_tuning;
 
 /* Creates a context on CUDA device `cuda_device` (must be compute capability 10.x).  Allocates a few

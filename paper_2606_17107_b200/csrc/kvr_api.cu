@@ -313,7 +313,7 @@ kvr_status kvr_reposition_splice(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   KVR_CUDA(c, cudaMemcpyAsync(slot.dev, slot.host, (size_t)n * sizeof(SegDev), cudaMemcpyHostToDevice, stream));
   cudaError_t e;
   if (path == 2) {
-    RingConfig rc{tu.ctas_per_sm, tu.consumer_warps, tu.stages, tu.v_bulk_store};
+    RingConfig rc{tu.ctas_per_sm, tu.consumer_warps, tu.stages, tu.v_bulk_store, tu.max_ctas};
     e = launch_ring(P, rc, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
   } else {
     e = launch_generic(P, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);

@@ -145,7 +145,7 @@ __device__ __forceinline__ uint32_t f32x2_to_e4m3x2_sat(float lo, float hi) {
 cudaError_t launch_generic(const CallParams& P, int sm_count, cudaStream_t stream, int* grid, int* block, int* smem);
 
 struct RingConfig {
-  int ctas_per_sm, consumer_warps, stages, v_bulk_store;
+  int ctas_per_sm, consumer_warps, stages, v_bulk_store, max_ctas;
 };
 bool ring_supported(const CallParams& P, const SegDev* host_segs, const char** why);
 cudaError_t launch_ring(const CallParams& P, const RingConfig& cfg, int sm_count, cudaStream_t stream,

@@ -18,6 +18,8 @@
 //                   then release the stage through its "empty" mbarrier.
 //
 // Tiles are uniform, so units are dealt round-robin to the persistent CTAs (grid = SMs x CTAs/SM).
+#include <cstdio>
+
 #include "kvr_common.cuh"
 
 namespace kvr {
@@ -61,14 +63,29 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t byt
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
-      "WAIT_%=:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-      "@p bra DONE_%=;\n\t"
-      "bra WAIT_%=;\n\t"
-      "DONE_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
+// Bounded wait: a protocol bug must surface as a trapped launch (an error the caller sees), never as a hung GPU.
+#ifndef KVR_WATCHDOG_CYCLES
+#define KVR_WATCHDOG_CYCLES (20ll * 1000 * 1000 * 1000)   /* ~10 s */
+#endif
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int who = 0) {
+  if (mbar_try_wait(bar, parity)) return;
+  const long long t0 = clock64();
+  while (!mbar_try_wait(bar, parity)) {
+    if (clock64() - t0 > KVR_WATCHDOG_CYCLES) {
+#ifdef KVR_WATCHDOG_PRINT
+      printf("kvr watchdog: cta %d thread %d who %d bar_off %u parity %u\n", blockIdx.x, threadIdx.x, who, bar, parity);
+#endif
+      __trap();
+    }
+  }
 }
 __device__ __forceinline__ uint64_t policy_evict_first() {
   uint64_t p;
@@ -209,103 +226,134 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
   if (warp == NW) {
     // =========================================================================== PRODUCER
     const uint64_t pol = policy_evict_first();
-    int64_t i = 0;                 // tiles issued by this CTA
+    uint32_t i = 0;                // tiles issued by this CTA; (stage, phase) of the next one
+    int stage = 0;
+    uint32_t phase = 0;
     int tb = 0, gen = 0;           // current table buffer / generation
     int64_t cur_key = -1;          // segment (segment mode) or unit (map mode) the current table belongs to
-    int64_t last_use[4] = {-1, -1, -1, -1};
+    uint32_t lu_i[2] = {0, 0}, lu_phase[2] = {0, 0};   // last tile that used each table buffer
+    int lu_stage[2] = {0, 0};
+    bool lu_valid[2] = {false, false};
+    int cur_si = -1;
+    SegDev sg{};                   // current segment, held in registers
     const int hgroups = P.heads / RP.hpt;
+    const unsigned FULL = 0xFFFFFFFFu;
 
-    for (int64_t unit = blockIdx.x; unit < P.total_units; unit += gridDim.x) {
-      const int si = find_segment(P.segs, P.n_segs, unit);
-      const SegDev& sg = P.segs[si];
-      const int64_t local = unit - sg.unit_begin;
-      const int n_chunks = sg.n_chunks;
-      const int lg = (int)(local / n_chunks);
-      const int c = (int)(local % n_chunks);
-      const Chunk ch = chunk_of(sg, c, RP.cg, P.block_size);
-      const int32_t blk = P.block_table[(int64_t)sg.dst_seq * P.max_blocks + ch.blk_index];
-      if (blk < 0 || blk >= P.num_blocks) {
-        if (lane == 0) report_bad_block(P.status, sg.index, ch.t0);
-        continue;
+    for (int64_t base = blockIdx.x; base < P.total_units; base += (int64_t)gridDim.x * 32) {
+      // ---- batch decode: lane j resolves unit base + j*grid (segment, chunk, block-table entry: step a4),
+      //      so the dependent global loads are paid once per 32 units, off the per-tile path ----
+      const int64_t my_unit = base + (int64_t)lane * gridDim.x;
+      int d_si = -1, d_t0 = 0, d_ntok = 0, d_off = 0, d_lg = 0, d_blk = -1;
+      if (my_unit < P.total_units) {
+        d_si = find_segment(P.segs, P.n_segs, my_unit);
+        const SegDev* s = P.segs + d_si;
+        const int64_t local = my_unit - s->unit_begin;
+        const int n_chunks = s->n_chunks;
+        d_lg = (int)(local / n_chunks);
+        const int c = (int)(local - (int64_t)d_lg * n_chunks);
+        const Chunk ch = chunk_of(*s, c, RP.cg, P.block_size);
+        d_t0 = ch.t0; d_ntok = ch.n_tok; d_off = ch.off;
+        d_blk = P.block_table[(int64_t)s->dst_seq * P.max_blocks + ch.blk_index];
       }
-      const int32_t delta_seg = sg.delta;
-      const int32_t* pos_map = sg.pos_map;
-      const bool seg_map = MAP;   // a position-map launch builds per-token rows for every segment
-      // ---- angle table (step a1) ----
-      const int64_t key = seg_map ? (unit | ((int64_t)1 << 62)) : (int64_t)si;
-      if (key != cur_key) {
-        const int nb = (tb + 1) % RP.NTB;
-        if (lane == 0 && last_use[nb] >= 0 && last_use[nb] > i - 1 - S) {
-          const int64_t q = last_use[nb];   // still possibly in flight: wait until its stage was released
-          mbar_wait(s_empty + 8u * (uint32_t)(q % S), (uint32_t)((q / S) & 1));
+      for (int j = 0; j < 32; ++j) {
+        const int si = __shfl_sync(FULL, d_si, j);
+        if (si < 0) break;
+        const int t0 = __shfl_sync(FULL, d_t0, j), n_tok = __shfl_sync(FULL, d_ntok, j);
+        const int off = __shfl_sync(FULL, d_off, j), lg = __shfl_sync(FULL, d_lg, j);
+        const int blk = __shfl_sync(FULL, d_blk, j);
+        if (si != cur_si) { sg = P.segs[si]; cur_si = si; }
+        if (blk < 0 || blk >= P.num_blocks) {
+          if (lane == 0) report_bad_block(P.status, sg.index, t0);
+          continue;
         }
-        __syncwarp();
-        float4* tab = reinterpret_cast<float4*>(smem + RP.off_tab + nb * RP.tab_stride);
-        const int rows = seg_map ? ch.n_tok : 1;
-        for (int idx = lane; idx < rows * RP.half_R; idx += 32) {
-          const int t = idx / RP.half_R, p = idx % RP.half_R;
-          const int64_t delta = (seg_map && pos_map) ? (int64_t)pos_map[ch.t0 + t] - ((int64_t)sg.old_start + ch.t0 + t)
-                                                     : (int64_t)delta_seg;
-          tab[t * RP.half_R + tab_pos<G::PPV>(p, RP.NV)] = angle_entry(delta, P.inv_freq[p]);
-          if (MAP && p == 0)
-            reinterpret_cast<int32_t*>(tab + RP.cg * RP.half_R)[t] = (delta == 0);
+        // ---- angle table (step a1) ----
+        const int64_t key = MAP ? (base + (int64_t)j * gridDim.x) : (int64_t)si;
+        if (key != cur_key) {
+          const int nb = tb ^ 1;
+          if (lane == 0 && (nb ? lu_valid[1] : lu_valid[0]) && (nb ? lu_i[1] : lu_i[0]) + (uint32_t)S >= i)   // tiles <= i-1-S are known released
+            mbar_wait(s_empty + 8u * (nb ? lu_stage[1] : lu_stage[0]), nb ? lu_phase[1] : lu_phase[0], 1);   // its last reader may still be in flight
+          __syncwarp();
+          float4* tab = reinterpret_cast<float4*>(smem + RP.off_tab + nb * RP.tab_stride);
+          const int rows = MAP ? n_tok : 1;
+          for (int idx = lane; idx < rows * RP.half_R; idx += 32) {
+            const int t = idx / RP.half_R, p = idx - t * RP.half_R;
+            const int64_t delta = (MAP && sg.pos_map)
+                                      ? (int64_t)sg.pos_map[t0 + t] - ((int64_t)sg.old_start + t0 + t)
+                                      : (int64_t)sg.delta;
+            tab[t * RP.half_R + tab_pos<G::PPV>(p, RP.NV)] = angle_entry(delta, P.inv_freq[p]);
+            if (MAP && p == 0) reinterpret_cast<int32_t*>(tab + RP.cg * RP.half_R)[t] = (delta == 0);
+          }
+          __syncwarp();
+          tb = nb; gen += 1; cur_key = key;
         }
-        __syncwarp();
-        tb = nb; gen += 1; cur_key = key;
-      }
-      if (lane == 0) {
-        const int l0 = lg * P.lpu, l1 = min(P.layers, l0 + P.lpu);
-        const int flags = (seg_map || delta_seg != 0) ? kFlagRotate : 0;
-        const uint32_t run_bytes = (uint32_t)(ch.n_tok * RP.rowB);
-        const bool packed_rows = (sg.st == P.head_dim);
-        const int64_t dst_chunk = (int64_t)blk * P.d_sb + (int64_t)ch.off * P.d_st;
-        for (int l = l0; l < l1; ++l) {
-          for (int hg = 0; hg < hgroups; ++hg) {
-            const int stage = (int)(i % S);
-            const uint32_t bar = s_full + 8u * stage;
-            mbar_wait(s_empty + 8u * stage, (uint32_t)(((i / S) & 1) ^ 1));
-            const int h0 = hg * RP.hpt;
-            TileMeta m;
-            m.dst_off = (int64_t)l * P.d_sl + dst_chunk + (int64_t)h0 * P.d_sh;
-            m.n_tok = ch.n_tok; m.flags = flags; m.tab = tb; m.gen = gen;
-            m.scale_idx = l * P.heads + h0; m.seg = si;
-            meta[stage] = m;
-            mbar_arrive_expect_tx(bar, 2u * RP.hpt * run_bytes);
-            const uint32_t sk = s_base + RP.off_stage + (uint32_t)stage * RP.stage_bytes;
-            const uint32_t sv = sk + RP.tile_bytes;
-            for (int hh = 0; hh < RP.hpt; ++hh) {
-              const int64_t src_off = ((int64_t)l * sg.sl + (int64_t)(h0 + hh) * sg.sh + (int64_t)ch.t0 * sg.st) * E;
-              const uint32_t so = (uint32_t)(hh * RP.cg * RP.rowB);
-              if (packed_rows) {
-                bulk_g2s(sk + so, sg.k_src + src_off, run_bytes, bar, pol);
-                bulk_g2s(sv + so, sg.v_src + src_off, run_bytes, bar, pol);
-              } else {
-                for (int t = 0; t < ch.n_tok; ++t) {
-                  bulk_g2s(sk + so + t * RP.rowB, sg.k_src + src_off + (int64_t)t * sg.st * E, RP.rowB, bar, pol);
-                  bulk_g2s(sv + so + t * RP.rowB, sg.v_src + src_off + (int64_t)t * sg.st * E, RP.rowB, bar, pol);
+        {
+          // ---- tile issue (steps a2 / a6-read): lane t takes tile t of the unit, so up to min(32, S) tiles are
+          //      armed and issued per pass instead of one (a single thread needs ~1k cycles per tile) ----
+          const int l0 = lg * P.lpu, l1 = min(P.layers, l0 + P.lpu);
+          const int n_tiles = (l1 - l0) * hgroups;
+          const int flags = (MAP || sg.delta != 0) ? kFlagRotate : 0;
+          const uint32_t run_bytes = (uint32_t)(n_tok * RP.rowB);
+          const bool packed_rows = (sg.st == P.head_dim);
+          const int64_t dst_chunk = (int64_t)blk * P.d_sb + (int64_t)off * P.d_st;
+          const int64_t src_chunk = (int64_t)t0 * sg.st;
+          const int pass = S < 32 ? S : 32;
+          for (int tb0 = 0; tb0 < n_tiles; tb0 += pass) {
+            const int n = min(pass, n_tiles - tb0);
+            if (lane < n) {
+              const int t = tb0 + lane;
+              const int l = l0 + t / hgroups, h0 = (t % hgroups) * RP.hpt;
+              int my_stage = stage + lane;
+              uint32_t my_phase = phase;
+              if (my_stage >= S) { my_stage -= S; my_phase ^= 1u; }
+              const uint32_t bar = s_full + 8u * my_stage;
+              mbar_wait(s_empty + 8u * my_stage, my_phase ^ 1u, 2);
+              TileMeta m;
+              m.dst_off = (int64_t)l * P.d_sl + dst_chunk + (int64_t)h0 * P.d_sh;
+              m.n_tok = n_tok; m.flags = flags; m.tab = tb; m.gen = gen;
+              m.scale_idx = l * P.heads + h0; m.seg = si;
+              meta[my_stage] = m;
+              mbar_arrive_expect_tx(bar, 2u * RP.hpt * run_bytes);
+              const uint32_t sk = s_base + RP.off_stage + (uint32_t)my_stage * RP.stage_bytes;
+              const uint32_t sv = sk + RP.tile_bytes;
+              for (int hh = 0; hh < RP.hpt; ++hh) {
+                const int64_t src_off = ((int64_t)l * sg.sl + (int64_t)(h0 + hh) * sg.sh + src_chunk) * E;
+                const uint32_t so = (uint32_t)(hh * RP.cg * RP.rowB);
+                if (packed_rows) {
+                  bulk_g2s(sk + so, sg.k_src + src_off, run_bytes, bar, pol);
+                  bulk_g2s(sv + so, sg.v_src + src_off, run_bytes, bar, pol);
+                } else {
+                  for (int r = 0; r < n_tok; ++r) {
+                    bulk_g2s(sk + so + r * RP.rowB, sg.k_src + src_off + (int64_t)r * sg.st * E, RP.rowB, bar, pol);
+                    bulk_g2s(sv + so + r * RP.rowB, sg.v_src + src_off + (int64_t)r * sg.st * E, RP.rowB, bar, pol);
+                  }
                 }
               }
             }
-            last_use[tb] = i;
-            ++i;
+            __syncwarp();
+            i += (uint32_t)n;
+            stage += n;
+            if (stage >= S) { stage -= S; phase ^= 1u; }
+          }
+          // the unit's last tile is the last reader of table buffer tb
+          if (n_tiles > 0) {
+            const int ls = (stage == 0) ? S - 1 : stage - 1;
+            const uint32_t lp = (stage == 0) ? (phase ^ 1u) : phase;
+            if (tb) { lu_i[1] = i - 1u; lu_stage[1] = ls; lu_phase[1] = lp; lu_valid[1] = true; }
+            else { lu_i[0] = i - 1u; lu_stage[0] = ls; lu_phase[0] = lp; lu_valid[0] = true; }
           }
         }
       }
-      i = __shfl_sync(0xFFFFFFFFu, i, 0);
-#pragma unroll
-      for (int k = 0; k < 4; ++k) last_use[k] = __shfl_sync(0xFFFFFFFFu, last_use[k], 0);
     }
-    // one DONE tile per consumer warp, through the same ring
-    if (lane == 0) {
-      for (int w = 0; w < NW; ++w) {
-        const int stage = (int)(i % S);
-        mbar_wait(s_empty + 8u * stage, (uint32_t)(((i / S) & 1) ^ 1));
-        TileMeta m{};
-        m.flags = kFlagDone;
-        meta[stage] = m;
-        mbar_arrive(s_full + 8u * stage);
-        ++i;
-      }
+    // one DONE tile per consumer warp, through the same ring (NW <= S, so the stages are distinct)
+    if (lane < NW) {
+      int my_stage = stage + lane;
+      uint32_t my_phase = phase;
+      if (my_stage >= S) { my_stage -= S; my_phase ^= 1u; }
+      mbar_wait(s_empty + 8u * my_stage, my_phase ^ 1u, 3);
+      TileMeta m{};
+      m.flags = kFlagDone;
+      meta[my_stage] = m;
+      mbar_arrive(s_full + 8u * my_stage);
     }
     return;
   }
@@ -338,9 +386,10 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
   int my_gen = -1;
   const bool dst_rows_packed = (P.d_st == P.head_dim);
 
-  for (int64_t i = warp;; i += NW) {
-    const int stage = (int)(i % S);
-    mbar_wait(s_full + 8u * stage, (uint32_t)((i / S) & 1));
+  int stage = warp % S;
+  uint32_t phase = (uint32_t)(warp / S) & 1u;
+  for (;; ) {
+    mbar_wait(s_full + 8u * stage, phase, 4);
     const TileMeta m = meta[stage];
     if (m.flags & kFlagDone) break;
     const uint32_t sk = s_base + RP.off_stage + (uint32_t)stage * RP.stage_bytes;
@@ -428,6 +477,8 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     if (RP.v_bulk && lane == 0) bulk_wait_read0();   // V bytes have left shared memory
     __syncwarp();
     if (lane == 0) mbar_arrive(s_empty + 8u * stage);
+    stage += NW;
+    if (stage >= S) { stage -= S; phase ^= 1u; }
   }
   if (RP.v_bulk && lane == 0) bulk_wait_all0();
   (void)dst_rows_packed;
@@ -484,7 +535,7 @@ cudaError_t launch_ring(const CallParams& P, const RingConfig& cfg, int sm_count
   const int ctas = cfg.ctas_per_sm > 0 ? cfg.ctas_per_sm : 2;
   RP.NW = cfg.consumer_warps > 0 ? cfg.consumer_warps : 6;
   if (RP.NW > 16) RP.NW = 16;
-  RP.NTB = 2;
+  RP.NTB = 2;                                              // the producer's bookkeeping assumes two
   const int tab_rows = P.any_pos_map ? RP.cg : 1;
   RP.tab_stride = ((tab_rows * RP.half_R * 16 + RP.cg * 4) + 127) & ~127;
   RP.n_scales = P.dtype == 1 ? P.layers * P.heads : 0;
@@ -500,12 +551,15 @@ cudaError_t launch_ring(const CallParams& P, const RingConfig& cfg, int sm_count
   int S = cfg.stages > 0 ? cfg.stages : 64;
   while (S > 2 && layout(S) > budget) --S;
   if (layout(S) > budget) return cudaErrorInvalidConfiguration;
-  if (S < RP.NW) RP.NW = S;                                // every consumer warp needs a stage to wait on
+  if (S < RP.NW) RP.NW = S;
+  S -= S % RP.NW;   // stage s is always served by consumer warp s % NW: successive phases of one mbarrier are then
+                    // ordered by one warp's program order (a warp two phases ahead would pass a parity wait early)
   RP.S = S;
   const int smem = layout(S);
   RP.v_bulk = cfg.v_bulk_store == 1 ? 1 : (cfg.v_bulk_store == 2 ? 0 : (P.d_st == P.head_dim ? 1 : 0));
   if (P.d_st != P.head_dim) RP.v_bulk = 0;                 // bulk V stores need one contiguous run per (head, chunk)
   int64_t g = (int64_t)sm_count * ctas;
+  if (cfg.max_ctas > 0 && g > cfg.max_ctas) g = cfg.max_ctas;
   if (g > P.total_units) g = P.total_units;
   if (g < 1) g = 1;
   const int block = (RP.NW + 1) * 32;

@@ -64,6 +64,19 @@ def test_small_configs(c, layout, path):
         assert np.mean(d == 0) > 0.95          # almost every element is the correctly rounded fp64 result
 
 
+@pytest.mark.parametrize("tuning", [dict(max_ctas=3, stages=2, consumer_warps=1),
+                                    dict(max_ctas=2, stages=7, consumer_warps=3),
+                                    dict(max_ctas=5, stages=13, consumer_warps=6),
+                                    dict(max_ctas=4, stages=64, consumer_warps=16, ctas_per_sm=1),
+                                    dict(max_ctas=1, stages=4, consumer_warps=4, layers_per_unit=1)])
+@pytest.mark.parametrize("c", [1, 2, 3, 4])
+def test_ring_wraps_many_times_per_cta(c, tuning):
+    """A handful of persistent CTAs each stream hundreds of tiles through a short ring: exercises mbarrier
+    phase wrap-around, stage ownership, table-buffer reuse and the DONE hand-shake."""
+    w = config_small(c, "NHD" if c % 2 else "HND")
+    check_parity(w, "ring", **tuning)
+
+
 @pytest.mark.parametrize("path", ["generic", "ring"])
 @pytest.mark.parametrize("layout", ["NHD", "HND"])
 @pytest.mark.parametrize("pairing,D,R,dtype", [("neox", 32, 32, "bf16"), ("gptj", 32, 16, "bf16"),
