@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""bench.py -- KV tokens repositioned+spliced per second on B200 (BASELINE.json `metric`).
+
+A "step" is one pass of the whole hot path (SURVEY.md 8(a) a1..a6 = one kvr_reposition_splice call) over one
+BASELINE.json configuration of synthetic seeded input.  Default workload: configs[1] (Qwen3-8B-shaped, bf16,
+one 4096-token skill at new_start = 2000); `--config c` times another one with the same JSON contract.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c] [--impl kvr|reference]
+
+* value      whole-job KV tokens/s, inputs resident in HBM, timed with CUDA events on the launching stream,
+             barrier + synchronize on both sides, max over ranks (N > 1: independent replicas, "weak").
+* roofline   algorithmic bytes (4 * layers*kv_heads*head_dim*esz per KV token) / measured launch time
+             against MEASURED_PEAKS.json `hbm_gbs` (the measured copy bandwidth of this pool's B200s).
+* e2e        the same metric through kvr_reposition_splice_host: sources in pinned HOST memory, the
+             host->device copies and the device->host read of the status word inside the timed region.
+* cpu_baseline  the fp64 oracle (oracle/, as it stands) on this box's host cores over a bounded sample.
+* --impl reference  times the oracle alone (rank 0 only), same metric/config, JSON line with "impl": "reference".
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "KV tokens repositioned+spliced/sec"
+UNIT = "KV tokens/s"
+FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback ("of fallback")
+CACHE_DTYPE = {"bf16": "bf16", "fp8": "fp8-e4m3"}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from one `ncu --set full`
+# capture of the bench command (profiles/, named per round); None until a capture of that config exists.
+NCU_TRAFFIC_BYTES = {}
+try:
+    with open(os.path.join(ROOT, "profiles", "traffic.txt")) as _f:     # lines: "<workload name> <bytes> <source file>"
+        for _line in _f:
+            _p = _line.split()
+            if len(_p) >= 2 and not _line.startswith("#"):
+                NCU_TRAFFIC_BYTES[_p[0]] = int(_p[1])
+except OSError:
+    pass
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--layout", default="NHD", choices=["NHD", "HND"])
+    ap.add_argument("--impl", default="kvr", choices=["kvr", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=None)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--tune", default="", help="kvr_tuning overrides, e.g. ctas_per_sm=1,stages=12")
+    return ap.parse_args()
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except (OSError, KeyError, ValueError):
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# --------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+    BAD = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20}
+    NOTE = {"sw_power_cap": 0x4}
+
+    def __init__(self, torch_device):
+        self.samples, self.reasons, self.max_mhz, self._stop, self._h = [], 0, None, threading.Event(), None
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            uuid = str(torch.cuda.get_device_properties(torch_device).uuid)
+            try:
+                self._h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + uuid) if not uuid.startswith("GPU-") else uuid)
+            except Exception:
+                self._h = pynvml.nvmlDeviceGetHandleByIndex(torch.device(torch_device).index or 0)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:      # noqa: BLE001 -- no NVML: the clocks object says so
+            self.error = repr(e)
+
+    def sample(self):
+        if self._h is None:
+            return
+        try:
+            self.samples.append(int(self._nv.nvmlDeviceGetClockInfo(self._h, self._nv.NVML_CLOCK_SM)))
+            self.reasons |= int(self._nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+        except Exception:           # noqa: BLE001
+            pass
+
+    def _run(self):
+        while not self._stop.is_set():
+            self.sample()
+            time.sleep(0.003)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable: " + getattr(self, "error", "no samples")]}
+        s = sorted(self.samples)
+        names = [n for n, bit in {**self.BAD, **self.NOTE}.items() if self.reasons & bit]
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": names, "samples": len(s)}
+
+
+# --------------------------------------------------------------------------------------- oracle timing
+def _oracle_sample(c, layout, k_steps_total, get_sources, cpu_work_target_s=15.0, wall_cap_s=120.0):
+    """Times the oracle, as it stands, on a bounded sample of config c: the first `ls` layers of every segment
+    (every head, token and element of them).  Returns (seconds per step over the sample, ls, layers, threads,
+    run_step) where run_step() performs one sample pass.  The sample is sized from one calibration layer so that
+    a step is ~cpu_work_target_s of CPU work and k_steps_total steps stay under wall_cap_s."""
+    import numpy as np
+    from oracle import kvr_oracle as orc
+    from workloads import SENTINEL_BF16, SENTINEL_FP8, config
+    threads = orc.host_threads()
+    full = config(c, layout)
+
+    def make(ls):
+        w = config(c, layout, layers=ls)
+        srcs = get_sources(w, ls)
+        edt = np.uint16 if w.dtype == "bf16" else np.uint8
+        kc = np.full(w.pool_elems(), SENTINEL_BF16 if w.dtype == "bf16" else SENTINEL_FP8, dtype=edt)
+        vc = kc.copy()
+        return w, srcs, kc, vc
+
+    w1, s1, kc, vc = make(1)
+    t0 = time.perf_counter()
+    orc.splice_workload(w1, s1, kc, vc, n_threads=threads)
+    per_layer = time.perf_counter() - t0
+    per_step_target = min(cpu_work_target_s / threads, wall_cap_s / max(1, k_steps_total))
+    ls = int(max(1, min(full.layers, per_step_target / max(per_layer, 1e-9))))
+    ls = max(ls, min(full.layers, -(-threads // full.kv_heads)))     # enough (layer, head) units for every thread
+    threads = min(threads, ls * full.kv_heads)                       # the OpenMP loop runs over (layer, head)
+    w, srcs, kc, vc = (w1, s1, kc, vc) if ls == 1 else make(ls)
+
+    def run_step():
+        t = time.perf_counter()
+        orc.splice_workload(w, srcs, kc, vc, n_threads=threads)
+        return time.perf_counter() - t
+
+    return ls, full.layers, threads, run_step, full
+
+
+def cpu_sources_from_device(dw):
+    from paper_2606_17107_b200.harness import bits_to_numpy
+
+    def get(w, ls):
+        return [(bits_to_numpy(k[:ls]), bits_to_numpy(v[:ls])) for k, v in dw.sources]
+    return get
+
+
+def cpu_sources_fresh():
+    def get(w, ls):
+        from paper_2606_17107_b200.harness import bits_to_numpy
+        from workloads import make_sources
+        return [(bits_to_numpy(k), bits_to_numpy(v)) for k, v in make_sources(w, "cpu")]
+    return get
+
+
+def time_oracle(c, layout, steps, warmup, get_sources):
+    ls, layers, threads, run_step, full = _oracle_sample(c, layout, steps + warmup, get_sources)
+    for _ in range(warmup):
+        run_step()
+    ts = [run_step() for _ in range(steps)]
+    per_step = sum(ts) / len(ts)
+    # a KV token spans all layers: the sample covers ls of `layers`, cost is linear in layers (O(L))
+    tokens_per_s = full.tokens / (per_step * layers / ls)
+    sample = (f"layers 0..{ls - 1} of {layers} (all heads, all {full.tokens} tokens, every element) per step, "
+              f"{steps} step(s) after {warmup} warm-up, scaled linearly to {layers} layers")
+    return tokens_per_s, per_step, threads, sample, full
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    steps = args.steps if args.steps is not None else 5
+    warmup = args.warmup if args.warmup is not None else 1
+    value, per_step, threads, sample, full = time_oracle(args.config, args.layout, steps, warmup, cpu_sources_fresh())
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": warmup, "ms_per_step": per_step * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": full.name, "config_index": args.config, "layout": args.layout,
+                   "cache_dtype": CACHE_DTYPE[full.dtype], "tokens": full.tokens},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# --------------------------------------------------------------------------------------- the kvr arm
+def run_kvr(args):
+    import torch
+    from paper_2606_17107_b200 import kvr
+    from paper_2606_17107_b200.harness import DeviceWorkload
+    from paper_2606_17107_b200.replicas import Replicas, aggregate_throughput
+    from workloads import config
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the kvr path has no CPU fallback")
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    device = torch.device("cuda", local_rank)
+    torch.cuda.set_device(device)
+    rep = Replicas(backend="nccl", device=device)
+    steps = args.steps if args.steps is not None else 1000
+    warmup = max(3, args.warmup if args.warmup is not None else 50)
+
+    w = config(args.config, args.layout)
+    dw = DeviceWorkload(w, device)
+    tokens, bytes_per_step = w.tokens, dw.bytes_moved()
+    stream = torch.cuda.Stream(device=device)
+    ctx = kvr.Context(dw.model, device=local_rank)
+    if args.tune:
+        ctx.set_tuning(**{k: int(v) for k, v in (kv.split("=") for kv in args.tune.split(","))})
+
+    # ---- device-resident timing ----
+    for _ in range(warmup):
+        dw.run(ctx, stream=stream)
+    st = ctx.last_device_status()
+    assert st[0] == kvr.KVR_OK, st
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(device)
+    torch.cuda.synchronize(device)
+    rep.barrier()
+    launches0 = ctx.launch_count()
+    with sampler:
+        ev0.record(stream)
+        for _ in range(steps):
+            dw.run(ctx, stream=stream)
+        ev1.record(stream)
+        sampler.sample()                       # the queue is still draining: a sample under load even for short runs
+        torch.cuda.synchronize(device)
+    rep.barrier()
+    launches = ctx.launch_count() - launches0
+    seconds = ev0.elapsed_time(ev1) * 1e-3
+    agg = aggregate_throughput(rep, tokens * steps, seconds)
+    info = ctx.last_launch_info()
+    clocks = sampler.summary()
+    peak, peak_src = measured_peak()
+    achieved = bytes_per_step / (seconds / steps) / 1e9      # this rank's kernel: one launch per step
+
+    # ---- end to end: sources in pinned host memory, through kvr_reposition_splice_host ----
+    e2e = None
+    if not args.no_e2e:
+        dw.make_host_sources()
+        e2e_steps = args.e2e_steps if args.e2e_steps is not None else max(3, min(20, steps))
+        for _ in range(2):
+            dw.run_host(ctx, stream=stream)
+            assert ctx.last_device_status()[0] == kvr.KVR_OK
+        h2d = ctx.last_h2d_bytes() + len(dw.host_segs) * 96 * max(1, (w.layers + 3) // 4)
+        torch.cuda.synchronize(device)
+        rep.barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            dw.run_host(ctx, stream=stream)
+            st = ctx.last_device_status()      # device -> host read of the step's result (status word), syncs
+            assert st[0] == kvr.KVR_OK, st
+        torch.cuda.synchronize(device)
+        e2e_seconds = time.perf_counter() - t0
+        rep.barrier()
+        e_agg = aggregate_throughput(rep, tokens * e2e_steps, e2e_seconds)
+        e2e = {"value": e_agg["per_second"], "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": 16,
+               "steps": e2e_steps, "ms_per_step": e_agg["seconds"] / e2e_steps * 1e3,
+               "api": "kvr_reposition_splice_host (pinned host K/V sources -> staged H2D overlapped with the kernel) "
+                      "+ kvr_last_device_status"}
+
+    # ---- oracle on the host cores (rank 0, N = 1 only) ----
+    cpu = None
+    if rep.world == 1 and not args.no_cpu_baseline:
+        v, per_step, threads, sample, _ = time_oracle(args.config, args.layout, 1, 0, cpu_sources_from_device(dw))
+        cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample}
+
+    ctx.close()
+    if rep.rank == 0:
+        line = {
+            "metric": METRIC, "value": agg["per_second"], "unit": UNIT, "n_gpus": rep.world, "steps": steps,
+            "warmup": warmup, "ms_per_step": agg["seconds"] / steps * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "config_index": args.config, "layout": args.layout,
+                       "cache_dtype": CACHE_DTYPE[w.dtype], "tokens": tokens, "segments": len(w.segments),
+                       "bytes_per_step": bytes_per_step, "parallelism": f"replicas x{rep.world}",
+                       "l2": f"inputs larger than L2 ({bytes_per_step // 2} B of sources + as many pool bytes "
+                             "per step vs 126 MB L2); no flush",
+                       "kernel": {1: "kvr_generic_kernel", 2: "kvr_ring_kernel"}.get(info["path"], "?"),
+                       "grid": info["grid"], "block": info["block"], "smem": info["smem"]},
+            "gpu_launches": launches,
+            "clocks": clocks,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": NCU_TRAFFIC_BYTES.get(w.name), "peak_source": peak_src,
+                         "gb_s_of_nominal_8000": achieved / 8000.0},
+            "e2e": e2e,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line), flush=True)
+    rep.close()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_kvr(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

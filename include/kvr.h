@@ -136,6 +136,20 @@ KVR_API kvr_status kvr_validate(const kvr_model_desc* model, const kvr_paged_dst
 KVR_API kvr_status kvr_reposition_splice(kvr_ctx* ctx, const kvr_paged_dst* dst, const kvr_segment* segs,
                                          int32_t n_segs, void* cuda_stream);
 
+/* The same operation with HOST-resident sources (a library of precompiled skills kept in host RAM,
+ * PAPER.md:131 "we precompile a long skill", :393 "prefilled once in isolation"): every segment's k_src,
+ * v_src, pos_map and k_scale_src are HOST pointers; dst (pools, block_table, k_scale) stays DEVICE memory.
+ * Sources must be dense [layers][kv_heads][len][head_dim] (else KVR_ERR_UNSUPPORTED) and should be pinned
+ * (cudaHostAlloc / cudaHostRegister); pageable memory works but makes the copies synchronous.  The library
+ * stages groups of layers through two context-owned device buffers (allocated on first use, <= ~256 MB
+ * each, or one layer if that is larger): the host->device copies of group g+1 run on a context-owned copy
+ * stream while the kernel of group g runs on `cuda_stream`.  Returns when everything is enqueued; the host
+ * buffers must stay valid and unchanged until `cuda_stream` has passed this call.  Not capturable in a CUDA
+ * graph.  kvr_last_h2d_bytes reports the bytes the last such call copied host -> device. */
+KVR_API kvr_status kvr_reposition_splice_host(kvr_ctx* ctx, const kvr_paged_dst* dst, const kvr_segment* segs,
+                                              int32_t n_segs, void* cuda_stream);
+KVR_API uint64_t kvr_last_h2d_bytes(const kvr_ctx* ctx);
+
 /* Algorithmic bytes of a call: read K, read V, write K, write V = 4 * layers*kv_heads*head_dim*esz * sum(len).
  * This is the O(L) of PAPER.md:143 and the numerator of every GB/s this repository reports. */
 KVR_API uint64_t kvr_bytes_moved(const kvr_model_desc* model, const kvr_segment* segs, int32_t n_segs);

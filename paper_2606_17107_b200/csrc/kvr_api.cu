@@ -13,7 +13,8 @@ using namespace kvr;
 
 namespace {
 
-constexpr int kSlots = 8;           // descriptor staging ring (calls in flight per context)
+constexpr int kSlots = 16;          // descriptor staging ring (launches in flight per context)
+constexpr int kStageBufs = 2;       // host-source path: device staging buffers (copy of group g+1 overlaps kernel g)
 constexpr int kInitialSegCap = 256;
 
 struct Slot {
@@ -97,6 +98,17 @@ struct kvr_ctx {
   int last_path = 0, last_grid = 0, last_block = 0, last_smem = 0;
   cudaStream_t last_stream = nullptr;
   std::string last_err;
+  // host-source path (kvr_reposition_splice_host)
+  cudaStream_t copy_stream = nullptr;
+  uint8_t* stage[kStageBufs] = {nullptr, nullptr};
+  size_t stage_cap = 0;
+  cudaEvent_t stage_filled[kStageBufs] = {nullptr, nullptr};   // recorded on copy_stream
+  cudaEvent_t stage_drained[kStageBufs] = {nullptr, nullptr};  // recorded on the caller's stream
+  bool stage_drained_valid[kStageBufs] = {false, false};
+  cudaEvent_t fork_ev = nullptr;
+  void* aux_dev = nullptr;            // pos_map / k_scale_src copies
+  size_t aux_cap = 0;
+  uint64_t h2d_bytes = 0;             // bytes the last host-source call copied host -> device
 
   kvr_status cuda_fail(cudaError_t e, const char* what) {
     last_err = std::string(what) + ": " + cudaGetErrorString(e);
@@ -178,6 +190,14 @@ kvr_status kvr_destroy(kvr_ctx* c) {
     if (s.dev) cudaFree(s.dev);
     if (s.ev) cudaEventDestroy(s.ev);
   }
+  for (int b = 0; b < kStageBufs; ++b) {
+    if (c->stage[b]) cudaFree(c->stage[b]);
+    if (c->stage_filled[b]) cudaEventDestroy(c->stage_filled[b]);
+    if (c->stage_drained[b]) cudaEventDestroy(c->stage_drained[b]);
+  }
+  if (c->fork_ev) cudaEventDestroy(c->fork_ev);
+  if (c->aux_dev) cudaFree(c->aux_dev);
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->d_inv_freq) cudaFree(c->d_inv_freq);
   if (c->d_status) cudaFree(c->d_status);
   if (c->h_status) cudaFreeHost(c->h_status);
@@ -206,23 +226,14 @@ uint64_t kvr_bytes_moved(const kvr_model_desc* m, const kvr_segment* segs, int32
          (uint64_t)elt_bytes(m->dtype) * tokens;
 }
 
-kvr_status kvr_reposition_splice(kvr_ctx* c, const kvr_paged_dst* d, const kvr_segment* segs, int32_t n,
-                                 void* cuda_stream) {
-  if (!c) return KVR_ERR_INVALID_ARG;
-  c->last_err.clear();
-  kvr_status st = check_call(&c->model, d, segs, n);
-  if (st != KVR_OK) return st;
-  if (n == 0) return KVR_OK;
-  for (int32_t i = 0; i < n; ++i) {
-    int64_t delta = (int64_t)segs[i].new_start - (int64_t)segs[i].old_start;
-    if (!segs[i].pos_map && (delta > INT32_MAX || delta < INT32_MIN)) return KVR_ERR_INVALID_ARG;
-  }
-  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-  int prev = 0;
-  cudaGetDevice(&prev);
-  if (prev != c->device) KVR_CUDA(c, cudaSetDevice(c->device));
-  struct Restore { int prev, cur; ~Restore() { if (prev != cur) cudaSetDevice(prev); } } restore{prev, c->device};
+}  // extern "C"
 
+// One launch over layers [l0, l0 + nl) of the model.  All segment pointers are DEVICE pointers.  The
+// destination, its scales and the source scales are advanced to layer l0; the K/V sources are advanced too
+// unless `src_group_local` (the host-source path stages exactly the group's layers at layer index 0).
+static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_segment* segs, int32_t n,
+                                 cudaStream_t stream, int l0, int nl, bool src_group_local) {
+  kvr_status st = KVR_OK;
   cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
   KVR_CUDA(c, cudaStreamIsCapturing(stream, &cap));
   const bool capturing = cap != cudaStreamCaptureStatusNone;
@@ -239,13 +250,17 @@ kvr_status kvr_reposition_splice(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     if (st != KVR_OK) return st;
   }
 
-  const kvr_model_desc& m = c->model;
+  kvr_model_desc m = c->model;
+  m.layers = nl;
+  const int E = elt_bytes(m.dtype);
   CallParams P{};
   P.layers = m.layers; P.heads = m.kv_heads; P.head_dim = m.head_dim; P.rotary_dim = m.rotary_dim;
   P.pairing = m.pairing; P.dtype = m.dtype; P.inv_freq = c->d_inv_freq;
-  P.k_cache = static_cast<uint8_t*>(d->k_cache); P.v_cache = static_cast<uint8_t*>(d->v_cache);
+  P.k_cache = static_cast<uint8_t*>(d->k_cache) + (int64_t)l0 * d->stride_layer * E;
+  P.v_cache = static_cast<uint8_t*>(d->v_cache) + (int64_t)l0 * d->stride_layer * E;
   P.d_sl = d->stride_layer; P.d_sb = d->stride_block; P.d_st = d->stride_token; P.d_sh = d->stride_head;
-  P.block_table = d->block_table; P.k_scale_dst = d->k_scale;
+  P.block_table = d->block_table;
+  P.k_scale_dst = d->k_scale ? d->k_scale + (int64_t)l0 * m.kv_heads : nullptr;
   P.num_blocks = d->num_blocks; P.block_size = d->block_size; P.num_seqs = d->num_seqs;
   P.max_blocks = d->max_blocks_per_seq;
   P.segs = slot.dev; P.n_segs = n; P.status = c->d_status;
@@ -264,9 +279,12 @@ kvr_status kvr_reposition_splice(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     for (int32_t i = 0; i < n; ++i) {
       const kvr_segment& s = segs[i];
       SegDev& o = slot.host[i];
-      o.k_src = static_cast<const uint8_t*>(s.k_src); o.v_src = static_cast<const uint8_t*>(s.v_src);
+      const int64_t src_adv = src_group_local ? 0 : (int64_t)l0 * s.src_stride_layer * E;
+      o.k_src = static_cast<const uint8_t*>(s.k_src) + src_adv;
+      o.v_src = static_cast<const uint8_t*>(s.v_src) + src_adv;
       o.pos_map = s.pos_map;
       o.k_scale_src = s.k_scale_src ? s.k_scale_src : d->k_scale;
+      if (o.k_scale_src) o.k_scale_src += (int64_t)l0 * m.kv_heads;
       o.sl = s.src_stride_layer; o.sh = s.src_stride_head; o.st = s.src_stride_token;
       o.len = s.len; o.old_start = s.old_start; o.delta = (int32_t)((int64_t)s.new_start - s.old_start);
       o.dst_seq = s.dst_seq; o.dst_token_start = s.dst_token_start;
@@ -328,6 +346,148 @@ kvr_status kvr_reposition_splice(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   }
   return KVR_OK;
 }
+
+static kvr_status check_deltas(const kvr_segment* segs, int32_t n) {
+  for (int32_t i = 0; i < n; ++i) {
+    int64_t delta = (int64_t)segs[i].new_start - (int64_t)segs[i].old_start;
+    if (!segs[i].pos_map && (delta > INT32_MAX || delta < INT32_MIN)) return KVR_ERR_INVALID_ARG;
+  }
+  return KVR_OK;
+}
+
+struct DeviceGuard {
+  int prev = 0, cur = 0;
+  explicit DeviceGuard(int dev) : cur(dev) { cudaGetDevice(&prev); if (prev != cur) cudaSetDevice(cur); }
+  ~DeviceGuard() { if (prev != cur) cudaSetDevice(prev); }
+};
+
+extern "C" {
+
+kvr_status kvr_reposition_splice(kvr_ctx* c, const kvr_paged_dst* d, const kvr_segment* segs, int32_t n,
+                                 void* cuda_stream) {
+  if (!c) return KVR_ERR_INVALID_ARG;
+  c->last_err.clear();
+  kvr_status st = check_call(&c->model, d, segs, n);
+  if (st != KVR_OK) return st;
+  if (n == 0) return KVR_OK;
+  if ((st = check_deltas(segs, n)) != KVR_OK) return st;
+  DeviceGuard guard(c->device);
+  return enqueue_layers(c, d, segs, n, static_cast<cudaStream_t>(cuda_stream), 0, c->model.layers, false);
+}
+
+// Host-resident sources (a skill library kept in host RAM): stage layer groups through two context-owned device
+// buffers; the H2D copies of group g+1 run on the context's copy stream while the kernel of group g runs on the
+// caller's stream.  No arithmetic happens on the host: the staged bytes go through the same kernels.
+kvr_status kvr_reposition_splice_host(kvr_ctx* c, const kvr_paged_dst* d, const kvr_segment* segs, int32_t n,
+                                      void* cuda_stream) {
+  if (!c) return KVR_ERR_INVALID_ARG;
+  c->last_err.clear();
+  c->h2d_bytes = 0;
+  const kvr_model_desc& m = c->model;
+  const int E = elt_bytes(m.dtype);
+  // validate with stand-in device addresses for the host pointers (alignment rules are the same)
+  kvr_status st = check_call(&m, d, segs, n);
+  if (st != KVR_OK) return st;
+  if (n == 0) return KVR_OK;
+  if ((st = check_deltas(segs, n)) != KVR_OK) return st;
+  int64_t tokens = 0;
+  size_t aux_need = 0;
+  for (int32_t i = 0; i < n; ++i) {
+    const kvr_segment& s = segs[i];
+    // host sources must be dense [layers][kv_heads][len][head_dim] so that a layer group is one contiguous run
+    if (s.src_stride_token != m.head_dim || s.src_stride_head != (int64_t)s.len * m.head_dim ||
+        s.src_stride_layer != (int64_t)m.kv_heads * s.len * m.head_dim)
+      return KVR_ERR_UNSUPPORTED;
+    tokens += s.len;
+    if (s.pos_map) aux_need += (((size_t)s.len * 4) + 15) & ~(size_t)15;
+    if (s.k_scale_src) aux_need += (((size_t)m.layers * m.kv_heads * 4) + 15) & ~(size_t)15;
+  }
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  DeviceGuard guard(c->device);
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  KVR_CUDA(c, cudaStreamIsCapturing(stream, &cap));
+  if (cap != cudaStreamCaptureStatusNone) return KVR_ERR_UNSUPPORTED;   // allocates and uses a second stream
+
+  // ---- layer-group size: staging buffer of <= ~256 MB, at least one layer ----
+  const size_t layer_bytes = 2u * (size_t)tokens * m.kv_heads * m.head_dim * E;   // K + V of one layer, all segments
+  int lg = (int)((256ull << 20) / (layer_bytes ? layer_bytes : 1));
+  if (lg < 1) lg = 1;
+  if (lg > m.layers) lg = m.layers;
+  if (m.layers >= 4 && lg > m.layers / 4) lg = m.layers / 4;                        // keep >= 4 groups so copy and kernel overlap
+  const size_t need = (size_t)lg * layer_bytes;
+  if (need > c->stage_cap) {
+    KVR_CUDA(c, cudaDeviceSynchronize());
+    for (int b = 0; b < kStageBufs; ++b) { if (c->stage[b]) cudaFree(c->stage[b]); c->stage[b] = nullptr; }
+    c->stage_cap = 0;
+    for (int b = 0; b < kStageBufs; ++b) KVR_CUDA(c, cudaMalloc(&c->stage[b], need));
+    c->stage_cap = need;
+    c->stage_drained_valid[0] = c->stage_drained_valid[1] = false;
+  }
+  if (aux_need > c->aux_cap) {
+    KVR_CUDA(c, cudaDeviceSynchronize());
+    if (c->aux_dev) cudaFree(c->aux_dev);
+    c->aux_dev = nullptr; c->aux_cap = 0;
+    KVR_CUDA(c, cudaMalloc(&c->aux_dev, aux_need));
+    c->aux_cap = aux_need;
+  }
+  if (!c->copy_stream) {
+    KVR_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    for (int b = 0; b < kStageBufs; ++b) {
+      KVR_CUDA(c, cudaEventCreateWithFlags(&c->stage_filled[b], cudaEventDisableTiming));
+      KVR_CUDA(c, cudaEventCreateWithFlags(&c->stage_drained[b], cudaEventDisableTiming));
+    }
+    KVR_CUDA(c, cudaEventCreateWithFlags(&c->fork_ev, cudaEventDisableTiming));
+  }
+  // the copy stream starts after everything already enqueued on the caller's stream
+  KVR_CUDA(c, cudaEventRecord(c->fork_ev, stream));
+  KVR_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->fork_ev, 0));
+
+  // ---- per-token maps and source scales: small, copied once ----
+  std::vector<kvr_segment> dsegs(segs, segs + n);
+  {
+    uint8_t* at = static_cast<uint8_t*>(c->aux_dev);
+    for (int32_t i = 0; i < n; ++i) {
+      if (segs[i].pos_map) {
+        const size_t b = (size_t)segs[i].len * 4;
+        KVR_CUDA(c, cudaMemcpyAsync(at, segs[i].pos_map, b, cudaMemcpyHostToDevice, c->copy_stream));
+        dsegs[i].pos_map = reinterpret_cast<const int32_t*>(at);
+        at += (b + 15) & ~(size_t)15; c->h2d_bytes += b;
+      }
+      if (segs[i].k_scale_src) {
+        const size_t b = (size_t)m.layers * m.kv_heads * 4;
+        KVR_CUDA(c, cudaMemcpyAsync(at, segs[i].k_scale_src, b, cudaMemcpyHostToDevice, c->copy_stream));
+        dsegs[i].k_scale_src = reinterpret_cast<const float*>(at);
+        at += (b + 15) & ~(size_t)15; c->h2d_bytes += b;
+      }
+    }
+  }
+  int g = 0;
+  for (int l0 = 0; l0 < m.layers; l0 += lg, ++g) {
+    const int nl = (m.layers - l0 < lg) ? (m.layers - l0) : lg;
+    const int b = g % kStageBufs;
+    if (c->stage_drained_valid[b]) KVR_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->stage_drained[b], 0));
+    uint8_t* at = c->stage[b];
+    for (int32_t i = 0; i < n; ++i) {
+      const kvr_segment& s = segs[i];
+      const size_t run = (size_t)nl * s.src_stride_layer * E;
+      const size_t off = (size_t)l0 * s.src_stride_layer * E;
+      KVR_CUDA(c, cudaMemcpyAsync(at, static_cast<const uint8_t*>(s.k_src) + off, run, cudaMemcpyHostToDevice, c->copy_stream));
+      dsegs[i].k_src = at; at += run;
+      KVR_CUDA(c, cudaMemcpyAsync(at, static_cast<const uint8_t*>(s.v_src) + off, run, cudaMemcpyHostToDevice, c->copy_stream));
+      dsegs[i].v_src = at; at += run;
+      c->h2d_bytes += 2 * run;
+    }
+    KVR_CUDA(c, cudaEventRecord(c->stage_filled[b], c->copy_stream));
+    KVR_CUDA(c, cudaStreamWaitEvent(stream, c->stage_filled[b], 0));
+    st = enqueue_layers(c, d, dsegs.data(), n, stream, l0, nl, true);
+    if (st != KVR_OK) return st;
+    KVR_CUDA(c, cudaEventRecord(c->stage_drained[b], stream));
+    c->stage_drained_valid[b] = true;
+  }
+  return KVR_OK;
+}
+
+uint64_t kvr_last_h2d_bytes(const kvr_ctx* c) { return c ? c->h2d_bytes : 0; }
 
 kvr_status kvr_last_device_status(kvr_ctx* c, int32_t* bad_segment, int32_t* bad_token) {
   if (!c) return KVR_ERR_INVALID_ARG;

@@ -56,3 +56,27 @@ class DeviceWorkload:
 
     def run(self, ctx, stream=None, dst=None):
         return ctx.reposition_splice(dst if dst is not None else self.dst, self.segs, stream=stream)
+
+    # ---- host-resident sources (kvr_reposition_splice_host) ----
+    def make_host_sources(self):
+        """Pinned host copies of the sources, position maps and source scales, and the segment array that
+        points at them.  Dense [layers][heads][len][dim] only (the host entry point requires it)."""
+        w = self.w
+        assert all(s.src_row_pad == 0 for s in w.segments)
+        self.host_sources = [(k.cpu().pin_memory(), v.cpu().pin_memory()) for k, v in self.sources]
+        self.host_pos_maps = [None if pm is None else pm.cpu().pin_memory() for pm in self.pos_maps]
+        self.host_k_scale_src = None if self.k_scale_src is None else self.k_scale_src.cpu().pin_memory()
+        self.host_segs = kvr.segment_array([
+            kvr.segment(k, v, w.src_strides(s), s.len, s.old_start, s.new_start, s.dst_seq, s.dst_token_start,
+                        pos_map=pm, k_scale_src=self.host_k_scale_src)
+            for s, (k, v), pm in zip(w.segments, self.host_sources, self.host_pos_maps)])
+        return self.host_segs
+
+    def run_host(self, ctx, stream=None, dst=None):
+        return ctx.reposition_splice_host(dst if dst is not None else self.dst, self.host_segs, stream=stream)
+
+
+def bits_to_numpy(t):
+    """Bit-pattern tensor (int16 for bf16, uint8 for fp8) -> contiguous numpy array (uint16 / uint8) on the host."""
+    a = t.detach().cpu().contiguous().numpy()
+    return a.view(np.uint16) if a.dtype == np.int16 else a

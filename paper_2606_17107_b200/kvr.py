@@ -50,6 +50,7 @@ class kvr_tuning(C.Structure):
 
 
 EXPORTS = ["kvr_create", "kvr_destroy", "kvr_set_tuning", "kvr_validate", "kvr_reposition_splice",
+           "kvr_reposition_splice_host", "kvr_last_h2d_bytes",
            "kvr_bytes_moved", "kvr_last_device_status", "kvr_launch_count", "kvr_last_launch_info",
            "kvr_status_string", "kvr_last_cuda_error", "kvr_version"]
 
@@ -70,6 +71,10 @@ def _load():
     lib.kvr_validate.argtypes = [P(kvr_model_desc), P(kvr_paged_dst), P(kvr_segment), C.c_int32]
     lib.kvr_reposition_splice.restype = C.c_int
     lib.kvr_reposition_splice.argtypes = [C.c_void_p, P(kvr_paged_dst), P(kvr_segment), C.c_int32, C.c_void_p]
+    lib.kvr_reposition_splice_host.restype = C.c_int
+    lib.kvr_reposition_splice_host.argtypes = lib.kvr_reposition_splice.argtypes
+    lib.kvr_last_h2d_bytes.restype = C.c_uint64
+    lib.kvr_last_h2d_bytes.argtypes = [C.c_void_p]
     lib.kvr_bytes_moved.restype = C.c_uint64
     lib.kvr_bytes_moved.argtypes = [P(kvr_model_desc), P(kvr_segment), C.c_int32]
     lib.kvr_last_device_status.restype = C.c_int
@@ -188,6 +193,18 @@ class Context:
         if check and st != KVR_OK:
             raise KvrError(st, lib.kvr_last_cuda_error(self._h).decode())
         return st
+
+    def reposition_splice_host(self, dst: kvr_paged_dst, segs, stream=None, check=True):
+        """kvr_reposition_splice_host: the segments' k_src / v_src / pos_map / k_scale_src are HOST pointers."""
+        arr = segs if not isinstance(segs, (list, tuple)) else segment_array(segs)
+        s = None if stream is None else (stream if isinstance(stream, int) else stream.cuda_stream)
+        st = lib.kvr_reposition_splice_host(self._h, C.byref(dst), arr, len(arr), s)
+        if check and st != KVR_OK:
+            raise KvrError(st, lib.kvr_last_cuda_error(self._h).decode())
+        return st
+
+    def last_h2d_bytes(self):
+        return int(lib.kvr_last_h2d_bytes(self._h))
 
     def last_device_status(self):
         seg, tok = C.c_int32(-1), C.c_int32(-1)

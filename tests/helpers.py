@@ -105,24 +105,8 @@ def materialize_cpu(w):
 
 def run_oracle(w, srcs, k_cache, v_cache, n_threads=1, layer_begin=0, layer_end=None, segments=None):
     """Splices every segment of w into (k_cache, v_cache) in place with the oracle."""
-    s_l, s_b, s_t, s_h = w.dst_strides()
-    for i, seg in enumerate(w.segments):
-        if segments is not None and i not in segments:
-            continue
-        k_src, v_src = srcs[i]
-        sl, sh, st = w.src_strides(seg)
-        status = orc.reposition_splice(
-            layers=w.layers, kv_heads=w.kv_heads, head_dim=w.head_dim, rotary_dim=w.rotary_dim,
-            pairing=PAIRING[w.pairing], dtype=DTYPE[w.dtype], inv_freq=w.inv_freq,
-            k_cache=k_cache, v_cache=v_cache, stride_layer=s_l, stride_block=s_b, stride_token=s_t,
-            stride_head=s_h, num_blocks=w.num_blocks, block_size=w.block_size, block_table=w.block_table,
-            k_scale_dst=w.k_scale, k_src=np.ascontiguousarray(k_src).reshape(-1),
-            v_src=np.ascontiguousarray(v_src).reshape(-1),
-            src_stride_layer=sl, src_stride_head=sh, src_stride_token=st,
-            len=seg.len, old_start=seg.old_start, new_start=seg.new_start, dst_seq=seg.dst_seq,
-            dst_token_start=seg.dst_token_start, pos_map=seg.pos_map, k_scale_src=w.k_scale_src,
-            layer_begin=layer_begin, layer_end=layer_end, n_threads=n_threads)
-        assert status == orc.OK, (i, status)
+    orc.splice_workload(w, srcs, k_cache, v_cache, n_threads=n_threads, layer_begin=layer_begin,
+                        layer_end=layer_end, segments=segments)
 
 
 # ---------------------------------------------------------------- brute-force slot enumeration

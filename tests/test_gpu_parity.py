@@ -239,3 +239,25 @@ def test_full_size_cfg3_sampled_layers():
     if free < 80e9:
         pytest.skip("needs ~65 GB of device memory")
     _sampled_full_size(3, "NHD", [0, 31], dict(path=0))
+
+
+# ------------------------------------------------------------------ host-resident sources
+@pytest.mark.parametrize("layout", ["NHD", "HND"])
+@pytest.mark.parametrize("c", [0, 1, 2, 3, 4])
+def test_host_sources_entry_point(c, layout):
+    """kvr_reposition_splice_host (pinned host K/V, staged per layer group) gives the same bytes as the oracle."""
+    from paper_2606_17107_b200 import kvr
+    from paper_2606_17107_b200.harness import DeviceWorkload
+    w = config_small(c, layout)
+    srcs, kc, vc = materialize_cpu(w)
+    dw = DeviceWorkload(w, "cuda:0", sources=[(torch_bits(k), torch_bits(v)) for k, v in srcs])
+    dw.make_host_sources()
+    with kvr.Context(dw.model) as ctx:
+        for _ in range(3):                      # staging buffers are reused across calls
+            dw.run_host(ctx)
+        assert ctx.last_device_status()[0] == 0
+        assert ctx.last_h2d_bytes() >= dw.bytes_moved() // 2
+    torch.cuda.synchronize()
+    run_oracle(w, srcs, kc, vc)
+    assert np.array_equal(np_bits(dw.v_cache), vc)
+    assert k_distance(w, np_bits(dw.k_cache), kc).max() <= K_TOL[w.dtype]
