@@ -114,7 +114,8 @@ typedef struct {
   int32_t layers_per_unit; /* layers one scheduled unit covers                                  */
   int32_t v_bulk_store;    /* 0 auto, 1 V leaves shared memory by bulk (TMA) stores, 2 by warps */
   int32_t max_ctas;        /* cap on the persistent grid (tests use it to force many tiles per CTA)  */
-  int32_t reserved[9];
+  int32_t grab;            /* units a CTA draws from the dynamic scheduler per atomic (1..32)               */
+  int32_t reserved[8];
 } kvr_tuning;
 
 /* Creates a context on CUDA device `cuda_device` (must be compute capability 10.x).  Allocates a few

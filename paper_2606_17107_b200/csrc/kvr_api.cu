@@ -90,6 +90,7 @@ struct kvr_ctx {
   double* d_inv_freq = nullptr;
   int32_t* d_status = nullptr;
   int32_t* h_status = nullptr;      // pinned
+  unsigned long long* d_sched = nullptr;   // ring kernel's unit counter + finished-CTA counter (zero between launches)
   int device = 0, sm_count = 0;
   Slot slots[kSlots];
   int next_slot = 0;
@@ -167,6 +168,8 @@ kvr_status kvr_create(kvr_ctx** out, const kvr_model_desc* model, int cuda_devic
   if (e == cudaSuccess) e = cudaMalloc(&c->d_status, 4 * sizeof(int32_t));
   if (e == cudaSuccess) e = cudaMemset(c->d_status, 0, 4 * sizeof(int32_t));
   if (e == cudaSuccess) e = cudaMallocHost(&c->h_status, 4 * sizeof(int32_t));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_sched, 2 * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMemset(c->d_sched, 0, 2 * sizeof(unsigned long long));
   for (int i = 0; i < kSlots && e == cudaSuccess; ++i)
     e = cudaEventCreateWithFlags(&c->slots[i].ev, cudaEventDisableTiming);
   cudaSetDevice(prev);
@@ -200,6 +203,7 @@ kvr_status kvr_destroy(kvr_ctx* c) {
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->d_inv_freq) cudaFree(c->d_inv_freq);
   if (c->d_status) cudaFree(c->d_status);
+  if (c->d_sched) cudaFree(c->d_sched);
   if (c->h_status) cudaFreeHost(c->h_status);
   cudaSetDevice(prev);
   (void)cudaGetLastError();
@@ -264,6 +268,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   P.num_blocks = d->num_blocks; P.block_size = d->block_size; P.num_seqs = d->num_seqs;
   P.max_blocks = d->max_blocks_per_seq;
   P.segs = slot.dev; P.n_segs = n; P.status = c->d_status;
+  P.sched = c->d_sched;
 
   bool any_map = false, scales_differ = false;
   for (int32_t i = 0; i < n; ++i) {
@@ -328,10 +333,14 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     decompose(chunk_granularity(d->block_size, limit < 16 ? limit : 16), tu.layers_per_unit);
   }
 
-  KVR_CUDA(c, cudaMemcpyAsync(slot.dev, slot.host, (size_t)n * sizeof(SegDev), cudaMemcpyHostToDevice, stream));
+  if (n <= kInlineSegs) {
+    for (int32_t i = 0; i < n; ++i) P.inline_segs[i] = slot.host[i];   // descriptors ride in the kernel parameters
+  } else {
+    KVR_CUDA(c, cudaMemcpyAsync(slot.dev, slot.host, (size_t)n * sizeof(SegDev), cudaMemcpyHostToDevice, stream));
+  }
   cudaError_t e;
   if (path == 2) {
-    RingConfig rc{tu.ctas_per_sm, tu.consumer_warps, tu.stages, tu.v_bulk_store, tu.max_ctas};
+    RingConfig rc{tu.ctas_per_sm, tu.consumer_warps, tu.stages, tu.v_bulk_store, tu.max_ctas, tu.grab};
     e = launch_ring(P, rc, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
   } else {
     e = launch_generic(P, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);

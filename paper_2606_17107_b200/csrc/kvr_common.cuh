@@ -34,6 +34,8 @@ struct SegDev {
   int32_t pad_;
 };
 
+constexpr int kInlineSegs = 8;    // calls with <= this many segments carry their descriptors in the kernel parameters
+
 struct CallParams {
   // model
   int32_t layers, heads, head_dim, rotary_dim, pairing, dtype;
@@ -55,7 +57,17 @@ struct CallParams {
   int32_t* status;             // DEVICE int32[4]: {flag, segment, token, -}
   int32_t any_pos_map;
   int32_t scales_differ;       // fp8: some segment has its own source scales
+  // dynamic unit scheduler (ring kernel): sched[0] = next unit to hand out, sched[1] = CTAs that have finished;
+  // both are zero between launches (the last CTA to finish resets them)
+  unsigned long long* sched;
+  int32_t grab;                // units handed out per atomic
+  int32_t pad_;
+  SegDev inline_segs[kInlineSegs];
 };
+
+__device__ __forceinline__ const SegDev* seg_array(const CallParams& P) {
+  return (P.n_segs <= kInlineSegs) ? P.inline_segs : P.segs;
+}
 
 __device__ __forceinline__ int find_segment(const SegDev* __restrict__ segs, int n, int64_t unit) {
   int lo = 0, hi = n - 1;      // last segment with unit_begin <= unit
@@ -145,7 +157,7 @@ __device__ __forceinline__ uint32_t f32x2_to_e4m3x2_sat(float lo, float hi) {
 cudaError_t launch_generic(const CallParams& P, int sm_count, cudaStream_t stream, int* grid, int* block, int* smem);
 
 struct RingConfig {
-  int ctas_per_sm, consumer_warps, stages, v_bulk_store, max_ctas;
+  int ctas_per_sm, consumer_warps, stages, v_bulk_store, max_ctas, grab;
 };
 bool ring_supported(const CallParams& P, const SegDev* host_segs, const char** why);
 cudaError_t launch_ring(const CallParams& P, const RingConfig& cfg, int sm_count, cudaStream_t stream,

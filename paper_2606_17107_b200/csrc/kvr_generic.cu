@@ -11,7 +11,7 @@
 namespace kvr {
 
 template <int DTYPE>
-__global__ void __launch_bounds__(256) kvr_generic_kernel(const CallParams P) {
+__global__ void __launch_bounds__(256) kvr_generic_kernel(const __grid_constant__ CallParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* tab = reinterpret_cast<float4*>(smem_raw);                 // [cg][R/2]
   int32_t* is_copy = reinterpret_cast<int32_t*>(tab + (size_t)P.cg * (P.rotary_dim / 2));  // [cg]
@@ -20,8 +20,9 @@ __global__ void __launch_bounds__(256) kvr_generic_kernel(const CallParams P) {
   const int D = P.head_dim, R = P.rotary_dim;
 
   for (int64_t unit = blockIdx.x; unit < P.total_units; unit += gridDim.x) {
-    const int si = find_segment(P.segs, P.n_segs, unit);
-    const SegDev s = P.segs[si];
+    const SegDev* segs = seg_array(P);
+    const int si = find_segment(segs, P.n_segs, unit);
+    const SegDev s = segs[si];
     const int64_t local = unit - s.unit_begin;
     const int lg = (int)(local / s.n_chunks);
     const int c = (int)(local % s.n_chunks);

@@ -17,7 +17,7 @@
 //                                                                                     (steps a3, a5)
 //                   then release the stage through its "empty" mbarrier.
 //
-// Tiles are uniform, so units are dealt round-robin to the persistent CTAs (grid = SMs x CTAs/SM).
+// Units are drawn by the persistent CTAs (grid = SMs x CTAs/SM) from one global counter (dynamic scheduling).
 #include <cstdio>
 
 #include "kvr_common.cuh"
@@ -239,14 +239,23 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     const int hgroups = P.heads / RP.hpt;
     const unsigned FULL = 0xFFFFFFFFu;
 
-    for (int64_t base = blockIdx.x; base < P.total_units; base += (int64_t)gridDim.x * 32) {
-      // ---- batch decode: lane j resolves unit base + j*grid (segment, chunk, block-table entry: step a4),
-      //      so the dependent global loads are paid once per 32 units, off the per-tile path ----
-      const int64_t my_unit = base + (int64_t)lane * gridDim.x;
+    const SegDev* segs = seg_array(P);
+    const int G = P.grab;          // units per grab, 1..32
+    // ---- dynamic scheduling: CTAs draw units from one global counter, so a CTA on a slower path to memory
+    //      simply takes fewer units (a static round-robin deal loses ~10 % of the copy bandwidth to drift and tail).
+    //      The next grab is requested before the current one is issued, so its latency is off the critical path. ----
+    unsigned long long nxt = 0;
+    if (lane == 0) nxt = atomicAdd(P.sched, (unsigned long long)G);
+    for (;;) {
+      const int64_t base = (int64_t)__shfl_sync(FULL, nxt, 0);
+      if (base >= P.total_units) break;
+      // ---- batch decode: lane j resolves unit base + j (segment, chunk, block-table entry: step a4),
+      //      so the dependent global loads are paid once per grab, off the per-tile path ----
+      const int64_t my_unit = base + lane;
       int d_si = -1, d_t0 = 0, d_ntok = 0, d_off = 0, d_lg = 0, d_blk = -1;
-      if (my_unit < P.total_units) {
-        d_si = find_segment(P.segs, P.n_segs, my_unit);
-        const SegDev* s = P.segs + d_si;
+      if (lane < G && my_unit < P.total_units) {
+        d_si = find_segment(segs, P.n_segs, my_unit);
+        const SegDev* s = segs + d_si;
         const int64_t local = my_unit - s->unit_begin;
         const int n_chunks = s->n_chunks;
         d_lg = (int)(local / n_chunks);
@@ -255,19 +264,20 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         d_t0 = ch.t0; d_ntok = ch.n_tok; d_off = ch.off;
         d_blk = P.block_table[(int64_t)s->dst_seq * P.max_blocks + ch.blk_index];
       }
-      for (int j = 0; j < 32; ++j) {
+      if (lane == 0) nxt = atomicAdd(P.sched, (unsigned long long)G);
+      for (int j = 0; j < G; ++j) {
         const int si = __shfl_sync(FULL, d_si, j);
         if (si < 0) break;
         const int t0 = __shfl_sync(FULL, d_t0, j), n_tok = __shfl_sync(FULL, d_ntok, j);
         const int off = __shfl_sync(FULL, d_off, j), lg = __shfl_sync(FULL, d_lg, j);
         const int blk = __shfl_sync(FULL, d_blk, j);
-        if (si != cur_si) { sg = P.segs[si]; cur_si = si; }
+        if (si != cur_si) { sg = segs[si]; cur_si = si; }
         if (blk < 0 || blk >= P.num_blocks) {
           if (lane == 0) report_bad_block(P.status, sg.index, t0);
           continue;
         }
         // ---- angle table (step a1) ----
-        const int64_t key = MAP ? (base + (int64_t)j * gridDim.x) : (int64_t)si;
+        const int64_t key = MAP ? (base + j) : (int64_t)si;
         if (key != cur_key) {
           const int nb = tb ^ 1;
           if (lane == 0 && (nb ? lu_valid[1] : lu_valid[0]) && (nb ? lu_i[1] : lu_i[0]) + (uint32_t)S >= i)   // tiles <= i-1-S are known released
@@ -355,6 +365,14 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       meta[my_stage] = m;
       mbar_arrive(s_full + 8u * my_stage);
     }
+    // every CTA's last grab has returned >= total_units once all of them are here: the last one re-arms the scheduler
+    if (lane == 0) {
+      __threadfence();
+      if (atomicAdd(P.sched + 1, 1ull) == (unsigned long long)gridDim.x - 1ull) {
+        P.sched[0] = 0ull; P.sched[1] = 0ull;
+        __threadfence();
+      }
+    }
     return;
   }
 
@@ -436,7 +454,7 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       bool requant = false;
       if (DTYPE == 1) {
         const float s_dst = s_scales[m.scale_idx + hh];
-        s_src = P.scales_differ ? P.segs[m.seg].k_scale_src[m.scale_idx + hh] : s_dst;
+        s_src = P.scales_differ ? seg_array(P)[m.seg].k_scale_src[m.scale_idx + hh] : s_dst;
         requant = (s_src != s_dst);
         inv_dst = __frcp_rn(s_dst);
       }
@@ -513,8 +531,10 @@ static cudaError_t launch_inst(const CallParams& P, const RingParams& RP, int gr
   return cudaGetLastError();
 }
 
-cudaError_t launch_ring(const CallParams& P, const RingConfig& cfg, int sm_count, cudaStream_t stream,
+cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_count, cudaStream_t stream,
                         int* grid_out, int* block_out, int* smem_out) {
+  CallParams P = P_in;
+  P.grab = cfg.grab > 0 ? (cfg.grab > 32 ? 32 : cfg.grab) : 1;
   const int E = P.dtype == 0 ? 2 : 1;
   RingParams RP{};
   RP.cg = P.cg;

@@ -46,7 +46,7 @@ class kvr_segment(C.Structure):
 class kvr_tuning(C.Structure):
     _fields_ = [("path", C.c_int32), ("ctas_per_sm", C.c_int32), ("consumer_warps", C.c_int32),
                 ("stages", C.c_int32), ("layers_per_unit", C.c_int32), ("v_bulk_store", C.c_int32),
-                ("max_ctas", C.c_int32), ("reserved", C.c_int32 * 9)]
+                ("max_ctas", C.c_int32), ("grab", C.c_int32), ("reserved", C.c_int32 * 8)]
 
 
 EXPORTS = ["kvr_create", "kvr_destroy", "kvr_set_tuning", "kvr_validate", "kvr_reposition_splice",
