@@ -48,6 +48,10 @@
  * form inv_freq = pi/2 (Delta = 1, 2, 4), exhaustive codec checks against
  * ml_dtypes, brute-force slot enumeration with a sentinel-filled pool, and a
  * cross-check of the direct-RoPE helper against the transformers library.
+ * kvr_oracle_reposition_inplace (reading R20) is pinned by
+ * tests/test_oracle_inplace.py: the pi/2 closed form through brute-force slot
+ * enumeration, Delta = 0 leaves every byte, untouched slots and pass-through dims
+ * keep their bytes, Delta then -Delta, and the RoPE identity through the pool.
  * Nothing in this file is "parity unpinned".
  *
  * Build: gcc -O2 -std=c11 -fopenmp -shared -fPIC (oracle/build.py).  No
@@ -285,6 +289,89 @@ int kvr_oracle_reposition_splice(
           if (s_src != s_dst) /* pass-through dims are re-expressed in the new scale */
             for (int d = rotary_dim; d < head_dim; ++d)
               kd[d] = kvr_oracle_e4m3_encode_sat(kvr_oracle_e4m3_decode(ks[d]) * s_src / s_dst);
+        }
+      }
+    }
+  }
+  return KVRO_OK;
+}
+
+/* ------------------------------------------------- in-place reposition (NEXT-1) */
+
+/*
+ * Re-rotation of a chunk that is ALREADY RESIDENT in the paged pool (reading R20).
+ *   PAPER.md:528 (App. H): "the user-memory chunk is precompiled once in isolation and
+ *     RoPE-repositioned to float just before the query each turn (an O(L_mem) re-rotation,
+ *     no re-prefill)";  PAPER.md:167 (sec. 7): the chunk is re-floated every turn.
+ * The chunk occupies logical tokens [token_start, token_start + len) of block-table row `seq`.
+ * Every K row of it is decoded, rotated by Delta_t exactly as in the splice (same readings R1,
+ * R6, R7, R13), rounded once, and written back to the slot it came from.  V is position-free
+ * and is not touched: there is no V argument.  fp8: the pool's scale is both the
+ * source and the destination scale.  Delta_t == 0 leaves the row's bytes alone.
+ * Returns KVRO_ERR_OUT_OF_RANGE, writing nothing, if a touched block-table entry is invalid.
+ */
+int kvr_oracle_reposition_inplace(
+    int layers, int kv_heads, int head_dim, int rotary_dim, int pairing, int dtype,
+    const double* inv_freq,
+    void* k_cache,
+    int64_t stride_layer, int64_t stride_block, int64_t stride_token, int64_t stride_head,
+    int num_blocks, int block_size,
+    const int32_t* block_table, int num_seqs, int max_blocks_per_seq,
+    const float* k_scale,
+    int seq, int token_start, int len, int old_start, int new_start, const int32_t* pos_map,
+    int layer_begin, int layer_end, int n_threads) {
+  if (!inv_freq || !k_cache || !block_table) return KVRO_ERR_INVALID_ARG;
+  if (layers <= 0 || kv_heads <= 0 || head_dim <= 0) return KVRO_ERR_INVALID_ARG;
+  if (rotary_dim < 2 || (rotary_dim & 1) || rotary_dim > head_dim) return KVRO_ERR_INVALID_ARG;
+  if (pairing != KVRO_PAIR_NEOX_HALF && pairing != KVRO_PAIR_GPTJ_INTERLEAVED) return KVRO_ERR_INVALID_ARG;
+  if (dtype != KVRO_BF16 && dtype != KVRO_FP8_E4M3) return KVRO_ERR_INVALID_ARG;
+  if (dtype == KVRO_FP8_E4M3 && !k_scale) return KVRO_ERR_INVALID_ARG;
+  if (block_size <= 0 || num_blocks <= 0 || num_seqs <= 0 || max_blocks_per_seq <= 0) return KVRO_ERR_INVALID_ARG;
+  if (len <= 0 || seq < 0 || seq >= num_seqs || token_start < 0) return KVRO_ERR_INVALID_ARG;
+  if ((int64_t)token_start + len > (int64_t)max_blocks_per_seq * block_size) return KVRO_ERR_INVALID_ARG;
+  if (layer_begin < 0 || layer_end > layers || layer_begin > layer_end) return KVRO_ERR_INVALID_ARG;
+  if (n_threads < 1) return KVRO_ERR_INVALID_ARG;
+
+  const int esz = (dtype == KVRO_BF16) ? 2 : 1;
+  const int32_t* table_row = block_table + (int64_t)seq * max_blocks_per_seq;
+  for (int t = 0; t < len; ++t) {
+    int32_t blk = table_row[((int64_t)token_start + t) / block_size];
+    if (blk < 0 || blk >= num_blocks) return KVRO_ERR_OUT_OF_RANGE;
+  }
+
+#pragma omp parallel for collapse(2) schedule(static) num_threads(n_threads) if (n_threads > 1)
+  for (int l = layer_begin; l < layer_end; ++l) {
+    for (int h = 0; h < kv_heads; ++h) {
+      const double sc = (dtype == KVRO_FP8_E4M3) ? (double)k_scale[l * kv_heads + h] : 1.0;
+      for (int t = 0; t < len; ++t) {
+        int64_t delta = pos_map ? (int64_t)pos_map[t] - ((int64_t)old_start + t)
+                                : (int64_t)new_start - (int64_t)old_start;
+        if (delta == 0) continue;                       /* reading R13: bytes stay as they are */
+        int64_t j = (int64_t)token_start + t;
+        int64_t blk = table_row[j / block_size];
+        int64_t off = j % block_size;
+        uint8_t* row = (uint8_t*)k_cache + ((int64_t)l * stride_layer + blk * stride_block +
+                                            off * stride_token + (int64_t)h * stride_head) * esz;
+        for (int i = 0; i < rotary_dim / 2; ++i) {
+          int ia, ib;
+          pair_indices(pairing, rotary_dim, i, &ia, &ib);
+          double phi = (double)delta * inv_freq[i];
+          double c = cos(phi), s = sin(phi);
+          if (dtype == KVRO_BF16) {
+            uint16_t ua, ub;
+            memcpy(&ua, row + 2 * ia, 2);
+            memcpy(&ub, row + 2 * ib, 2);
+            double a = kvr_oracle_bf16_decode(ua), b = kvr_oracle_bf16_decode(ub);
+            uint16_t ra = kvr_oracle_bf16_encode(a * c - b * s);
+            uint16_t rb = kvr_oracle_bf16_encode(b * c + a * s);
+            memcpy(row + 2 * ia, &ra, 2);
+            memcpy(row + 2 * ib, &rb, 2);
+          } else {
+            double a = kvr_oracle_e4m3_decode(row[ia]) * sc;
+            double b = kvr_oracle_e4m3_decode(row[ib]) * sc;
+            row[ia] = kvr_oracle_e4m3_encode_sat((a * c - b * s) / sc);
+            row[ib] = kvr_oracle_e4m3_encode_sat((b * c + a * s) / sc);
+          }
         }
       }
     }

@@ -45,6 +45,13 @@ def lib():
             [C.c_void_p, C.c_void_p] + [C.c_int64] * 3 + [C.c_int] * 5 +
             [C.c_void_p, C.c_void_p] +                            # segment
             [C.c_int] * 3)                                        # control
+        _lib.kvr_oracle_reposition_inplace.restype = C.c_int
+        _lib.kvr_oracle_reposition_inplace.argtypes = (
+            [C.c_int] * 6 + [C.c_void_p] +                      # model
+            [C.c_void_p] + [C.c_int64] * 4 + [C.c_int, C.c_int] +
+            [C.c_void_p, C.c_int, C.c_int, C.c_void_p] +          # pool (K only)
+            [C.c_int] * 5 + [C.c_void_p] +                        # the resident span
+            [C.c_int] * 3)                                        # control
         _lib.kvr_oracle_bytes_moved.restype = C.c_uint64
         _lib.kvr_oracle_bytes_moved.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int64]
     return _lib
@@ -133,6 +140,27 @@ def reposition_splice(*, layers, kv_heads, head_dim, rotary_dim, pairing, dtype,
         layer_begin, layer_end, n_threads)
 
 
+def reposition_inplace(*, layers, kv_heads, head_dim, rotary_dim, pairing, dtype, inv_freq,
+                       k_cache, stride_layer, stride_block, stride_token, stride_head,
+                       num_blocks, block_size, block_table, k_scale=None,
+                       seq, token_start, len, old_start, new_start, pos_map=None,
+                       layer_begin=0, layer_end=None, n_threads=1):
+    """Re-rotates ONE resident span of k_cache in place (kvr_oracle_reposition_inplace).  Returns the status."""
+    edt = np.uint16 if dtype == BF16 else np.uint8
+    inv_freq = np.ascontiguousarray(inv_freq, dtype=np.float64)
+    assert inv_freq.shape == (rotary_dim // 2,)
+    assert block_table.dtype == np.int32 and block_table.ndim == 2
+    num_seqs, max_blocks = block_table.shape
+    if layer_end is None:
+        layer_end = layers
+    return lib().kvr_oracle_reposition_inplace(
+        layers, kv_heads, head_dim, rotary_dim, pairing, dtype, _ptr(inv_freq),
+        _ptr(k_cache, edt, True), stride_layer, stride_block, stride_token, stride_head,
+        num_blocks, block_size, _ptr(block_table, np.int32), num_seqs, max_blocks, _ptr(k_scale, np.float32),
+        seq, token_start, len, old_start, new_start, _ptr(pos_map, np.int32),
+        layer_begin, layer_end, n_threads)
+
+
 def bytes_moved(layers, kv_heads, head_dim, dtype, tokens):
     return int(lib().kvr_oracle_bytes_moved(layers, kv_heads, head_dim, dtype, tokens))
 
@@ -170,3 +198,20 @@ def splice_workload(w, srcs, k_cache, v_cache, n_threads=1, layer_begin=0, layer
             layer_begin=layer_begin, layer_end=layer_end, n_threads=n_threads)
         if status != OK:
             raise RuntimeError(f"oracle: segment {i} -> status {status}")
+
+
+def inplace_workload(w, k_cache, n_threads=1, layer_begin=0, layer_end=None, deltas=None):
+    """Re-rotates, in place, the span every segment of w occupies in k_cache: segment i moves from the positions
+    it was spliced at (new_start.., or its pos_map) by deltas[i] more positions.  Pure marshalling."""
+    s_l, s_b, s_t, s_h = w.dst_strides()
+    for i, seg in enumerate(w.segments):
+        d = int(deltas[i])
+        status = reposition_inplace(
+            layers=w.layers, kv_heads=w.kv_heads, head_dim=w.head_dim, rotary_dim=w.rotary_dim,
+            pairing=_PAIRING[w.pairing], dtype=_DTYPE[w.dtype], inv_freq=w.inv_freq, k_cache=k_cache,
+            stride_layer=s_l, stride_block=s_b, stride_token=s_t, stride_head=s_h, num_blocks=w.num_blocks,
+            block_size=w.block_size, block_table=w.block_table, k_scale=w.k_scale,
+            seq=seg.dst_seq, token_start=seg.dst_token_start, len=seg.len, old_start=0, new_start=d,
+            layer_begin=layer_begin, layer_end=layer_end, n_threads=n_threads)
+        if status != OK:
+            raise RuntimeError(f"oracle in-place: segment {i} -> status {status}")
