@@ -52,6 +52,9 @@ def parse_args():
     ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
     ap.add_argument("--layout", default="NHD", choices=["NHD", "HND"])
     ap.add_argument("--impl", default="kvr", choices=["kvr", "reference"])
+    ap.add_argument("--op", default="splice", choices=["splice", "inplace"],
+                    help="splice = kvr_reposition_splice (the BASELINE.json metric); inplace = kvr_reposition_inplace "
+                         "(SURVEY.md 8(f) NEXT-1: re-float resident chunks, 2*B1 bytes per token; device-timed only)")
     ap.add_argument("--e2e-steps", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -233,29 +236,37 @@ def run_kvr(args):
     if args.tune:
         ctx.set_tuning(**{k: int(v) for k, v in (kv.split("=") for kv in args.tune.split(","))})
 
+    run_step = lambda: dw.run(ctx, stream=stream)
+    if args.op == "inplace":
+        dw.run(ctx, stream=stream)                       # the chunks must be resident first (finite keys in the slots)
+        spans = dw.inplace_spans([161 + 7 * i for i in range(len(w.segments))])
+        bytes_per_step = kvr.kvr_inplace_bytes_moved(dw.model, spans)
+        run_step = lambda: dw.run_inplace(ctx, spans, stream=stream)
+        args.no_e2e = args.no_cpu_baseline = True
+
     # ---- device-resident timing ----
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(device)             # NVML init happens here, before the warm-up, not after it
     for _ in range(warmup):
-        dw.run(ctx, stream=stream)
+        run_step()
     # An idle B200 sits at ~120 MHz SM clock and needs some tens of ms of load to reach its running clocks; a
     # handful of sub-ms warm-up steps does not get it there.  Keep warming (untimed) until the GPU has been
     # busy for >= 0.3 s, then go straight into the timed region.  `warmup` in the JSON line is the count done.
     t_ramp = time.perf_counter()
     while time.perf_counter() - t_ramp < 0.3 and warmup < 100000:
         for _ in range(8):
-            dw.run(ctx, stream=stream)
+            run_step()
         warmup += 8
         torch.cuda.synchronize(device)
     st = ctx.last_device_status()
     assert st[0] == kvr.KVR_OK, st
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler = ClockSampler(device)
     torch.cuda.synchronize(device)
     rep.barrier()
     launches0 = ctx.launch_count()
     with sampler:
         ev0.record(stream)
         for _ in range(steps):
-            dw.run(ctx, stream=stream)
+            run_step()
         ev1.record(stream)
         sampler.sample()                       # the queue is still draining: a sample under load even for short runs
         torch.cuda.synchronize(device)
@@ -302,10 +313,11 @@ def run_kvr(args):
     ctx.close()
     if rep.rank == 0:
         line = {
-            "metric": METRIC, "value": agg["per_second"], "unit": UNIT, "n_gpus": rep.world, "steps": steps,
+            "metric": METRIC if args.op == "splice" else "KV tokens repositioned in place/sec",
+            "value": agg["per_second"], "unit": UNIT, "n_gpus": rep.world, "steps": steps,
             "warmup": warmup, "ms_per_step": agg["seconds"] / steps * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": w.name, "config_index": args.config, "layout": args.layout,
+            "config": {"workload": w.name, "op": args.op, "config_index": args.config, "layout": args.layout,
                        "cache_dtype": CACHE_DTYPE[w.dtype], "tokens": tokens, "segments": len(w.segments),
                        "bytes_per_step": bytes_per_step, "parallelism": f"replicas x{rep.world}",
                        "l2": f"inputs larger than L2 ({bytes_per_step // 2} B of sources + as many pool bytes "
@@ -315,7 +327,7 @@ def run_kvr(args):
             "gpu_launches": launches,
             "clocks": clocks,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC_BYTES.get(w.name), "peak_source": peak_src,
+                         "traffic": NCU_TRAFFIC_BYTES.get(w.name if args.op == "splice" else w.name + ":inplace"), "peak_source": peak_src,
                          "gb_s_of_nominal_8000": achieved / 8000.0},
             "e2e": e2e,
             "cpu_baseline": cpu,

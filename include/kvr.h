@@ -112,10 +112,12 @@ typedef struct {
   int32_t consumer_warps;  /* consumer warps per CTA                                           */
   int32_t stages;          /* ring depth (tiles in flight per CTA)                             */
   int32_t layers_per_unit; /* layers one scheduled unit covers                                  */
-  int32_t v_bulk_store;    /* 0 auto, 1 V leaves shared memory by bulk (TMA) stores, 2 by warps */
+  int32_t v_bulk_store;    /* 0 auto, 1 V leaves shared memory by bulk (TMA) stores, 2 by warps, 3 one bulk store per row */
   int32_t max_ctas;        /* cap on the persistent grid (tests use it to force many tiles per CTA)  */
   int32_t grab;            /* units a CTA draws from the dynamic scheduler per atomic (1..32)               */
-  int32_t reserved[8];
+  int32_t pdl;             /* programmatic dependent launch of the ring kernel: 0 auto (on), 1 on, 2 off            */
+  int32_t hsplit;          /* split a unit's heads into this many units (finer tail); 0 auto                        */
+  int32_t reserved[6];
 } kvr_tuning;
 
 /* Creates a context on CUDA device `cuda_device` (must be compute capability 10.x).  Allocates a few
@@ -150,6 +152,46 @@ KVR_API kvr_status kvr_reposition_splice(kvr_ctx* ctx, const kvr_paged_dst* dst,
 KVR_API kvr_status kvr_reposition_splice_host(kvr_ctx* ctx, const kvr_paged_dst* dst, const kvr_segment* segs,
                                               int32_t n_segs, void* cuda_stream);
 KVR_API uint64_t kvr_last_h2d_bytes(const kvr_ctx* ctx);
+
+/* ---- NEXT-1: in-place reposition of a chunk that is ALREADY RESIDENT in the paged pool -------------------
+ * PAPER.md:528 (App. H): "the user-memory chunk is precompiled once in isolation and RoPE-repositioned to float
+ * just before the query each turn (an O(L_mem) re-rotation, no re-prefill)"; PAPER.md:167 (sec. 7).
+ * A resident span is logical tokens [token_start, token_start + len) of block-table row `seq`.  Every K row of it
+ * is rotated by delta = new_start - old_start (or, with pos_map (DEVICE int32 [len]), by
+ * delta_t = pos_map[t] - (old_start + t)) exactly as in kvr_reposition_splice and written back to the slot it was
+ * read from.  V is position-free and is neither read nor written: pool->v_cache may be NULL.
+ * fp8: pool->k_scale is both the source and the destination scale.  delta_t == 0 leaves the row's bytes alone.
+ * Traffic is 2 * layers*kv_heads*head_dim*esz bytes per token (kvr_inplace_bytes_moved), half of a re-splice.
+ * Spans of one call must not overlap (undefined).  Same asynchrony, validation and error rules as the splice:
+ * host-detectable faults are rejected before any launch; an invalid block-table entry skips its tokens and
+ * raises the sticky device status. */
+typedef struct {
+  int32_t seq, token_start, len;
+  int32_t old_start, new_start;
+  const int32_t* pos_map;
+} kvr_resident_span;
+
+KVR_API kvr_status kvr_reposition_inplace(kvr_ctx* ctx, const kvr_paged_dst* pool, const kvr_resident_span* spans,
+                                          int32_t n_spans, void* cuda_stream);
+KVR_API uint64_t kvr_inplace_bytes_moved(const kvr_model_desc* model, const kvr_resident_span* spans, int32_t n_spans);
+
+/* ---- NEXT-2: span overwrite -----------------------------------------------------------------------------
+ * PAPER.md:348 (App. B) / :112 (sec. 4): the field-only edit overwrites the KV of a short value span in place;
+ * PAPER.md:141 (sec. 5) / :171 / :528: one (or a few) boundary tokens of a transplanted chunk are recomputed
+ * ("seam repair").  Producing the new K/V needs a model and is the caller's business; writing them into the paged
+ * pool is this call: K and V rows k_src / v_src (DEVICE, logical [layers][kv_heads][len][head_dim], element
+ * strides as in kvr_segment; K already RoPE'd at its final positions) are copied byte for byte to logical tokens
+ * [dst_token_start, dst_token_start + len) of block-table row dst_seq.  It is the delta = 0 case of
+ * kvr_reposition_splice and runs through the same kernels. */
+typedef struct {
+  const void* k_src;
+  const void* v_src;
+  int64_t src_stride_layer, src_stride_head, src_stride_token; /* elements */
+  int32_t len, dst_seq, dst_token_start;
+} kvr_span;
+
+KVR_API kvr_status kvr_write_span(kvr_ctx* ctx, const kvr_paged_dst* dst, const kvr_span* spans, int32_t n_spans,
+                                  void* cuda_stream);
 
 /* Algorithmic bytes of a call: read K, read V, write K, write V = 4 * layers*kv_heads*head_dim*esz * sum(len).
  * This is the O(L) of PAPER.md:143 and the numerator of every GB/s this repository reports. */

@@ -211,7 +211,7 @@ def inplace_workload(w, k_cache, n_threads=1, layer_begin=0, layer_end=None, del
             pairing=_PAIRING[w.pairing], dtype=_DTYPE[w.dtype], inv_freq=w.inv_freq, k_cache=k_cache,
             stride_layer=s_l, stride_block=s_b, stride_token=s_t, stride_head=s_h, num_blocks=w.num_blocks,
             block_size=w.block_size, block_table=w.block_table, k_scale=w.k_scale,
-            seq=seg.dst_seq, token_start=seg.dst_token_start, len=seg.len, old_start=0, new_start=d,
+            seq=seg.dst_seq, token_start=seg.dst_token_start, len=seg.len, old_start=max(0, -d), new_start=max(0, d),
             layer_begin=layer_begin, layer_end=layer_end, n_threads=n_threads)
         if status != OK:
             raise RuntimeError(f"oracle in-place: segment {i} -> status {status}")

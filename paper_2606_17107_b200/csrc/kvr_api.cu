@@ -236,7 +236,7 @@ uint64_t kvr_bytes_moved(const kvr_model_desc* m, const kvr_segment* segs, int32
 // destination, its scales and the source scales are advanced to layer l0; the K/V sources are advanced too
 // unless `src_group_local` (the host-source path stages exactly the group's layers at layer index 0).
 static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_segment* segs, int32_t n,
-                                 cudaStream_t stream, int l0, int nl, bool src_group_local) {
+                                 cudaStream_t stream, int l0, int nl, bool src_group_local, bool inplace = false) {
   kvr_status st = KVR_OK;
   cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
   KVR_CUDA(c, cudaStreamIsCapturing(stream, &cap));
@@ -261,7 +261,8 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   P.layers = m.layers; P.heads = m.kv_heads; P.head_dim = m.head_dim; P.rotary_dim = m.rotary_dim;
   P.pairing = m.pairing; P.dtype = m.dtype; P.inv_freq = c->d_inv_freq;
   P.k_cache = static_cast<uint8_t*>(d->k_cache) + (int64_t)l0 * d->stride_layer * E;
-  P.v_cache = static_cast<uint8_t*>(d->v_cache) + (int64_t)l0 * d->stride_layer * E;
+  P.v_cache = d->v_cache ? static_cast<uint8_t*>(d->v_cache) + (int64_t)l0 * d->stride_layer * E : nullptr;
+  P.inplace = inplace ? 1 : 0;
   P.d_sl = d->stride_layer; P.d_sb = d->stride_block; P.d_st = d->stride_token; P.d_sh = d->stride_head;
   P.block_table = d->block_table;
   P.k_scale_dst = d->k_scale ? d->k_scale + (int64_t)l0 * m.kv_heads : nullptr;
@@ -278,8 +279,16 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   P.any_pos_map = any_map; P.scales_differ = scales_differ;
 
   // ---- work decomposition: (segment, chunk of <= cg destination tokens, group of lpu layers) ----
-  auto decompose = [&](int cg, int lpu_request) {
+  auto decompose = [&](int cg, int lpu_request, int hsplit_request) {
     P.cg = cg;
+    // head split (ring kernel only): must divide the number of head groups of a unit
+    int hsplit = 1;
+    if (hsplit_request > 1 && !any_map) {
+      const int hgroups = m.kv_heads / ring_heads_per_tile(P);
+      hsplit = hsplit_request > hgroups ? hgroups : hsplit_request;
+      while (hsplit > 1 && hgroups % hsplit) --hsplit;
+    }
+    P.hsplit = hsplit;
     int64_t chunks_total = 0;
     for (int32_t i = 0; i < n; ++i) {
       const kvr_segment& s = segs[i];
@@ -308,7 +317,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       }
     }
     if (lpu > m.layers) lpu = m.layers;
-    P.lpu = lpu; P.n_lgroups = (m.layers + lpu - 1) / lpu;
+    P.lpu = lpu; P.n_lgroups = ((m.layers + lpu - 1) / lpu) * hsplit;
     int64_t at = 0;
     for (int32_t i = 0; i < n; ++i) {
       slot.host[i].unit_begin = at;
@@ -321,7 +330,13 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   int path = tu.path;
   const char* why = nullptr;
   if (path == 0 || path == 2) {
-    decompose(chunk_granularity(d->block_size, 16), tu.layers_per_unit);
+    int cg_limit = 16;
+    if (inplace && d->stride_token != m.head_dim) {
+      // token-major pool, in place: a tile is cg tokens x ALL heads (one contiguous run); keep it near 8 KB
+      cg_limit = (int)(8192 / ((int64_t)m.kv_heads * m.head_dim * E));
+      cg_limit = cg_limit < 1 ? 1 : (cg_limit > 16 ? 16 : cg_limit);
+    }
+    decompose(chunk_granularity(d->block_size, cg_limit), tu.layers_per_unit, tu.hsplit);
     bool ok = ring_supported(P, slot.host, &why);
     if (!ok && path == 2) { c->last_err = std::string("ring kernel unsupported: ") + (why ? why : ""); return KVR_ERR_UNSUPPORTED; }
     path = ok ? 2 : 1;
@@ -330,7 +345,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     // generic kernel: chunk table [cg][R/2] float4 must fit 48 KB of static-limit shared memory
     int limit = (int)(47 * 1024 / ((m.rotary_dim / 2) * 16 + 4));
     if (limit < 1) return KVR_ERR_UNSUPPORTED;
-    decompose(chunk_granularity(d->block_size, limit < 16 ? limit : 16), tu.layers_per_unit);
+    decompose(chunk_granularity(d->block_size, limit < 16 ? limit : 16), tu.layers_per_unit, 1);
   }
 
   if (n <= kInlineSegs) {
@@ -340,7 +355,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   }
   cudaError_t e;
   if (path == 2) {
-    RingConfig rc{tu.ctas_per_sm, tu.consumer_warps, tu.stages, tu.v_bulk_store, tu.max_ctas, tu.grab};
+    RingConfig rc{tu.ctas_per_sm, tu.consumer_warps, tu.stages, tu.v_bulk_store, tu.max_ctas, tu.grab, tu.pdl};
     e = launch_ring(P, rc, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
   } else {
     e = launch_generic(P, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
@@ -497,6 +512,80 @@ kvr_status kvr_reposition_splice_host(kvr_ctx* c, const kvr_paged_dst* d, const 
 }
 
 uint64_t kvr_last_h2d_bytes(const kvr_ctx* c) { return c ? c->h2d_bytes : 0; }
+
+// ---- NEXT-1: in-place reposition of resident spans (R20) ----
+static kvr_status check_inplace(const kvr_model_desc* m, const kvr_paged_dst* d, const kvr_resident_span* sp, int32_t n) {
+  kvr_status st = check_model(m);
+  if (st != KVR_OK) return st;
+  if (!d || n < 0 || (n > 0 && !sp)) return KVR_ERR_INVALID_ARG;
+  if (!d->k_cache || !d->block_table) return KVR_ERR_INVALID_ARG;
+  if (d->num_blocks <= 0 || d->block_size <= 0 || d->num_seqs <= 0 || d->max_blocks_per_seq <= 0)
+    return KVR_ERR_INVALID_ARG;
+  if (d->stride_layer < 0 || d->stride_block <= 0 || (d->stride_token < m->head_dim && d->block_size > 1))
+    return KVR_ERR_INVALID_ARG;
+  if (d->stride_head < m->head_dim && m->kv_heads > 1) return KVR_ERR_INVALID_ARG;
+  if (m->dtype == KVR_FP8_E4M3 && !d->k_scale) return KVR_ERR_INVALID_ARG;
+  const int E = elt_bytes(m->dtype);
+  if (!aligned16(d->k_cache)) return KVR_ERR_ALIGNMENT;
+  const int64_t ds[4] = {d->stride_layer, d->stride_block, d->stride_token, d->stride_head};
+  for (int64_t s : ds)
+    if ((s * E) % 16 != 0) return KVR_ERR_ALIGNMENT;
+  const int64_t cap = (int64_t)d->max_blocks_per_seq * d->block_size;
+  for (int32_t i = 0; i < n; ++i) {
+    const kvr_resident_span& s = sp[i];
+    if (s.len <= 0 || s.seq < 0 || s.seq >= d->num_seqs || s.token_start < 0) return KVR_ERR_INVALID_ARG;
+    if (s.old_start < 0 || (!s.pos_map && s.new_start < 0)) return KVR_ERR_INVALID_ARG;
+    if ((int64_t)s.token_start + s.len > cap) return KVR_ERR_OUT_OF_RANGE;
+    if (s.pos_map && (reinterpret_cast<uintptr_t>(s.pos_map) & 3u)) return KVR_ERR_ALIGNMENT;
+  }
+  return KVR_OK;
+}
+
+kvr_status kvr_reposition_inplace(kvr_ctx* c, const kvr_paged_dst* pool, const kvr_resident_span* spans, int32_t n,
+                                  void* cuda_stream) {
+  if (!c) return KVR_ERR_INVALID_ARG;
+  c->last_err.clear();
+  kvr_status st = check_inplace(&c->model, pool, spans, n);
+  if (st != KVR_OK) return st;
+  if (n == 0) return KVR_OK;
+  std::vector<kvr_segment> segs((size_t)n);
+  for (int32_t i = 0; i < n; ++i) {
+    kvr_segment& g = segs[(size_t)i];
+    g = kvr_segment{};
+    g.k_src = pool->k_cache; g.v_src = pool->k_cache;      // placeholders: the kernels read the pool slot itself
+    g.src_stride_layer = g.src_stride_head = 0; g.src_stride_token = c->model.head_dim;
+    g.len = spans[i].len; g.old_start = spans[i].old_start; g.new_start = spans[i].new_start;
+    g.dst_seq = spans[i].seq; g.dst_token_start = spans[i].token_start;
+    g.pos_map = spans[i].pos_map; g.k_scale_src = nullptr;
+  }
+  if ((st = check_deltas(segs.data(), n)) != KVR_OK) return st;
+  DeviceGuard guard(c->device);
+  return enqueue_layers(c, pool, segs.data(), n, static_cast<cudaStream_t>(cuda_stream), 0, c->model.layers, false, true);
+}
+
+uint64_t kvr_inplace_bytes_moved(const kvr_model_desc* m, const kvr_resident_span* spans, int32_t n) {
+  if (!m || (n > 0 && !spans)) return 0;
+  uint64_t tokens = 0;
+  for (int32_t i = 0; i < n; ++i) tokens += spans[i].len > 0 ? (uint64_t)spans[i].len : 0u;
+  return 2ull * (uint64_t)m->layers * (uint64_t)m->kv_heads * (uint64_t)m->head_dim * (uint64_t)elt_bytes(m->dtype) * tokens;
+}
+
+// ---- NEXT-2: span overwrite = the delta == 0 splice (R21) ----
+kvr_status kvr_write_span(kvr_ctx* c, const kvr_paged_dst* dst, const kvr_span* spans, int32_t n, void* cuda_stream) {
+  if (!c) return KVR_ERR_INVALID_ARG;
+  if (n < 0 || (n > 0 && !spans)) return KVR_ERR_INVALID_ARG;
+  std::vector<kvr_segment> segs((size_t)n);
+  for (int32_t i = 0; i < n; ++i) {
+    kvr_segment& g = segs[(size_t)i];
+    g = kvr_segment{};
+    g.k_src = spans[i].k_src; g.v_src = spans[i].v_src;
+    g.src_stride_layer = spans[i].src_stride_layer; g.src_stride_head = spans[i].src_stride_head;
+    g.src_stride_token = spans[i].src_stride_token;
+    g.len = spans[i].len; g.old_start = 0; g.new_start = 0;          // delta = 0: K rows are byte copies
+    g.dst_seq = spans[i].dst_seq; g.dst_token_start = spans[i].dst_token_start;
+  }
+  return kvr_reposition_splice(c, dst, segs.data(), n, cuda_stream);
+}
 
 kvr_status kvr_last_device_status(kvr_ctx* c, int32_t* bad_segment, int32_t* bad_token) {
   if (!c) return KVR_ERR_INVALID_ARG;

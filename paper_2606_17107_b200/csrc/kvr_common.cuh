@@ -61,7 +61,9 @@ struct CallParams {
   // both are zero between launches (the last CTA to finish resets them)
   unsigned long long* sched;
   int32_t grab;                // units handed out per atomic
+  int32_t hsplit;              // ring kernel: a (chunk, layer group) is split into hsplit units over its head groups
   int32_t pad_;
+  int32_t inplace;             // kvr_reposition_inplace: K rows are read from the pool slot they are written back to; no V
   SegDev inline_segs[kInlineSegs];
 };
 
@@ -157,8 +159,9 @@ __device__ __forceinline__ uint32_t f32x2_to_e4m3x2_sat(float lo, float hi) {
 cudaError_t launch_generic(const CallParams& P, int sm_count, cudaStream_t stream, int* grid, int* block, int* smem);
 
 struct RingConfig {
-  int ctas_per_sm, consumer_warps, stages, v_bulk_store, max_ctas, grab;
+  int ctas_per_sm, consumer_warps, stages, v_bulk_store, max_ctas, grab, pdl;
 };
+int ring_heads_per_tile(const CallParams& P);   // heads one tile of the ring kernel covers (needs P.cg)
 bool ring_supported(const CallParams& P, const SegDev* host_segs, const char** why);
 cudaError_t launch_ring(const CallParams& P, const RingConfig& cfg, int sm_count, cudaStream_t stream,
                         int* grid, int* block, int* smem);

@@ -5,7 +5,8 @@
 //   1. angle table for the chunk's tokens: fp64 sincos -> fp32 hi/lo in shared memory (step a1)
 //   2. block-table lookup for the chunk (step a4)
 //   3. K rotary pairs, scalar element loads (a2, a3, a5); K pass-through dims; V 16-byte copies (a6)
-// Steps refer to SURVEY.md 8(a) / DESIGN.md "Path".
+// Steps refer to SURVEY.md 8(a) / DESIGN.md "Path".  With P.inplace (kvr_reposition_inplace, R20) the K row
+// is read from the pool slot it is written back to, and pass-through dims and V are left alone.
 #include "kvr_common.cuh"
 
 namespace kvr {
@@ -55,8 +56,9 @@ __global__ void __launch_bounds__(256) kvr_generic_kernel(const __grid_constant_
       int l = l0 + row / (ch.n_tok * P.heads);
       int ia = (P.pairing == 0) ? i : 2 * i;
       int ib = (P.pairing == 0) ? i + half : 2 * i + 1;
-      const uint8_t* src = s.k_src + ((int64_t)l * s.sl + (int64_t)h * s.sh + (int64_t)(ch.t0 + t) * s.st) * E;
       uint8_t* dst = P.k_cache + ((int64_t)l * P.d_sl + (int64_t)h * P.d_sh + (int64_t)t * P.d_st + dst_base) * E;
+      const uint8_t* src = P.inplace ? dst      // each pair is read and written by this one thread: aliasing-safe
+                                     : s.k_src + ((int64_t)l * s.sl + (int64_t)h * s.sh + (int64_t)(ch.t0 + t) * s.st) * E;
       float4 cs = tab[t * half + i];
       if (DTYPE == 0) {
         uint16_t ua = reinterpret_cast<const uint16_t*>(src)[ia], ub = reinterpret_cast<const uint16_t*>(src)[ib];
@@ -82,6 +84,7 @@ __global__ void __launch_bounds__(256) kvr_generic_kernel(const __grid_constant_
         dst[ib] = qb;
       }
     }
+    if (P.inplace) continue;   // pass-through dims and V already hold their bytes
     // ---- K pass-through dims [R, D) ----
     const int pass = D - R;
     for (int64_t idx = threadIdx.x; idx < (int64_t)rows * pass; idx += blockDim.x) {

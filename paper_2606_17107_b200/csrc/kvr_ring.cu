@@ -35,6 +35,10 @@ struct RingParams {
   int off_meta, off_scales, off_tab, tab_stride, NTB, off_stage;
   int v_bulk;                             // V leaves shared memory by bulk stores (needs stride_token == head_dim)
   int n_scales;                           // fp8: layers * heads destination scales preloaded to shared memory
+  int off_ub, n_ub;                       // segments' first-unit prefix sums in shared memory (calls with many segments)
+  int no_v;                               // in-place mode: a stage holds K only and V is never touched
+  int ip_mode;                            // in-place source runs: 0 one run per head (d_st == head_dim), 1 one run for the
+                                          // whole tile (token-major pool, all heads in the tile), 2 one copy per row
 };
 
 struct __align__(16) TileMeta {
@@ -48,7 +52,7 @@ struct __align__(16) TileMeta {
 };
 static_assert(sizeof(TileMeta) == 32, "TileMeta layout");
 
-constexpr int kFlagDone = 1, kFlagRotate = 2;
+constexpr int kFlagDone = 1, kFlagRotate = 2, kFlagTokMajor = 4;   // TokMajor: the stage is laid out [token][head][dim]
 constexpr int kMaxThreads = 32 * 17;
 
 // ------------------------------------------------------------------------------- PTX helpers
@@ -156,6 +160,9 @@ __device__ __forceinline__ void rot_bf16_gptj(uint4& A, const float4* T) {
   }
 }
 // fp8, NeoX: A = 16 "a" codes, B = 16 "b" codes; T[j] = (cos, sin) of element j.
+// SCALE = false: source and destination scales are the same number, so dequantise/requantise cancel exactly
+// ((q s c - q' s s') / s = q c - q' s'): the codes are rotated as they are, which is both cheaper and closer to fp64.
+template <bool SCALE>
 __device__ __forceinline__ void rot_fp8_neox(uint4& A, uint4& B, const float2* T, float s_src, float inv_dst, bool rot) {
   uint32_t* a = reinterpret_cast<uint32_t*>(&A);
   uint32_t* b = reinterpret_cast<uint32_t*>(&B);
@@ -168,15 +175,20 @@ __device__ __forceinline__ void rot_fp8_neox(uint4& A, uint4& B, const float2* T
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
       float2 cs = rot ? T[4 * w + j] : make_float2(1.0f, 0.0f);
-      rotate_plain(__fmul_rn(av[j], s_src), __fmul_rn(bv[j], s_src), cs.x, cs.y, ra[j], rb[j]);
-      ra[j] = __fmul_rn(ra[j], inv_dst);
-      rb[j] = __fmul_rn(rb[j], inv_dst);
+      if (SCALE) {
+        rotate_plain(__fmul_rn(av[j], s_src), __fmul_rn(bv[j], s_src), cs.x, cs.y, ra[j], rb[j]);
+        ra[j] = __fmul_rn(ra[j], inv_dst);
+        rb[j] = __fmul_rn(rb[j], inv_dst);
+      } else {
+        rotate_plain(av[j], bv[j], cs.x, cs.y, ra[j], rb[j]);
+      }
     }
     a[w] = f32x2_to_e4m3x2_sat(ra[0], ra[1]) | (f32x2_to_e4m3x2_sat(ra[2], ra[3]) << 16);
     b[w] = f32x2_to_e4m3x2_sat(rb[0], rb[1]) | (f32x2_to_e4m3x2_sat(rb[2], rb[3]) << 16);
   }
 }
 // fp8, GPT-J: word w = codes (a, b, a, b) of pairs 2w, 2w+1.
+template <bool SCALE>
 __device__ __forceinline__ void rot_fp8_gptj(uint4& A, const float2* T, float s_src, float inv_dst, bool rot) {
   uint32_t* a = reinterpret_cast<uint32_t*>(&A);
 #pragma unroll
@@ -184,10 +196,16 @@ __device__ __forceinline__ void rot_fp8_gptj(uint4& A, const float2* T, float s_
     float2 p0 = e4m3x2_to_f32x2(a[w] & 0xFFFFu), p1 = e4m3x2_to_f32x2(a[w] >> 16);
     float2 c0 = rot ? T[2 * w] : make_float2(1.0f, 0.0f), c1 = rot ? T[2 * w + 1] : make_float2(1.0f, 0.0f);
     float ra0, rb0, ra1, rb1;
-    rotate_plain(__fmul_rn(p0.x, s_src), __fmul_rn(p0.y, s_src), c0.x, c0.y, ra0, rb0);
-    rotate_plain(__fmul_rn(p1.x, s_src), __fmul_rn(p1.y, s_src), c1.x, c1.y, ra1, rb1);
-    a[w] = f32x2_to_e4m3x2_sat(__fmul_rn(ra0, inv_dst), __fmul_rn(rb0, inv_dst)) |
-           (f32x2_to_e4m3x2_sat(__fmul_rn(ra1, inv_dst), __fmul_rn(rb1, inv_dst)) << 16);
+    if (SCALE) {
+      rotate_plain(__fmul_rn(p0.x, s_src), __fmul_rn(p0.y, s_src), c0.x, c0.y, ra0, rb0);
+      rotate_plain(__fmul_rn(p1.x, s_src), __fmul_rn(p1.y, s_src), c1.x, c1.y, ra1, rb1);
+      a[w] = f32x2_to_e4m3x2_sat(__fmul_rn(ra0, inv_dst), __fmul_rn(rb0, inv_dst)) |
+             (f32x2_to_e4m3x2_sat(__fmul_rn(ra1, inv_dst), __fmul_rn(rb1, inv_dst)) << 16);
+    } else {
+      rotate_plain(p0.x, p0.y, c0.x, c0.y, ra0, rb0);
+      rotate_plain(p1.x, p1.y, c1.x, c1.y, ra1, rb1);
+      a[w] = f32x2_to_e4m3x2_sat(ra0, rb0) | (f32x2_to_e4m3x2_sat(ra1, rb1) << 16);
+    }
   }
 }
 // fp8 pass-through vector under a scale change: requantise every code
@@ -219,8 +237,15 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     for (int s = 0; s < S; ++s) { mbar_init(s_full + 8u * s, 1); mbar_init(s_empty + 8u * s, 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  // Programmatic dependent launch: let the next launch on this stream bring its CTAs up (they take an SM's shared
+  // memory as soon as a CTA of this grid exits) and run this prologue while our tail drains; it touches no global
+  // memory until griddepcontrol.wait has seen the previous grid complete and flush.
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   if (DTYPE == 1)
     for (int i = threadIdx.x; i < RP.n_scales; i += blockDim.x) s_scales[i] = P.k_scale_dst[i];
+  for (int i = threadIdx.x; i < RP.n_ub; i += blockDim.x)
+    reinterpret_cast<int64_t*>(smem + RP.off_ub)[i] = P.segs[i].unit_begin;
   __syncthreads();
 
   if (warp == NW) {
@@ -244,17 +269,21 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     // ---- dynamic scheduling: CTAs draw units from one global counter, so a CTA on a slower path to memory
     //      simply takes fewer units (a static round-robin deal loses ~10 % of the copy bandwidth to drift and tail).
     //      The next grab is requested before the current one is issued, so its latency is off the critical path. ----
-    unsigned long long nxt = 0;
-    if (lane == 0) nxt = atomicAdd(P.sched, (unsigned long long)G);
-    for (;;) {
-      const int64_t base = (int64_t)__shfl_sync(FULL, nxt, 0);
-      if (base >= P.total_units) break;
-      // ---- batch decode: lane j resolves unit base + j (segment, chunk, block-table entry: step a4),
-      //      so the dependent global loads are paid once per grab, off the per-tile path ----
-      const int64_t my_unit = base + lane;
-      int d_si = -1, d_t0 = 0, d_ntok = 0, d_off = 0, d_lg = 0, d_blk = -1;
+    // ---- batch decode: lane j resolves unit base + j (segment, chunk, block-table entry: step a4).  The decode of
+    //      grab k+1 is started BEFORE the tiles of grab k are issued, so its dependent global loads (descriptor,
+    //      block table) complete while the producer is busy arming stages: small units cost no producer stalls. ----
+    const int64_t* ub = reinterpret_cast<const int64_t*>(smem + RP.off_ub);
+    auto decode = [&](int64_t base_, int& d_si, int& d_t0, int& d_ntok, int& d_off, int& d_lg, int& d_blk) {
+      const int64_t my_unit = base_ + lane;
+      d_si = -1; d_t0 = 0; d_ntok = 0; d_off = 0; d_lg = 0; d_blk = -1;
       if (lane < G && my_unit < P.total_units) {
-        d_si = find_segment(segs, P.n_segs, my_unit);
+        if (RP.n_ub) {               // prefix sums of the segments' unit counts, staged in shared memory
+          int lo = 0, hi = P.n_segs - 1;
+          while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (ub[mid] <= my_unit) lo = mid; else hi = mid - 1; }
+          d_si = lo;
+        } else {
+          d_si = find_segment(segs, P.n_segs, my_unit);
+        }
         const SegDev* s = segs + d_si;
         const int64_t local = my_unit - s->unit_begin;
         const int n_chunks = s->n_chunks;
@@ -264,7 +293,19 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         d_t0 = ch.t0; d_ntok = ch.n_tok; d_off = ch.off;
         d_blk = P.block_table[(int64_t)s->dst_seq * P.max_blocks + ch.blk_index];
       }
-      if (lane == 0) nxt = atomicAdd(P.sched, (unsigned long long)G);
+    };
+    unsigned long long nxt = 0;
+    if (lane == 0) nxt = atomicAdd(P.sched, (unsigned long long)G);
+    int64_t base = (int64_t)__shfl_sync(FULL, nxt, 0);
+    if (lane == 0) nxt = atomicAdd(P.sched, (unsigned long long)G);
+    int d_si, d_t0, d_ntok, d_off, d_lg, d_blk;
+    decode(base, d_si, d_t0, d_ntok, d_off, d_lg, d_blk);
+    for (;;) {
+      if (base >= P.total_units) break;
+      const int64_t base_n = (int64_t)__shfl_sync(FULL, nxt, 0);
+      if (lane == 0 && base_n < P.total_units) nxt = atomicAdd(P.sched, (unsigned long long)G);
+      int n_si, n_t0, n_ntok, n_off, n_lg, n_blk;
+      decode(base_n, n_si, n_t0, n_ntok, n_off, n_lg, n_blk);
       for (int j = 0; j < G; ++j) {
         const int si = __shfl_sync(FULL, d_si, j);
         if (si < 0) break;
@@ -299,9 +340,12 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         {
           // ---- tile issue (steps a2 / a6-read): lane t takes tile t of the unit, so up to min(32, S) tiles are
           //      armed and issued per pass instead of one (a single thread needs ~1k cycles per tile) ----
-          const int l0 = lg * P.lpu, l1 = min(P.layers, l0 + P.lpu);
-          const int n_tiles = (l1 - l0) * hgroups;
-          const int flags = (MAP || sg.delta != 0) ? kFlagRotate : 0;
+          const int lgi = lg / P.hsplit, hpart = lg - lgi * P.hsplit;     // layer group, head part of this unit
+          const int l0 = lgi * P.lpu, l1 = min(P.layers, l0 + P.lpu);
+          const int hg_per = hgroups / P.hsplit;
+          const int n_tiles = (l1 - l0) * hg_per;
+          const bool inplace = P.inplace != 0;
+          const int flags = ((MAP || sg.delta != 0) ? kFlagRotate : 0) | ((inplace && RP.ip_mode == 1) ? kFlagTokMajor : 0);
           const uint32_t run_bytes = (uint32_t)(n_tok * RP.rowB);
           const bool packed_rows = (sg.st == P.head_dim);
           const int64_t dst_chunk = (int64_t)blk * P.d_sb + (int64_t)off * P.d_st;
@@ -311,7 +355,7 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
             const int n = min(pass, n_tiles - tb0);
             if (lane < n) {
               const int t = tb0 + lane;
-              const int l = l0 + t / hgroups, h0 = (t % hgroups) * RP.hpt;
+              const int l = l0 + t / hg_per, h0 = (hpart * hg_per + t % hg_per) * RP.hpt;
               int my_stage = stage + lane;
               uint32_t my_phase = phase;
               if (my_stage >= S) { my_stage -= S; my_phase ^= 1u; }
@@ -322,9 +366,24 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
               m.n_tok = n_tok; m.flags = flags; m.tab = tb; m.gen = gen;
               m.scale_idx = l * P.heads + h0; m.seg = si;
               meta[my_stage] = m;
-              mbar_arrive_expect_tx(bar, 2u * RP.hpt * run_bytes);
+              mbar_arrive_expect_tx(bar, (inplace ? 1u : 2u) * RP.hpt * run_bytes);
               const uint32_t sk = s_base + RP.off_stage + (uint32_t)my_stage * RP.stage_bytes;
               const uint32_t sv = sk + RP.tile_bytes;
+              if (inplace) {
+                // the tile's source IS its destination: K rows already resident in the paged pool (R20)
+                const uint8_t* src = P.k_cache + m.dst_off * E;
+                if (RP.ip_mode == 1) {
+                  bulk_g2s(sk, src, RP.hpt * run_bytes, bar, pol);                    // [token][head][dim], one run
+                } else if (RP.ip_mode == 0) {
+                  for (int hh = 0; hh < RP.hpt; ++hh)                                  // [head][token][dim], a run per head
+                    bulk_g2s(sk + (uint32_t)(hh * RP.cg * RP.rowB), src + (int64_t)hh * P.d_sh * E, run_bytes, bar, pol);
+                } else {
+                  for (int hh = 0; hh < RP.hpt; ++hh)
+                    for (int r = 0; r < n_tok; ++r)
+                      bulk_g2s(sk + (uint32_t)((hh * RP.cg + r) * RP.rowB),
+                               src + ((int64_t)hh * P.d_sh + (int64_t)r * P.d_st) * E, RP.rowB, bar, pol);
+                }
+              } else
               for (int hh = 0; hh < RP.hpt; ++hh) {
                 const int64_t src_off = ((int64_t)l * sg.sl + (int64_t)(h0 + hh) * sg.sh + src_chunk) * E;
                 const uint32_t so = (uint32_t)(hh * RP.cg * RP.rowB);
@@ -353,6 +412,8 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
           }
         }
       }
+      base = base_n;
+      d_si = n_si; d_t0 = n_t0; d_ntok = n_ntok; d_off = n_off; d_lg = n_lg; d_blk = n_blk;
     }
     // one DONE tile per consumer warp, through the same ring (NW <= S, so the stages are distinct)
     if (lane < NW) {
@@ -415,7 +476,16 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     const int n_tok = m.n_tok;
 
     // ---- V (step a6): bytes unchanged ----
-    if (RP.v_bulk) {
+    if (RP.no_v) {
+      // in-place: V is position-free and already where it belongs
+    } else if (RP.v_bulk == 2) {
+      // token-major pool: one bulk store per (head, token) row, lane r issues row r (n_tok <= 32)
+      for (int hh = 0; hh < RP.hpt; ++hh)
+        if (lane < n_tok)
+          bulk_s2g(P.v_cache + (m.dst_off + (int64_t)hh * P.d_sh + (int64_t)lane * P.d_st) * E,
+                   sv + (hh * RP.cg + lane) * RP.rowB, (uint32_t)RP.rowB);
+      bulk_commit();
+    } else if (RP.v_bulk) {
       if (lane == 0) {
         for (int hh = 0; hh < RP.hpt; ++hh)
           bulk_s2g(P.v_cache + (m.dst_off + (int64_t)hh * P.d_sh) * E, sv + hh * RP.cg * RP.rowB, (uint32_t)(n_tok * RP.rowB));
@@ -447,8 +517,10 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         }
       }
     }
+    const int sm_sh = (m.flags & kFlagTokMajor) ? RP.rowB : RP.cg * RP.rowB;        // stage strides of a head / a token
+    const int sm_st = (m.flags & kFlagTokMajor) ? RP.hpt * RP.rowB : RP.rowB;
     for (int hh = 0; hh < RP.hpt; ++hh) {
-      const uint32_t ks = sk + hh * RP.cg * RP.rowB;
+      const uint32_t ks = sk + hh * sm_sh;
       uint8_t* kd = P.k_cache + (m.dst_off + (int64_t)hh * P.d_sh) * E;
       float s_src = 1.0f, inv_dst = 1.0f;
       bool requant = false;
@@ -459,8 +531,8 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         inv_dst = __frcp_rn(s_dst);
       }
       for (int t = rsub; t < n_tok; t += rpi) {
-        uint4 A = lds128(ks + t * RP.rowB + va * 16);
-        uint4 B = lds128(ks + t * RP.rowB + vb * 16);
+        uint4 A = lds128(ks + t * sm_st + va * 16);
+        uint4 B = lds128(ks + t * sm_st + vb * 16);
         bool rot_row = rotate;
         if (MAP) {
           rot_row = reinterpret_cast<const int32_t*>(smem + RP.off_tab + m.tab * RP.tab_stride + RP.cg * RP.half_R * 16)[t] == 0;
@@ -479,12 +551,21 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
             else { if (rot_a) rot_bf16_gptj(A, T4); if (rot_b) rot_bf16_gptj(B, T4 + G::PPV); }
           }
         } else if (rot_row || requant) {
-          if constexpr (PAIRING == 0) {
-            if (rot_a) rot_fp8_neox(A, B, T2, s_src, inv_dst, rot_row);
-            else if (requant) { requant_fp8(A, s_src, inv_dst); requant_fp8(B, s_src, inv_dst); }
-          } else {
-            if (rot_a) rot_fp8_gptj(A, T2, s_src, inv_dst, rot_row); else if (requant) requant_fp8(A, s_src, inv_dst);
-            if (rot_b) rot_fp8_gptj(B, T2 + G::PPV, s_src, inv_dst, rot_row); else if (requant) requant_fp8(B, s_src, inv_dst);
+          if (requant) {
+            if constexpr (PAIRING == 0) {
+              if (rot_a) rot_fp8_neox<true>(A, B, T2, s_src, inv_dst, rot_row);
+              else { requant_fp8(A, s_src, inv_dst); requant_fp8(B, s_src, inv_dst); }
+            } else {
+              if (rot_a) rot_fp8_gptj<true>(A, T2, s_src, inv_dst, rot_row); else requant_fp8(A, s_src, inv_dst);
+              if (rot_b) rot_fp8_gptj<true>(B, T2 + G::PPV, s_src, inv_dst, rot_row); else requant_fp8(B, s_src, inv_dst);
+            }
+          } else {                       // equal scales (then rot_row holds): they cancel
+            if constexpr (PAIRING == 0) {
+              if (rot_a) rot_fp8_neox<false>(A, B, T2, 1.0f, 1.0f, true);
+            } else {
+              if (rot_a) rot_fp8_gptj<false>(A, T2, 1.0f, 1.0f, true);
+              if (rot_b) rot_fp8_gptj<false>(B, T2 + G::PPV, 1.0f, 1.0f, true);
+            }
           }
         }
         uint8_t* row = kd + (int64_t)t * P.d_st * E;
@@ -492,18 +573,28 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         stg128(row + vb * 16, B);
       }
     }
-    if (RP.v_bulk && lane == 0) bulk_wait_read0();   // V bytes have left shared memory
+    if (RP.v_bulk == 2 || (RP.v_bulk && lane == 0)) bulk_wait_read0();   // V bytes have left shared memory
     __syncwarp();
     if (lane == 0) mbar_arrive(s_empty + 8u * stage);
     stage += NW;
     if (stage >= S) { stage -= S; phase ^= 1u; }
   }
-  if (RP.v_bulk && lane == 0) bulk_wait_all0();
+  if (RP.v_bulk == 2 || (RP.v_bulk && lane == 0)) bulk_wait_all0();
   (void)dst_rows_packed;
 }
 
 // ------------------------------------------------------------------------------- host side
 static int ilog2(int x) { int l = 0; while ((1 << l) < x) ++l; return l; }
+
+// heads per tile: smallest divisor of heads whose K run reaches 4 KB; a dense token-major pool re-floated in place
+// takes all heads (its tile is then one contiguous run of the pool)
+int ring_heads_per_tile(const CallParams& P) {
+  const int rowB = P.head_dim * (P.dtype == 0 ? 2 : 1);
+  if (P.inplace && P.d_st != P.head_dim && P.d_sh == P.head_dim && P.d_st == (int64_t)P.heads * P.head_dim) return P.heads;
+  for (int h = 1; h <= P.heads; ++h)
+    if (P.heads % h == 0 && h * P.cg * rowB >= 4096) return h;
+  return P.heads;
+}
 
 bool ring_supported(const CallParams& P, const SegDev* segs, const char** why) {
   const int E = P.dtype == 0 ? 2 : 1;
@@ -520,15 +611,20 @@ bool ring_supported(const CallParams& P, const SegDev* segs, const char** why) {
 }
 
 template <int DTYPE, int PAIRING, bool MAP>
-static cudaError_t launch_inst(const CallParams& P, const RingParams& RP, int grid, int block, int smem, cudaStream_t st) {
+static cudaError_t launch_inst(const CallParams& P, const RingParams& RP, int grid, int block, int smem, cudaStream_t st, bool pdl) {
   static int configured = 0;   // per instantiation
   if (configured < smem) {
     cudaError_t e = cudaFuncSetAttribute(kvr_ring_kernel<DTYPE, PAIRING, MAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     configured = smem;
   }
-  kvr_ring_kernel<DTYPE, PAIRING, MAP><<<grid, block, smem, st>>>(P, RP);
-  return cudaGetLastError();
+  cudaLaunchConfig_t lc{};
+  lc.gridDim = dim3((unsigned)grid); lc.blockDim = dim3((unsigned)block); lc.dynamicSmemBytes = (size_t)smem; lc.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = at; lc.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&lc, kvr_ring_kernel<DTYPE, PAIRING, MAP>, P, RP);
 }
 
 cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_count, cudaStream_t stream,
@@ -545,13 +641,17 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   RP.half_R = P.rotary_dim / 2;
   const int ppv = (P.pairing == 0) ? 16 / E : 8 / E;
   RP.NV = RP.half_R / ppv;
-  // heads per tile: smallest divisor of heads whose K run reaches 4 KB
-  int hpt = P.heads;
-  for (int h = 1; h <= P.heads; ++h)
-    if (P.heads % h == 0 && h * RP.cg * RP.rowB >= 4096) { hpt = h; break; }
+  RP.no_v = P.inplace ? 1 : 0;
+  RP.ip_mode = 0;
+  if (P.inplace) {
+    if (P.d_st == P.head_dim) RP.ip_mode = 0;                                             // head-major pool
+    else if (P.d_sh == P.head_dim && P.d_st == (int64_t)P.heads * P.head_dim) RP.ip_mode = 1;   // token-major, dense
+    else RP.ip_mode = 2;                                                                  // padded rows
+  }
+  const int hpt = ring_heads_per_tile(P);
   RP.hpt = hpt;
   RP.tile_bytes = hpt * RP.cg * RP.rowB;
-  RP.stage_bytes = 2 * RP.tile_bytes;
+  RP.stage_bytes = (RP.no_v ? 1 : 2) * RP.tile_bytes;
   const int ctas = cfg.ctas_per_sm > 0 ? cfg.ctas_per_sm : 2;
   RP.NW = cfg.consumer_warps > 0 ? cfg.consumer_warps : 6;
   if (RP.NW > 16) RP.NW = 16;
@@ -559,11 +659,13 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   const int tab_rows = P.any_pos_map ? RP.cg : 1;
   RP.tab_stride = ((tab_rows * RP.half_R * 16 + RP.cg * 4) + 127) & ~127;
   RP.n_scales = P.dtype == 1 ? P.layers * P.heads : 0;
+  RP.n_ub = (P.n_segs > kInlineSegs && P.n_segs <= 2048) ? P.n_segs : 0;
   const int budget = (227 * 1024) / ctas - 1024;          // per-CTA dynamic shared memory (1 KB reserved per CTA)
   auto layout = [&](int S) {
     int off = 16 * S;
     off = (off + 31) & ~31; RP.off_meta = off; off += 32 * S;
     off = (off + 15) & ~15; RP.off_scales = off; off += 4 * RP.n_scales;
+    off = (off + 15) & ~15; RP.off_ub = off; off += 8 * RP.n_ub;
     off = (off + 127) & ~127; RP.off_tab = off; off += RP.NTB * RP.tab_stride;
     off = (off + 127) & ~127; RP.off_stage = off; off += S * RP.stage_bytes;
     return off;
@@ -576,8 +678,14 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
                     // ordered by one warp's program order (a warp two phases ahead would pass a parity wait early)
   RP.S = S;
   const int smem = layout(S);
-  RP.v_bulk = cfg.v_bulk_store == 1 ? 1 : (cfg.v_bulk_store == 2 ? 0 : (P.d_st == P.head_dim ? 1 : 0));
-  if (P.d_st != P.head_dim) RP.v_bulk = 0;                 // bulk V stores need one contiguous run per (head, chunk)
+  // V out of shared memory: 1 = one bulk store per (head, chunk) run (needs d_st == head_dim), 2 = one bulk store per
+  // row, 0 = 16-byte warp copies.  Tuning v_bulk_store: 0 auto, 1 bulk wherever possible, 2 warp copies, 3 row bulk.
+  const bool runs = (P.d_st == P.head_dim);
+  if (cfg.v_bulk_store == 2) RP.v_bulk = 0;
+  else if (cfg.v_bulk_store == 3) RP.v_bulk = 2;
+  else if (cfg.v_bulk_store == 1) RP.v_bulk = runs ? 1 : 2;
+  else RP.v_bulk = runs ? 1 : 0;
+  if (RP.no_v) RP.v_bulk = 0;
   int64_t g = (int64_t)sm_count * ctas;
   if (cfg.max_ctas > 0 && g > cfg.max_ctas) g = cfg.max_ctas;
   if (g > P.total_units) g = P.total_units;
@@ -585,7 +693,7 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   const int block = (RP.NW + 1) * 32;
   *grid_out = (int)g; *block_out = block; *smem_out = smem;
   const bool map = P.any_pos_map != 0;
-#define KVR_LAUNCH(D, PR, M) return launch_inst<D, PR, M>(P, RP, (int)g, block, smem, stream)
+#define KVR_LAUNCH(D, PR, M) return launch_inst<D, PR, M>(P, RP, (int)g, block, smem, stream, cfg.pdl != 2)
   if (P.dtype == 0) {
     if (P.pairing == 0) { if (map) KVR_LAUNCH(0, 0, true); else KVR_LAUNCH(0, 0, false); }
     else { if (map) KVR_LAUNCH(0, 1, true); else KVR_LAUNCH(0, 1, false); }

@@ -57,6 +57,30 @@ class DeviceWorkload:
     def run(self, ctx, stream=None, dst=None):
         return ctx.reposition_splice(dst if dst is not None else self.dst, self.segs, stream=stream)
 
+    # ---- NEXT-1: re-float the resident chunks in place (kvr_reposition_inplace) ----
+    def inplace_spans(self, deltas, with_pos_map=False):
+        """One resident span per segment of w: the slots the splice wrote, moved by deltas[i] more positions.
+        with_pos_map: express the same shift as a per-token position map (device int32) instead of old/new start."""
+        spans, self._ip_keep = [], []
+        for s, d in zip(self.w.segments, deltas):
+            d = int(d)
+            old, new = max(0, -d), max(0, d)             # positions are non-negative; new - old = d
+            pm = None
+            if with_pos_map:
+                pm = (torch.arange(s.len, dtype=torch.int32, device=self.device) + new)
+                self._ip_keep.append(pm)
+            spans.append(kvr.resident_span(s.dst_seq, s.dst_token_start, s.len, old, new, pos_map=pm))
+        return kvr.resident_span_array(spans)
+
+    def run_inplace(self, ctx, spans, stream=None, dst=None):
+        return ctx.reposition_inplace(dst if dst is not None else self.dst, spans, stream=stream)
+
+    # ---- NEXT-2: span overwrite (kvr_write_span) of every segment's rows, unrotated ----
+    def write_spans(self):
+        w = self.w
+        return kvr.span_array([kvr.span(k, v, w.src_strides(s), s.len, s.dst_seq, s.dst_token_start)
+                               for s, (k, v) in zip(w.segments, self.sources)])
+
     # ---- host-resident sources (kvr_reposition_splice_host) ----
     def make_host_sources(self):
         """Pinned host copies of the sources, position maps and source scales, and the segment array that

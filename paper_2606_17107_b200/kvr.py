@@ -46,10 +46,23 @@ class kvr_segment(C.Structure):
 class kvr_tuning(C.Structure):
     _fields_ = [("path", C.c_int32), ("ctas_per_sm", C.c_int32), ("consumer_warps", C.c_int32),
                 ("stages", C.c_int32), ("layers_per_unit", C.c_int32), ("v_bulk_store", C.c_int32),
-                ("max_ctas", C.c_int32), ("grab", C.c_int32), ("reserved", C.c_int32 * 8)]
+                ("max_ctas", C.c_int32), ("grab", C.c_int32), ("pdl", C.c_int32), ("hsplit", C.c_int32),
+                ("reserved", C.c_int32 * 6)]
 
 
-EXPORTS = ["kvr_create", "kvr_destroy", "kvr_set_tuning", "kvr_validate", "kvr_reposition_splice",
+class kvr_resident_span(C.Structure):
+    _fields_ = [("seq", C.c_int32), ("token_start", C.c_int32), ("len", C.c_int32),
+                ("old_start", C.c_int32), ("new_start", C.c_int32), ("pos_map", C.c_void_p)]
+
+
+class kvr_span(C.Structure):
+    _fields_ = [("k_src", C.c_void_p), ("v_src", C.c_void_p),
+                ("src_stride_layer", C.c_int64), ("src_stride_head", C.c_int64), ("src_stride_token", C.c_int64),
+                ("len", C.c_int32), ("dst_seq", C.c_int32), ("dst_token_start", C.c_int32)]
+
+
+EXPORTS = ["kvr_reposition_inplace", "kvr_inplace_bytes_moved", "kvr_write_span",
+           "kvr_create", "kvr_destroy", "kvr_set_tuning", "kvr_validate", "kvr_reposition_splice",
            "kvr_reposition_splice_host", "kvr_last_h2d_bytes",
            "kvr_bytes_moved", "kvr_last_device_status", "kvr_launch_count", "kvr_last_launch_info",
            "kvr_status_string", "kvr_last_cuda_error", "kvr_version"]
@@ -73,6 +86,12 @@ def _load():
     lib.kvr_reposition_splice.argtypes = [C.c_void_p, P(kvr_paged_dst), P(kvr_segment), C.c_int32, C.c_void_p]
     lib.kvr_reposition_splice_host.restype = C.c_int
     lib.kvr_reposition_splice_host.argtypes = lib.kvr_reposition_splice.argtypes
+    lib.kvr_reposition_inplace.restype = C.c_int
+    lib.kvr_reposition_inplace.argtypes = [C.c_void_p, P(kvr_paged_dst), P(kvr_resident_span), C.c_int32, C.c_void_p]
+    lib.kvr_inplace_bytes_moved.restype = C.c_uint64
+    lib.kvr_inplace_bytes_moved.argtypes = [P(kvr_model_desc), P(kvr_resident_span), C.c_int32]
+    lib.kvr_write_span.restype = C.c_int
+    lib.kvr_write_span.argtypes = [C.c_void_p, P(kvr_paged_dst), P(kvr_span), C.c_int32, C.c_void_p]
     lib.kvr_last_h2d_bytes.restype = C.c_uint64
     lib.kvr_last_h2d_bytes.argtypes = [C.c_void_p]
     lib.kvr_bytes_moved.restype = C.c_uint64
@@ -132,6 +151,28 @@ def segment(k_src, v_src, src_strides, len, old_start, new_start, dst_seq, dst_t
     sl, sh, st = src_strides
     return kvr_segment(_ptr(k_src), _ptr(v_src), sl, sh, st, len, old_start, new_start, dst_seq,
                        dst_token_start, _ptr(pos_map), _ptr(k_scale_src))
+
+
+def resident_span(seq, token_start, len, old_start, new_start, pos_map=None):
+    return kvr_resident_span(seq, token_start, len, old_start, new_start, _ptr(pos_map))
+
+
+def resident_span_array(spans):
+    return (kvr_resident_span * len(spans))(*spans)
+
+
+def span(k_src, v_src, src_strides, len, dst_seq, dst_token_start):
+    sl, sh, st = src_strides
+    return kvr_span(_ptr(k_src), _ptr(v_src), sl, sh, st, len, dst_seq, dst_token_start)
+
+
+def span_array(spans):
+    return (kvr_span * len(spans))(*spans)
+
+
+def kvr_inplace_bytes_moved(model, spans):
+    arr = spans if not isinstance(spans, (list, tuple)) else resident_span_array(spans)
+    return int(lib.kvr_inplace_bytes_moved(C.byref(model), arr, len(arr)))
 
 
 def segment_array(segs):
@@ -199,6 +240,24 @@ class Context:
         arr = segs if not isinstance(segs, (list, tuple)) else segment_array(segs)
         s = None if stream is None else (stream if isinstance(stream, int) else stream.cuda_stream)
         st = lib.kvr_reposition_splice_host(self._h, C.byref(dst), arr, len(arr), s)
+        if check and st != KVR_OK:
+            raise KvrError(st, lib.kvr_last_cuda_error(self._h).decode())
+        return st
+
+    def reposition_inplace(self, pool: kvr_paged_dst, spans, stream=None, check=True):
+        """kvr_reposition_inplace: spans = ctypes array from resident_span_array() or a list of kvr_resident_span."""
+        arr = spans if not isinstance(spans, (list, tuple)) else resident_span_array(spans)
+        s = None if stream is None else (stream if isinstance(stream, int) else stream.cuda_stream)
+        st = lib.kvr_reposition_inplace(self._h, C.byref(pool), arr, len(arr), s)
+        if check and st != KVR_OK:
+            raise KvrError(st, lib.kvr_last_cuda_error(self._h).decode())
+        return st
+
+    def write_span(self, dst: kvr_paged_dst, spans, stream=None, check=True):
+        """kvr_write_span: spans = ctypes array from span_array() or a list of kvr_span."""
+        arr = spans if not isinstance(spans, (list, tuple)) else span_array(spans)
+        s = None if stream is None else (stream if isinstance(stream, int) else stream.cuda_stream)
+        st = lib.kvr_write_span(self._h, C.byref(dst), arr, len(arr), s)
         if check and st != KVR_OK:
             raise KvrError(st, lib.kvr_last_cuda_error(self._h).decode())
         return st

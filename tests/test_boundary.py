@@ -33,6 +33,8 @@ def test_struct_layouts_match_header(kvr):
     assert C.sizeof(kvr.kvr_paged_dst) == 16 + 32 + 8 + 8 + 8 + 8
     assert C.sizeof(kvr.kvr_segment) == 16 + 24 + 20 + 4 + 16
     assert C.sizeof(kvr.kvr_tuning) == 64
+    assert C.sizeof(kvr.kvr_resident_span) == 32
+    assert C.sizeof(kvr.kvr_span) == 16 + 24 + 12 + 4
 
 
 def _call(kvr, **over):
@@ -75,6 +77,14 @@ def test_bytes_moved_is_linear(kvr):
     m8, keep8 = kvr.model_desc(32, 8, 128, 128, 0, 1, [1.0] * 64)
     assert kvr.kvr_bytes_moved(m8, [seg(1)]) == 131072
     assert kvr.kvr_bytes_moved(m, []) == 0
+
+
+def test_inplace_bytes_moved_is_half_of_a_splice(kvr):
+    """NEXT-1: K read + K write only = 2 * layers * kv_heads * head_dim * esz bytes per token."""
+    m, keep = kvr.model_desc(36, 8, 128, 128, 0, 0, [1.0] * 64)
+    sp = [kvr.resident_span(0, 0, 4096, 0, 161)]
+    assert kvr.kvr_inplace_bytes_moved(m, sp) == 1207959552 // 2
+    assert kvr.kvr_inplace_bytes_moved(m, []) == 0
 
 
 def test_no_cpu_fallback(kvr):

@@ -47,6 +47,25 @@ def inv_freq_llama3(theta: float, rotary_dim: int, factor: float, low_freq_facto
     return np.where(wavelen < high_wl, f, np.where(wavelen > low_wl, f / factor, mid))
 
 
+def inv_freq_mrope_temporal(theta: float, rotary_dim: int, sections, interleaved: bool = False) -> np.ndarray:
+    """M-RoPE adapter table (Fig. 22b: "re-rotate only the temporal channels"; R22).
+    The rotary_dim/2 pairs are divided among the (temporal, height, width) axes: `sections` = pairs per axis.
+    sectioned layout (Qwen2.5-VL-like): pairs [0, s_t) temporal, [s_t, s_t+s_h) height, the rest width;
+    interleaved layout (Qwen3-VL-like): pair i is height if i % 3 == 1 and i < 3*s_h, width if i % 3 == 2 and
+    i < 3*s_w, temporal otherwise.  A text-position shift moves only the temporal axis, so the table handed to
+    kvr_create is the standard one with ZERO frequency on the height/width pairs (angle 0: unrotated)."""
+    s_t, s_h, s_w = sections
+    half = rotary_dim // 2
+    assert s_t + s_h + s_w == half
+    i = np.arange(half)
+    if interleaved:
+        temporal = ~(((i % 3 == 1) & (i < 3 * s_h)) | ((i % 3 == 2) & (i < 3 * s_w)))
+    else:
+        temporal = i < s_t
+    assert int(temporal.sum()) == s_t
+    return np.where(temporal, inv_freq_standard(theta, rotary_dim), 0.0)
+
+
 def pos_map_with_gaps(length: int, first: int, gap_prob: float, max_gap: int, seed: int) -> np.ndarray:
     """pos[0] = first; pos[t+1] - pos[t] = 1 w.p. 1-gap_prob else 1 + U{1..max_gap} (R5)."""
     rng = np.random.default_rng(seed)
