@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--workload", default="", help="an adapter workload instead of --config (SURVEY.md 8(f) NEXT-3/4): "
+                    "mla-dsv2-lite | image-kv-qwen25vl-7b | image-kv-qwen3vl-8b; device-timed and e2e only")
     ap.add_argument("--layout", default="NHD", choices=["NHD", "HND"])
     ap.add_argument("--impl", default="kvr", choices=["kvr", "reference"])
     ap.add_argument("--op", default="splice", choices=["splice", "inplace"],
@@ -228,7 +230,12 @@ def run_kvr(args):
     steps = args.steps if args.steps is not None else 1000
     warmup = max(3, args.warmup if args.warmup is not None else 50)
 
-    w = config(args.config, args.layout)
+    if args.workload:
+        from workloads import adapter_config
+        w = adapter_config(args.workload, args.layout)
+        args.no_cpu_baseline = True
+    else:
+        w = config(args.config, args.layout)
     dw = DeviceWorkload(w, device)
     tokens, bytes_per_step = w.tokens, dw.bytes_moved()
     stream = torch.cuda.Stream(device=device)
@@ -317,7 +324,8 @@ def run_kvr(args):
             "value": agg["per_second"], "unit": UNIT, "n_gpus": rep.world, "steps": steps,
             "warmup": warmup, "ms_per_step": agg["seconds"] / steps * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": w.name, "op": args.op, "config_index": args.config, "layout": args.layout,
+            "config": {"workload": w.name, "op": args.op, "config_index": None if args.workload else args.config,
+                       "layout": args.layout,
                        "cache_dtype": CACHE_DTYPE[w.dtype], "tokens": tokens, "segments": len(w.segments),
                        "bytes_per_step": bytes_per_step, "parallelism": f"replicas x{rep.world}",
                        "l2": f"inputs larger than L2 ({bytes_per_step // 2} B of sources + as many pool bytes "

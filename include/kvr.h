@@ -60,13 +60,27 @@ typedef enum { KVR_PAIR_NEOX_HALF = 0, KVR_PAIR_GPTJ_INTERLEAVED = 1 } kvr_pairi
 
 /* Fixed per model.  inv_freq is a HOST array of rotary_dim/2 doubles, copied by kvr_create; the caller
  * applies any frequency scaling (standard theta^(-2i/R), llama3, YaRN ...; "RoPE [28] and
- * their extensions [25]").  rotary_dim is even, 2 <= rotary_dim <= head_dim (partial rotary allowed).
- * head_dim * sizeof(element) must be a multiple of 16 bytes. */
+ * their extensions [25]").  rotary_dim is even, 2 <= rotary_dim, rotary_offset + rotary_dim <= head_dim
+ * (partial rotary allowed).  head_dim * sizeof(element) must be a multiple of 16 bytes.
+ *
+ * Representation adapters (NEXT-3; Fig. 22), all expressed through this struct:
+ *  - M-RoPE, "moving an image within a trajectory re-rotates only the temporal channels": give the height /
+ *    width pairs inv_freq = 0 (their angle is then 0 for every Delta); sectioned and interleaved layouts differ
+ *    only in WHICH entries are zero.
+ *  - MLA, "repositioning re-rotates only k_pe and copies the latent as-is": a cached row is
+ *    [latent c_t | k_pe]; set kv_heads = 1, head_dim = latent width + rope width, rotary_offset = latent width,
+ *    rotary_dim = rope width.  Rotary pair i then is dims rotary_offset + (i, i + rotary_dim/2)  [NEOX_HALF] or
+ *    rotary_offset + (2i, 2i+1)  [GPTJ_INTERLEAVED]; every dim outside the window is copied unchanged.  Such a
+ *    cache has ONE tensor per token: pass v_cache = NULL in kvr_paged_dst and v_src = NULL in every segment
+ *    ("K-only" call; all-or-none, else KVR_ERR_INVALID_ARG).
+ * rotary_offset * sizeof(element) must be a multiple of 16 bytes. */
 typedef struct {
   int32_t layers, kv_heads, head_dim, rotary_dim;
   int32_t pairing; /* kvr_pairing */
   int32_t dtype;   /* kvr_dtype   */
   const double* inv_freq;
+  int32_t rotary_offset; /* first rotary dim of a row; 0 for ordinary K caches */
+  int32_t reserved_;     /* must be 0 */
 } kvr_model_desc;
 
 /* Destination paged pool: caller-owned DEVICE memory.  K and V pools share the four element strides;
@@ -193,7 +207,8 @@ typedef struct {
 KVR_API kvr_status kvr_write_span(kvr_ctx* ctx, const kvr_paged_dst* dst, const kvr_span* spans, int32_t n_spans,
                                   void* cuda_stream);
 
-/* Algorithmic bytes of a call: read K, read V, write K, write V = 4 * layers*kv_heads*head_dim*esz * sum(len).
+/* Algorithmic bytes of a call: read K, read V, write K, write V = 4 * layers*kv_heads*head_dim*esz * sum(len)
+ * (2 * ... for a K-only call, i.e. when segs[0].v_src == NULL).
  * This is the O(L) of PAPER.md:143 and the numerator of every GB/s this repository reports. */
 KVR_API uint64_t kvr_bytes_moved(const kvr_model_desc* model, const kvr_segment* segs, int32_t n_segs);
 

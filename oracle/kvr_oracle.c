@@ -190,9 +190,9 @@ int kvr_oracle_rotate_f64(const double* x, double* out, int64_t n, int head_dim,
  * Returns KVRO_ERR_OUT_OF_RANGE (and writes nothing at all) if any block-table
  * entry the segment touches is < 0 or >= num_blocks (reading R12).
  */
-int kvr_oracle_reposition_splice(
+static int splice_core(
     /* model */
-    int layers, int kv_heads, int head_dim, int rotary_dim, int pairing, int dtype,
+    int layers, int kv_heads, int head_dim, int rotary_dim, int rotary_offset, int pairing, int dtype,
     const double* inv_freq,
     /* destination paged pool */
     void* k_cache, void* v_cache,
@@ -207,9 +207,11 @@ int kvr_oracle_reposition_splice(
     const int32_t* pos_map, const float* k_scale_src,
     /* control */
     int layer_begin, int layer_end, int n_threads) {
-  if (!inv_freq || !k_cache || !v_cache || !block_table || !k_src || !v_src) return KVRO_ERR_INVALID_ARG;
+  if (!inv_freq || !k_cache || !block_table || !k_src) return KVRO_ERR_INVALID_ARG;
+  if ((v_cache == NULL) != (v_src == NULL)) return KVRO_ERR_INVALID_ARG; /* K-only (reading R23): both absent */
   if (layers <= 0 || kv_heads <= 0 || head_dim <= 0) return KVRO_ERR_INVALID_ARG;
-  if (rotary_dim < 2 || (rotary_dim & 1) || rotary_dim > head_dim) return KVRO_ERR_INVALID_ARG;
+  if (rotary_dim < 2 || (rotary_dim & 1) || rotary_offset < 0 || rotary_offset + rotary_dim > head_dim)
+    return KVRO_ERR_INVALID_ARG;
   if (pairing != KVRO_PAIR_NEOX_HALF && pairing != KVRO_PAIR_GPTJ_INTERLEAVED) return KVRO_ERR_INVALID_ARG;
   if (dtype != KVRO_BF16 && dtype != KVRO_FP8_E4M3) return KVRO_ERR_INVALID_ARG;
   if (dtype == KVRO_FP8_E4M3 && !k_scale_dst) return KVRO_ERR_INVALID_ARG;
@@ -248,21 +250,21 @@ int kvr_oracle_reposition_splice(
         int64_t src_e = (int64_t)l * src_stride_layer + (int64_t)h * src_stride_head +
                         (int64_t)t * src_stride_token;
         const uint8_t* ks = (const uint8_t*)k_src + src_e * esz;
-        const uint8_t* vs = (const uint8_t*)v_src + src_e * esz;
         uint8_t* kd = (uint8_t*)k_cache + dst_e * esz;
-        uint8_t* vd = (uint8_t*)v_cache + dst_e * esz;
 
-        /* V: position-free, copied unchanged */
-        memcpy(vd, vs, (size_t)head_dim * esz);
+        /* V: position-free, copied unchanged; absent for a latent cache (R23) */
+        if (v_src)
+          memcpy((uint8_t*)v_cache + dst_e * esz, (const uint8_t*)v_src + src_e * esz, (size_t)head_dim * esz);
 
         /* K: start from a byte copy -- this is the whole answer for the pass-through
-         * dims [R, D) and for Delta == 0 with equal scales (readings R13, R8) */
+         * dims (outside the rotary window) and for Delta == 0 with equal scales (readings R13, R8) */
         memcpy(kd, ks, (size_t)head_dim * esz);
         if (dtype == KVRO_BF16) {
           if (delta == 0) continue;
           for (int i = 0; i < rotary_dim / 2; ++i) {
             int ia, ib;
             pair_indices(pairing, rotary_dim, i, &ia, &ib);
+            ia += rotary_offset; ib += rotary_offset; /* the rotary window starts at rotary_offset (R23) */
             double phi = (double)delta * inv_freq[i];
             double c = cos(phi), s = sin(phi);
             uint16_t ua, ub;
@@ -279,6 +281,7 @@ int kvr_oracle_reposition_splice(
           for (int i = 0; i < rotary_dim / 2; ++i) {
             int ia, ib;
             pair_indices(pairing, rotary_dim, i, &ia, &ib);
+            ia += rotary_offset; ib += rotary_offset; /* the rotary window starts at rotary_offset (R23) */
             double phi = (double)delta * inv_freq[i];
             double c = (delta == 0) ? 1.0 : cos(phi), s = (delta == 0) ? 0.0 : sin(phi);
             double a = kvr_oracle_e4m3_decode(ks[ia]) * s_src;
@@ -287,13 +290,62 @@ int kvr_oracle_reposition_splice(
             kd[ib] = kvr_oracle_e4m3_encode_sat((b * c + a * s) / s_dst);
           }
           if (s_src != s_dst) /* pass-through dims are re-expressed in the new scale */
-            for (int d = rotary_dim; d < head_dim; ++d)
-              kd[d] = kvr_oracle_e4m3_encode_sat(kvr_oracle_e4m3_decode(ks[d]) * s_src / s_dst);
+            for (int d = 0; d < head_dim; ++d)
+              if (d < rotary_offset || d >= rotary_offset + rotary_dim)
+                kd[d] = kvr_oracle_e4m3_encode_sat(kvr_oracle_e4m3_decode(ks[d]) * s_src / s_dst);
         }
       }
     }
   }
   return KVRO_OK;
+}
+
+
+/* The hot path as BASELINE.json states it: rotary dims [0, R), K and V both present. */
+int kvr_oracle_reposition_splice(
+    int layers, int kv_heads, int head_dim, int rotary_dim, int pairing, int dtype, const double* inv_freq,
+    void* k_cache, void* v_cache,
+    int64_t stride_layer, int64_t stride_block, int64_t stride_token, int64_t stride_head,
+    int num_blocks, int block_size, const int32_t* block_table, int num_seqs, int max_blocks_per_seq,
+    const float* k_scale_dst,
+    const void* k_src, const void* v_src,
+    int64_t src_stride_layer, int64_t src_stride_head, int64_t src_stride_token,
+    int len, int old_start, int new_start, int dst_seq, int dst_token_start,
+    const int32_t* pos_map, const float* k_scale_src,
+    int layer_begin, int layer_end, int n_threads) {
+  if (!v_cache || !v_src) return KVRO_ERR_INVALID_ARG;
+  return splice_core(layers, kv_heads, head_dim, rotary_dim, 0, pairing, dtype, inv_freq, k_cache, v_cache,
+                     stride_layer, stride_block, stride_token, stride_head, num_blocks, block_size, block_table,
+                     num_seqs, max_blocks_per_seq, k_scale_dst, k_src, v_src, src_stride_layer, src_stride_head,
+                     src_stride_token, len, old_start, new_start, dst_seq, dst_token_start, pos_map, k_scale_src,
+                     layer_begin, layer_end, n_threads);
+}
+
+/*
+ * NEXT-3 representation adapter (reading R23).  PAPER.md:215 (sec. 8): "MLA (DeepSeek-V2/Coder-V2) caches a
+ * position-free latent plus a small decoupled-RoPE sub-vector; our decoupled k_pe reposition re-rotates only that
+ * sub-vector"; PAPER.md:514 (Fig. 22a): "repositioning re-rotates only k_pe and copies the latent as-is".
+ * A cached row is [latent c_t | k_pe]: the rotary pairs live in dims [rotary_offset, rotary_offset + rotary_dim)
+ * and every other dim is copied unchanged; such a cache has no separate V tensor (v_cache == v_src == NULL).
+ * Same definition otherwise; rotary_offset = 0 with V present is kvr_oracle_reposition_splice.
+ */
+int kvr_oracle_reposition_splice_ex(
+    int layers, int kv_heads, int head_dim, int rotary_dim, int rotary_offset, int pairing, int dtype,
+    const double* inv_freq,
+    void* k_cache, void* v_cache,
+    int64_t stride_layer, int64_t stride_block, int64_t stride_token, int64_t stride_head,
+    int num_blocks, int block_size, const int32_t* block_table, int num_seqs, int max_blocks_per_seq,
+    const float* k_scale_dst,
+    const void* k_src, const void* v_src,
+    int64_t src_stride_layer, int64_t src_stride_head, int64_t src_stride_token,
+    int len, int old_start, int new_start, int dst_seq, int dst_token_start,
+    const int32_t* pos_map, const float* k_scale_src,
+    int layer_begin, int layer_end, int n_threads) {
+  return splice_core(layers, kv_heads, head_dim, rotary_dim, rotary_offset, pairing, dtype, inv_freq, k_cache,
+                     v_cache, stride_layer, stride_block, stride_token, stride_head, num_blocks, block_size,
+                     block_table, num_seqs, max_blocks_per_seq, k_scale_dst, k_src, v_src, src_stride_layer,
+                     src_stride_head, src_stride_token, len, old_start, new_start, dst_seq, dst_token_start,
+                     pos_map, k_scale_src, layer_begin, layer_end, n_threads);
 }
 
 /* ------------------------------------------------- in-place reposition (NEXT-1) */
@@ -310,8 +362,8 @@ int kvr_oracle_reposition_splice(
  * source and the destination scale.  Delta_t == 0 leaves the row's bytes alone.
  * Returns KVRO_ERR_OUT_OF_RANGE, writing nothing, if a touched block-table entry is invalid.
  */
-int kvr_oracle_reposition_inplace(
-    int layers, int kv_heads, int head_dim, int rotary_dim, int pairing, int dtype,
+static int inplace_core(
+    int layers, int kv_heads, int head_dim, int rotary_dim, int rotary_offset, int pairing, int dtype,
     const double* inv_freq,
     void* k_cache,
     int64_t stride_layer, int64_t stride_block, int64_t stride_token, int64_t stride_head,
@@ -322,7 +374,8 @@ int kvr_oracle_reposition_inplace(
     int layer_begin, int layer_end, int n_threads) {
   if (!inv_freq || !k_cache || !block_table) return KVRO_ERR_INVALID_ARG;
   if (layers <= 0 || kv_heads <= 0 || head_dim <= 0) return KVRO_ERR_INVALID_ARG;
-  if (rotary_dim < 2 || (rotary_dim & 1) || rotary_dim > head_dim) return KVRO_ERR_INVALID_ARG;
+  if (rotary_dim < 2 || (rotary_dim & 1) || rotary_offset < 0 || rotary_offset + rotary_dim > head_dim)
+    return KVRO_ERR_INVALID_ARG;
   if (pairing != KVRO_PAIR_NEOX_HALF && pairing != KVRO_PAIR_GPTJ_INTERLEAVED) return KVRO_ERR_INVALID_ARG;
   if (dtype != KVRO_BF16 && dtype != KVRO_FP8_E4M3) return KVRO_ERR_INVALID_ARG;
   if (dtype == KVRO_FP8_E4M3 && !k_scale) return KVRO_ERR_INVALID_ARG;
@@ -355,6 +408,7 @@ int kvr_oracle_reposition_inplace(
         for (int i = 0; i < rotary_dim / 2; ++i) {
           int ia, ib;
           pair_indices(pairing, rotary_dim, i, &ia, &ib);
+          ia += rotary_offset; ib += rotary_offset;
           double phi = (double)delta * inv_freq[i];
           double c = cos(phi), s = sin(phi);
           if (dtype == KVRO_BF16) {
@@ -377,6 +431,34 @@ int kvr_oracle_reposition_inplace(
     }
   }
   return KVRO_OK;
+}
+
+int kvr_oracle_reposition_inplace(
+    int layers, int kv_heads, int head_dim, int rotary_dim, int pairing, int dtype, const double* inv_freq,
+    void* k_cache, int64_t stride_layer, int64_t stride_block, int64_t stride_token, int64_t stride_head,
+    int num_blocks, int block_size, const int32_t* block_table, int num_seqs, int max_blocks_per_seq,
+    const float* k_scale,
+    int seq, int token_start, int len, int old_start, int new_start, const int32_t* pos_map,
+    int layer_begin, int layer_end, int n_threads) {
+  return inplace_core(layers, kv_heads, head_dim, rotary_dim, 0, pairing, dtype, inv_freq, k_cache, stride_layer,
+                      stride_block, stride_token, stride_head, num_blocks, block_size, block_table, num_seqs,
+                      max_blocks_per_seq, k_scale, seq, token_start, len, old_start, new_start, pos_map,
+                      layer_begin, layer_end, n_threads);
+}
+
+/* In-place re-float of a resident [latent | k_pe] chunk: only the rotary window moves (R23). */
+int kvr_oracle_reposition_inplace_ex(
+    int layers, int kv_heads, int head_dim, int rotary_dim, int rotary_offset, int pairing, int dtype,
+    const double* inv_freq,
+    void* k_cache, int64_t stride_layer, int64_t stride_block, int64_t stride_token, int64_t stride_head,
+    int num_blocks, int block_size, const int32_t* block_table, int num_seqs, int max_blocks_per_seq,
+    const float* k_scale,
+    int seq, int token_start, int len, int old_start, int new_start, const int32_t* pos_map,
+    int layer_begin, int layer_end, int n_threads) {
+  return inplace_core(layers, kv_heads, head_dim, rotary_dim, rotary_offset, pairing, dtype, inv_freq, k_cache,
+                      stride_layer, stride_block, stride_token, stride_head, num_blocks, block_size, block_table,
+                      num_seqs, max_blocks_per_seq, k_scale, seq, token_start, len, old_start, new_start, pos_map,
+                      layer_begin, layer_end, n_threads);
 }
 
 /* Algorithmic bytes of one segment: read K, read V, write K, write V. */

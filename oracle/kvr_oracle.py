@@ -45,6 +45,21 @@ def lib():
             [C.c_void_p, C.c_void_p] + [C.c_int64] * 3 + [C.c_int] * 5 +
             [C.c_void_p, C.c_void_p] +                            # segment
             [C.c_int] * 3)                                        # control
+        _lib.kvr_oracle_reposition_splice_ex.restype = C.c_int
+        _lib.kvr_oracle_reposition_splice_ex.argtypes = (
+            [C.c_int] * 7 + [C.c_void_p] +                      # model (+ rotary_offset)
+            [C.c_void_p, C.c_void_p] + [C.c_int64] * 4 + [C.c_int, C.c_int] +
+            [C.c_void_p, C.c_int, C.c_int, C.c_void_p] +
+            [C.c_void_p, C.c_void_p] + [C.c_int64] * 3 + [C.c_int] * 5 +
+            [C.c_void_p, C.c_void_p] +
+            [C.c_int] * 3)
+        _lib.kvr_oracle_reposition_inplace_ex.restype = C.c_int
+        _lib.kvr_oracle_reposition_inplace_ex.argtypes = (
+            [C.c_int] * 7 + [C.c_void_p] +
+            [C.c_void_p] + [C.c_int64] * 4 + [C.c_int, C.c_int] +
+            [C.c_void_p, C.c_int, C.c_int, C.c_void_p] +
+            [C.c_int] * 5 + [C.c_void_p] +
+            [C.c_int] * 3)
         _lib.kvr_oracle_reposition_inplace.restype = C.c_int
         _lib.kvr_oracle_reposition_inplace.argtypes = (
             [C.c_int] * 6 + [C.c_void_p] +                      # model
@@ -120,8 +135,10 @@ def reposition_splice(*, layers, kv_heads, head_dim, rotary_dim, pairing, dtype,
                       k_src, v_src, src_stride_layer, src_stride_head, src_stride_token,
                       len, old_start, new_start, dst_seq, dst_token_start,
                       pos_map=None, k_scale_src=None,
-                      layer_begin=0, layer_end=None, n_threads=1):
-    """Splices ONE segment into (k_cache, v_cache) in place.  Returns the status code."""
+                      layer_begin=0, layer_end=None, n_threads=1, rotary_offset=0):
+    """Splices ONE segment into (k_cache, v_cache) in place.  Returns the status code.
+    rotary_offset != 0 or v_cache is None / v_src is None (a [latent | k_pe] cache, reading R23) go through
+    kvr_oracle_reposition_splice_ex."""
     edt = np.uint16 if dtype == BF16 else np.uint8
     inv_freq = np.ascontiguousarray(inv_freq, dtype=np.float64)
     assert inv_freq.shape == (rotary_dim // 2,)
@@ -129,6 +146,16 @@ def reposition_splice(*, layers, kv_heads, head_dim, rotary_dim, pairing, dtype,
     num_seqs, max_blocks = block_table.shape
     if layer_end is None:
         layer_end = layers
+    if rotary_offset != 0 or v_cache is None or v_src is None:
+        return lib().kvr_oracle_reposition_splice_ex(
+            layers, kv_heads, head_dim, rotary_dim, rotary_offset, pairing, dtype, _ptr(inv_freq),
+            _ptr(k_cache, edt, True), _ptr(v_cache, edt, True),
+            stride_layer, stride_block, stride_token, stride_head, num_blocks, block_size,
+            _ptr(block_table, np.int32), num_seqs, max_blocks, _ptr(k_scale_dst, np.float32),
+            _ptr(k_src, edt), _ptr(v_src, edt), src_stride_layer, src_stride_head, src_stride_token,
+            len, old_start, new_start, dst_seq, dst_token_start,
+            _ptr(pos_map, np.int32), _ptr(k_scale_src, np.float32),
+            layer_begin, layer_end, n_threads)
     return lib().kvr_oracle_reposition_splice(
         layers, kv_heads, head_dim, rotary_dim, pairing, dtype, _ptr(inv_freq),
         _ptr(k_cache, edt, True), _ptr(v_cache, edt, True),
@@ -144,7 +171,7 @@ def reposition_inplace(*, layers, kv_heads, head_dim, rotary_dim, pairing, dtype
                        k_cache, stride_layer, stride_block, stride_token, stride_head,
                        num_blocks, block_size, block_table, k_scale=None,
                        seq, token_start, len, old_start, new_start, pos_map=None,
-                       layer_begin=0, layer_end=None, n_threads=1):
+                       layer_begin=0, layer_end=None, n_threads=1, rotary_offset=0):
     """Re-rotates ONE resident span of k_cache in place (kvr_oracle_reposition_inplace).  Returns the status."""
     edt = np.uint16 if dtype == BF16 else np.uint8
     inv_freq = np.ascontiguousarray(inv_freq, dtype=np.float64)
@@ -153,6 +180,13 @@ def reposition_inplace(*, layers, kv_heads, head_dim, rotary_dim, pairing, dtype
     num_seqs, max_blocks = block_table.shape
     if layer_end is None:
         layer_end = layers
+    if rotary_offset != 0:
+        return lib().kvr_oracle_reposition_inplace_ex(
+            layers, kv_heads, head_dim, rotary_dim, rotary_offset, pairing, dtype, _ptr(inv_freq),
+            _ptr(k_cache, edt, True), stride_layer, stride_block, stride_token, stride_head,
+            num_blocks, block_size, _ptr(block_table, np.int32), num_seqs, max_blocks, _ptr(k_scale, np.float32),
+            seq, token_start, len, old_start, new_start, _ptr(pos_map, np.int32),
+            layer_begin, layer_end, n_threads)
     return lib().kvr_oracle_reposition_inplace(
         layers, kv_heads, head_dim, rotary_dim, pairing, dtype, _ptr(inv_freq),
         _ptr(k_cache, edt, True), stride_layer, stride_block, stride_token, stride_head,
@@ -184,18 +218,20 @@ def splice_workload(w, srcs, k_cache, v_cache, n_threads=1, layer_begin=0, layer
         if segments is not None and i not in segments:
             continue
         k_src, v_src = srcs[i]
+        no_v = v_src is None or v_cache is None      # a [latent | k_pe] cache has no V tensor (R23)
         sl, sh, st = w.src_strides(seg)
         status = reposition_splice(
             layers=w.layers, kv_heads=w.kv_heads, head_dim=w.head_dim, rotary_dim=w.rotary_dim,
             pairing=_PAIRING[w.pairing], dtype=_DTYPE[w.dtype], inv_freq=w.inv_freq,
-            k_cache=k_cache, v_cache=v_cache, stride_layer=s_l, stride_block=s_b, stride_token=s_t,
+            k_cache=k_cache, v_cache=None if no_v else v_cache, stride_layer=s_l, stride_block=s_b, stride_token=s_t,
             stride_head=s_h, num_blocks=w.num_blocks, block_size=w.block_size, block_table=w.block_table,
             k_scale_dst=w.k_scale, k_src=np.ascontiguousarray(k_src).reshape(-1),
-            v_src=np.ascontiguousarray(v_src).reshape(-1),
+            v_src=None if no_v else np.ascontiguousarray(v_src).reshape(-1),
             src_stride_layer=sl, src_stride_head=sh, src_stride_token=st,
             len=seg.len, old_start=seg.old_start, new_start=seg.new_start, dst_seq=seg.dst_seq,
             dst_token_start=seg.dst_token_start, pos_map=seg.pos_map, k_scale_src=w.k_scale_src,
-            layer_begin=layer_begin, layer_end=layer_end, n_threads=n_threads)
+            layer_begin=layer_begin, layer_end=layer_end, n_threads=n_threads,
+            rotary_offset=getattr(w, "rotary_offset", 0))
         if status != OK:
             raise RuntimeError(f"oracle: segment {i} -> status {status}")
 
@@ -212,6 +248,7 @@ def inplace_workload(w, k_cache, n_threads=1, layer_begin=0, layer_end=None, del
             stride_layer=s_l, stride_block=s_b, stride_token=s_t, stride_head=s_h, num_blocks=w.num_blocks,
             block_size=w.block_size, block_table=w.block_table, k_scale=w.k_scale,
             seq=seg.dst_seq, token_start=seg.dst_token_start, len=seg.len, old_start=max(0, -d), new_start=max(0, d),
-            layer_begin=layer_begin, layer_end=layer_end, n_threads=n_threads)
+            layer_begin=layer_begin, layer_end=layer_end, n_threads=n_threads,
+            rotary_offset=getattr(w, "rotary_offset", 0))
         if status != OK:
             raise RuntimeError(f"oracle in-place: segment {i} -> status {status}")

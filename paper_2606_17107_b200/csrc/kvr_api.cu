@@ -30,10 +30,13 @@ inline int elt_bytes(int dtype) { return dtype == KVR_BF16 ? 2 : 1; }
 kvr_status check_model(const kvr_model_desc* m) {
   if (!m || !m->inv_freq) return KVR_ERR_INVALID_ARG;
   if (m->layers <= 0 || m->kv_heads <= 0 || m->head_dim <= 0) return KVR_ERR_INVALID_ARG;
-  if (m->rotary_dim < 2 || (m->rotary_dim & 1) || m->rotary_dim > m->head_dim) return KVR_ERR_INVALID_ARG;
+  if (m->rotary_dim < 2 || (m->rotary_dim & 1) || m->rotary_offset < 0 || m->reserved_ != 0 ||
+      (int64_t)m->rotary_offset + m->rotary_dim > m->head_dim)
+    return KVR_ERR_INVALID_ARG;
   if (m->pairing != KVR_PAIR_NEOX_HALF && m->pairing != KVR_PAIR_GPTJ_INTERLEAVED) return KVR_ERR_INVALID_ARG;
   if (m->dtype != KVR_BF16 && m->dtype != KVR_FP8_E4M3) return KVR_ERR_INVALID_ARG;
   if (((int64_t)m->head_dim * elt_bytes(m->dtype)) % 16 != 0) return KVR_ERR_ALIGNMENT;
+  if (((int64_t)m->rotary_offset * elt_bytes(m->dtype)) % 16 != 0) return KVR_ERR_ALIGNMENT;
   return KVR_OK;
 }
 
@@ -43,7 +46,8 @@ kvr_status check_call(const kvr_model_desc* m, const kvr_paged_dst* d, const kvr
   kvr_status st = check_model(m);
   if (st != KVR_OK) return st;
   if (!d || n < 0 || (n > 0 && !segs)) return KVR_ERR_INVALID_ARG;
-  if (!d->k_cache || !d->v_cache || !d->block_table) return KVR_ERR_INVALID_ARG;
+  if (!d->k_cache || !d->block_table) return KVR_ERR_INVALID_ARG;
+  const bool k_only = (d->v_cache == nullptr);   // a [latent | k_pe] cache: one tensor per token (kvr.h, NEXT-3)
   if (d->num_blocks <= 0 || d->block_size <= 0 || d->num_seqs <= 0 || d->max_blocks_per_seq <= 0)
     return KVR_ERR_INVALID_ARG;
   if (d->stride_layer < 0 || d->stride_block <= 0 || (d->stride_token < m->head_dim && d->block_size > 1))
@@ -58,7 +62,7 @@ kvr_status check_call(const kvr_model_desc* m, const kvr_paged_dst* d, const kvr
   const int64_t cap = (int64_t)d->max_blocks_per_seq * d->block_size;
   for (int32_t i = 0; i < n; ++i) {
     const kvr_segment& s = segs[i];
-    if (!s.k_src || !s.v_src) return KVR_ERR_INVALID_ARG;
+    if (!s.k_src || (s.v_src == nullptr) != k_only) return KVR_ERR_INVALID_ARG;
     if (s.len <= 0 || s.dst_seq < 0 || s.dst_seq >= d->num_seqs || s.dst_token_start < 0)
       return KVR_ERR_INVALID_ARG;
     if (s.old_start < 0 || (!s.pos_map && s.new_start < 0)) return KVR_ERR_INVALID_ARG;
@@ -226,7 +230,8 @@ uint64_t kvr_bytes_moved(const kvr_model_desc* m, const kvr_segment* segs, int32
   if (!m || (n > 0 && !segs)) return 0;
   uint64_t tokens = 0;
   for (int32_t i = 0; i < n; ++i) tokens += segs[i].len > 0 ? (uint64_t)segs[i].len : 0u;
-  return 4ull * (uint64_t)m->layers * (uint64_t)m->kv_heads * (uint64_t)m->head_dim *
+  const uint64_t tensors = (n > 0 && segs[0].v_src == nullptr) ? 2ull : 4ull;   // K-only: read K, write K
+  return tensors * (uint64_t)m->layers * (uint64_t)m->kv_heads * (uint64_t)m->head_dim *
          (uint64_t)elt_bytes(m->dtype) * tokens;
 }
 
@@ -259,6 +264,8 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   const int E = elt_bytes(m.dtype);
   CallParams P{};
   P.layers = m.layers; P.heads = m.kv_heads; P.head_dim = m.head_dim; P.rotary_dim = m.rotary_dim;
+  P.rotary_offset = m.rotary_offset;
+  P.no_v = (inplace || d->v_cache == nullptr) ? 1 : 0;
   P.pairing = m.pairing; P.dtype = m.dtype; P.inv_freq = c->d_inv_freq;
   P.k_cache = static_cast<uint8_t*>(d->k_cache) + (int64_t)l0 * d->stride_layer * E;
   P.v_cache = d->v_cache ? static_cast<uint8_t*>(d->v_cache) + (int64_t)l0 * d->stride_layer * E : nullptr;
@@ -295,7 +302,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       SegDev& o = slot.host[i];
       const int64_t src_adv = src_group_local ? 0 : (int64_t)l0 * s.src_stride_layer * E;
       o.k_src = static_cast<const uint8_t*>(s.k_src) + src_adv;
-      o.v_src = static_cast<const uint8_t*>(s.v_src) + src_adv;
+      o.v_src = s.v_src ? static_cast<const uint8_t*>(s.v_src) + src_adv : nullptr;
       o.pos_map = s.pos_map;
       o.k_scale_src = s.k_scale_src ? s.k_scale_src : d->k_scale;
       if (o.k_scale_src) o.k_scale_src += (int64_t)l0 * m.kv_heads;
@@ -334,6 +341,11 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     if (inplace && d->stride_token != m.head_dim) {
       // token-major pool, in place: a tile is cg tokens x ALL heads (one contiguous run); keep it near 8 KB
       cg_limit = (int)(8192 / ((int64_t)m.kv_heads * m.head_dim * E));
+      cg_limit = cg_limit < 1 ? 1 : (cg_limit > 16 ? 16 : cg_limit);
+    }
+    if ((int64_t)m.head_dim * E > 1024) {
+      // long rows (MLA [latent | k_pe] = 1152 B): keep a tile near 8-16 KB so the ring still holds >= 6 stages
+      cg_limit = (int)(16384 / ((int64_t)m.head_dim * E));
       cg_limit = cg_limit < 1 ? 1 : (cg_limit > 16 ? 16 : cg_limit);
     }
     decompose(chunk_granularity(d->block_size, cg_limit), tu.layers_per_unit, tu.hsplit);
@@ -433,7 +445,8 @@ kvr_status kvr_reposition_splice_host(kvr_ctx* c, const kvr_paged_dst* d, const 
   if (cap != cudaStreamCaptureStatusNone) return KVR_ERR_UNSUPPORTED;   // allocates and uses a second stream
 
   // ---- layer-group size: staging buffer of <= ~256 MB, at least one layer ----
-  const size_t layer_bytes = 2u * (size_t)tokens * m.kv_heads * m.head_dim * E;   // K + V of one layer, all segments
+  const bool k_only = (d->v_cache == nullptr);
+  const size_t layer_bytes = (k_only ? 1u : 2u) * (size_t)tokens * m.kv_heads * m.head_dim * E;   // K (+ V) of one layer, all segments
   int lg = (int)((256ull << 20) / (layer_bytes ? layer_bytes : 1));
   if (lg < 1) lg = 1;
   if (lg > m.layers) lg = m.layers;
@@ -497,9 +510,11 @@ kvr_status kvr_reposition_splice_host(kvr_ctx* c, const kvr_paged_dst* d, const 
       const size_t off = (size_t)l0 * s.src_stride_layer * E;
       KVR_CUDA(c, cudaMemcpyAsync(at, static_cast<const uint8_t*>(s.k_src) + off, run, cudaMemcpyHostToDevice, c->copy_stream));
       dsegs[i].k_src = at; at += run;
+      c->h2d_bytes += run;
+      if (k_only) continue;
       KVR_CUDA(c, cudaMemcpyAsync(at, static_cast<const uint8_t*>(s.v_src) + off, run, cudaMemcpyHostToDevice, c->copy_stream));
       dsegs[i].v_src = at; at += run;
-      c->h2d_bytes += 2 * run;
+      c->h2d_bytes += run;
     }
     KVR_CUDA(c, cudaEventRecord(c->stage_filled[b], c->copy_stream));
     KVR_CUDA(c, cudaStreamWaitEvent(stream, c->stage_filled[b], 0));

@@ -40,6 +40,8 @@ struct CallParams {
   // model
   int32_t layers, heads, head_dim, rotary_dim, pairing, dtype;
   const double* inv_freq;      // DEVICE, rotary_dim/2
+  int32_t rotary_offset;       // first rotary dim of a row (kvr.h: MLA k_pe window); 0 for ordinary K caches
+  int32_t pad0_;
   // destination
   uint8_t* k_cache;
   uint8_t* v_cache;
@@ -62,7 +64,7 @@ struct CallParams {
   unsigned long long* sched;
   int32_t grab;                // units handed out per atomic
   int32_t hsplit;              // ring kernel: a (chunk, layer group) is split into hsplit units over its head groups
-  int32_t pad_;
+  int32_t no_v;                // V is neither read nor written (in-place calls; K-only [latent | k_pe] caches)
   int32_t inplace;             // kvr_reposition_inplace: K rows are read from the pool slot they are written back to; no V
   SegDev inline_segs[kInlineSegs];
 };
@@ -162,6 +164,7 @@ struct RingConfig {
   int ctas_per_sm, consumer_warps, stages, v_bulk_store, max_ctas, grab, pdl;
 };
 int ring_heads_per_tile(const CallParams& P);   // heads one tile of the ring kernel covers (needs P.cg)
+bool ring_window_mode(const CallParams& P);      // rows outside the power-of-two slot layout (e.g. MLA [latent | k_pe])
 bool ring_supported(const CallParams& P, const SegDev* host_segs, const char** why);
 cudaError_t launch_ring(const CallParams& P, const RingConfig& cfg, int sm_count, cudaStream_t stream,
                         int* grid, int* block, int* smem);

@@ -7,6 +7,7 @@
 //   3. K rotary pairs, scalar element loads (a2, a3, a5); K pass-through dims; V 16-byte copies (a6)
 // Steps refer to SURVEY.md 8(a) / DESIGN.md "Path".  With P.inplace (kvr_reposition_inplace, R20) the K row
 // is read from the pool slot it is written back to, and pass-through dims and V are left alone.
+// P.rotary_offset / P.no_v: the MLA adapter of kvr.h (rotary window inside the row; no V tensor).
 #include "kvr_common.cuh"
 
 namespace kvr {
@@ -54,8 +55,8 @@ __global__ void __launch_bounds__(256) kvr_generic_kernel(const __grid_constant_
       int t = row % ch.n_tok;
       int h = (row / ch.n_tok) % P.heads;
       int l = l0 + row / (ch.n_tok * P.heads);
-      int ia = (P.pairing == 0) ? i : 2 * i;
-      int ib = (P.pairing == 0) ? i + half : 2 * i + 1;
+      int ia = P.rotary_offset + ((P.pairing == 0) ? i : 2 * i);          // the rotary window starts at rotary_offset
+      int ib = P.rotary_offset + ((P.pairing == 0) ? i + half : 2 * i + 1);
       uint8_t* dst = P.k_cache + ((int64_t)l * P.d_sl + (int64_t)h * P.d_sh + (int64_t)t * P.d_st + dst_base) * E;
       const uint8_t* src = P.inplace ? dst      // each pair is read and written by this one thread: aliasing-safe
                                      : s.k_src + ((int64_t)l * s.sl + (int64_t)h * s.sh + (int64_t)(ch.t0 + t) * s.st) * E;
@@ -85,10 +86,11 @@ __global__ void __launch_bounds__(256) kvr_generic_kernel(const __grid_constant_
       }
     }
     if (P.inplace) continue;   // pass-through dims and V already hold their bytes
-    // ---- K pass-through dims [R, D) ----
+    // ---- K pass-through dims: [0, rotary_offset) and [rotary_offset + R, D) ----
     const int pass = D - R;
     for (int64_t idx = threadIdx.x; idx < (int64_t)rows * pass; idx += blockDim.x) {
-      int d = R + (int)(idx % pass);
+      int d = (int)(idx % pass);
+      if (d >= P.rotary_offset) d += R;
       int row = (int)(idx / pass);
       int t = row % ch.n_tok;
       int h = (row / ch.n_tok) % P.heads;
@@ -104,6 +106,7 @@ __global__ void __launch_bounds__(256) kvr_generic_kernel(const __grid_constant_
         dst[d] = q;
       }
     }
+    if (P.no_v) continue;      // K-only call: a [latent | k_pe] cache has no V tensor
     // ---- V: unchanged bytes, 16 B at a time (rows are 16-byte multiples and 16-byte aligned) ----
     const int vecs = D * E / 16;
     for (int64_t idx = threadIdx.x; idx < (int64_t)rows * vecs; idx += blockDim.x) {

@@ -36,7 +36,12 @@ struct RingParams {
   int v_bulk;                             // V leaves shared memory by bulk stores (needs stride_token == head_dim)
   int n_scales;                           // fp8: layers * heads destination scales preloaded to shared memory
   int off_ub, n_ub;                       // segments' first-unit prefix sums in shared memory (calls with many segments)
-  int no_v;                               // in-place mode: a stage holds K only and V is never touched
+  int no_v;                               // in-place / K-only calls: a stage holds K only and V is never touched
+  int win;                                // WINDOW mode (rows that are not a power of two, or rotary_offset != 0, e.g. the
+                                          // MLA [latent | k_pe] row): lanes are laid over the rotary window only and the
+                                          // rest of the row is moved by a plain 16-byte copy loop
+  int nv_slot;                            // vectors the lane slots are laid over: nv, or nr in window mode
+  int ro_v;                               // rotary_offset in 16-byte vectors
   int ip_mode;                            // in-place source runs: 0 one run per head (d_st == head_dim), 1 one run for the
                                           // whole tile (token-major pool, all heads in the tile), 2 one copy per row
 };
@@ -366,7 +371,7 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
               m.n_tok = n_tok; m.flags = flags; m.tab = tb; m.gen = gen;
               m.scale_idx = l * P.heads + h0; m.seg = si;
               meta[my_stage] = m;
-              mbar_arrive_expect_tx(bar, (inplace ? 1u : 2u) * RP.hpt * run_bytes);
+              mbar_arrive_expect_tx(bar, (RP.no_v ? 1u : 2u) * RP.hpt * run_bytes);
               const uint32_t sk = s_base + RP.off_stage + (uint32_t)my_stage * RP.stage_bytes;
               const uint32_t sv = sk + RP.tile_bytes;
               if (inplace) {
@@ -389,11 +394,11 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
                 const uint32_t so = (uint32_t)(hh * RP.cg * RP.rowB);
                 if (packed_rows) {
                   bulk_g2s(sk + so, sg.k_src + src_off, run_bytes, bar, pol);
-                  bulk_g2s(sv + so, sg.v_src + src_off, run_bytes, bar, pol);
+                  if (!RP.no_v) bulk_g2s(sv + so, sg.v_src + src_off, run_bytes, bar, pol);
                 } else {
                   for (int r = 0; r < n_tok; ++r) {
                     bulk_g2s(sk + so + r * RP.rowB, sg.k_src + src_off + (int64_t)r * sg.st * E, RP.rowB, bar, pol);
-                    bulk_g2s(sv + so + r * RP.rowB, sg.v_src + src_off + (int64_t)r * sg.st * E, RP.rowB, bar, pol);
+                    if (!RP.no_v) bulk_g2s(sv + so + r * RP.rowB, sg.v_src + src_off + (int64_t)r * sg.st * E, RP.rowB, bar, pol);
                   }
                 }
               }
@@ -439,8 +444,8 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
 
   // ============================================================================= CONSUMERS
   const int sp = RP.sp, q = lane & (sp - 1), rsub = lane >> RP.log_sp, rpi = RP.rpi;
-  const int nv = RP.nv, nr = RP.nr;
-  // this lane's slot: two 16-byte vectors (va, vb) of every row it visits
+  const int nv = RP.nv, nr = RP.nr, nvs = RP.nv_slot;
+  // this lane's slot: two 16-byte vectors (va, vb) of every row it visits (of its rotary window in window mode)
   int va, vb;
   bool rot_a, rot_b;
   int tpos[G::NT];               // table positions of this lane's pairs (only used if rotary)
@@ -451,7 +456,7 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
 #pragma unroll
     for (int k = 0; k < G::NT; ++k) tpos[k] = rot_a ? tab_pos<G::PPV>(va * G::EPV + k, RP.NV) : 0;
   } else {
-    va = q; vb = q + (nv >> 1);
+    va = q; vb = q + (nvs >> 1);
     rot_a = va < nr; rot_b = vb < nr;
 #pragma unroll
     for (int k = 0; k < G::NT; ++k) {
@@ -460,6 +465,7 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       tpos[k] = r ? tab_pos<G::PPV>(v * G::PPV + (k % G::PPV), RP.NV) : 0;
     }
   }
+  va += RP.ro_v; vb += RP.ro_v;       // table positions above are relative to the window; addresses are not
   float4 T4[DTYPE == 0 ? G::NT : 1];
   float2 T2[DTYPE == 1 ? G::NT : 1];
   int my_gen = -1;
@@ -498,7 +504,8 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         const int total = n_tok * nv;
 #pragma unroll 4
         for (int idx = lane; idx < total; idx += 32) {
-          const int t = idx >> RP.log_nv, v = idx & (nv - 1);
+          int t, v;
+          if (RP.log_nv >= 0) { t = idx >> RP.log_nv; v = idx & (nv - 1); } else { t = idx / nv; v = idx - t * nv; }
           stg128(vd + (int64_t)t * P.d_st * E + v * 16, lds128(vs + idx * 16));
         }
       }
@@ -572,6 +579,18 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         stg128(row + va * 16, A);
         stg128(row + vb * 16, B);
       }
+      if (RP.win) {
+        // window mode: everything outside the rotary window (the MLA latent) is position-free -- 16-byte copies
+        const int npass = nv - nr, total = n_tok * npass;
+        for (int idx = lane; idx < total; idx += 32) {
+          const int t = idx / npass;
+          int v = idx - t * npass;
+          if (v >= RP.ro_v) v += nr;
+          uint4 A = lds128(ks + t * sm_st + v * 16);
+          if (DTYPE == 1 && requant) requant_fp8(A, s_src, inv_dst);
+          stg128(kd + (int64_t)t * P.d_st * E + v * 16, A);
+        }
+      }
     }
     if (RP.v_bulk == 2 || (RP.v_bulk && lane == 0)) bulk_wait_read0();   // V bytes have left shared memory
     __syncwarp();
@@ -596,11 +615,23 @@ int ring_heads_per_tile(const CallParams& P) {
   return P.heads;
 }
 
+// rows the power-of-two slot layout cannot take: the lanes cover the rotary window, a copy loop moves the rest
+bool ring_window_mode(const CallParams& P) {
+  const int rowB = P.head_dim * (P.dtype == 0 ? 2 : 1);
+  return P.rotary_offset != 0 || rowB > 1024 || (rowB & (rowB - 1)) != 0;
+}
+
 bool ring_supported(const CallParams& P, const SegDev* segs, const char** why) {
   const int E = P.dtype == 0 ? 2 : 1;
   const int rowB = P.head_dim * E;
   const char* w = nullptr;
-  if (rowB < 32 || rowB > 1024 || (rowB & (rowB - 1))) w = "head_dim*esz must be a power of two in [32, 1024] bytes";
+  const int rotB = P.rotary_dim * E;
+  if (ring_window_mode(P)) {
+    if (rowB < 32 || rowB > 4096 || rowB % 16) w = "window mode: head_dim*esz must be a multiple of 16 in [32, 4096] bytes";
+    else if (rotB % 32 || rotB > 1024 || ((rotB / 32) & (rotB / 32 - 1))) w = "window mode: rotary_dim*esz must be 32 * a power of two, <= 1024";
+    else if (P.inplace) w = "window mode: in-place calls take the generic kernel (it touches only the rotary window)";
+  }
+  else if (rowB < 32 || rowB > 1024 || (rowB & (rowB - 1))) w = "head_dim*esz must be a power of two in [32, 1024] bytes";
   else if (P.pairing == 0 && (P.rotary_dim * E) % 32) w = "NeoX pairing needs rotary_dim*esz % 32 == 0";
   else if (P.pairing == 1 && (P.rotary_dim * E) % 16) w = "GPT-J pairing needs rotary_dim*esz % 16 == 0";
   else if (P.dtype == 1 && (int64_t)P.layers * P.heads > 8192) w = "too many (layer, head) scales for shared memory";
@@ -635,13 +666,16 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   RingParams RP{};
   RP.cg = P.cg;
   RP.rowB = P.head_dim * E;
-  RP.nv = RP.rowB / 16; RP.log_nv = ilog2(RP.nv);
-  RP.sp = RP.nv / 2; RP.log_sp = ilog2(RP.sp); RP.rpi = 32 / RP.sp;
   RP.nr = P.rotary_dim * E / 16;
+  RP.win = ring_window_mode(P) ? 1 : 0;
+  RP.ro_v = P.rotary_offset * E / 16;
+  RP.nv = RP.rowB / 16; RP.log_nv = (RP.nv & (RP.nv - 1)) ? -1 : ilog2(RP.nv);
+  RP.nv_slot = RP.win ? RP.nr : RP.nv;
+  RP.sp = RP.nv_slot / 2; RP.log_sp = ilog2(RP.sp); RP.rpi = 32 / RP.sp;
   RP.half_R = P.rotary_dim / 2;
   const int ppv = (P.pairing == 0) ? 16 / E : 8 / E;
   RP.NV = RP.half_R / ppv;
-  RP.no_v = P.inplace ? 1 : 0;
+  RP.no_v = (P.inplace || P.no_v) ? 1 : 0;
   RP.ip_mode = 0;
   if (P.inplace) {
     if (P.d_st == P.head_dim) RP.ip_mode = 0;                                             // head-major pool

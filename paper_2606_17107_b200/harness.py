@@ -14,7 +14,7 @@ _DTYPE = {"bf16": kvr.KVR_BF16, "fp8": kvr.KVR_FP8_E4M3}
 
 def model_of(w):
     return kvr.model_desc(w.layers, w.kv_heads, w.head_dim, w.rotary_dim, _PAIRING[w.pairing],
-                          _DTYPE[w.dtype], w.inv_freq)
+                          _DTYPE[w.dtype], w.inv_freq, rotary_offset=getattr(w, "rotary_offset", 0))
 
 
 class DeviceWorkload:
@@ -28,7 +28,8 @@ class DeviceWorkload:
         self.model, self._inv_keep = model_of(w)
         if sources is None:
             sources = make_sources(w, self.device)
-        self.sources = [(k.to(self.device).contiguous(), v.to(self.device).contiguous()) for k, v in sources]
+        self.sources = [(k.to(self.device).contiguous(), None if v is None else v.to(self.device).contiguous())
+                        for k, v in sources]      # v is None for a K-only [latent | k_pe] cache (kvr.h, NEXT-3)
         self.block_table = torch.from_numpy(np.ascontiguousarray(w.block_table)).to(self.device)
         self.k_scale = self.k_scale_src = None
         if w.k_scale is not None:
@@ -87,7 +88,8 @@ class DeviceWorkload:
         points at them.  Dense [layers][heads][len][dim] only (the host entry point requires it)."""
         w = self.w
         assert all(s.src_row_pad == 0 for s in w.segments)
-        self.host_sources = [(k.cpu().pin_memory(), v.cpu().pin_memory()) for k, v in self.sources]
+        self.host_sources = [(k.cpu().pin_memory(), None if v is None else v.cpu().pin_memory())
+                             for k, v in self.sources]
         self.host_pos_maps = [None if pm is None else pm.cpu().pin_memory() for pm in self.pos_maps]
         self.host_k_scale_src = None if self.k_scale_src is None else self.k_scale_src.cpu().pin_memory()
         self.host_segs = kvr.segment_array([

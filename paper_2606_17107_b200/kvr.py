@@ -21,7 +21,8 @@ PATH_AUTO, PATH_GENERIC, PATH_RING = 0, 1, 2
 class kvr_model_desc(C.Structure):
     _fields_ = [("layers", C.c_int32), ("kv_heads", C.c_int32), ("head_dim", C.c_int32),
                 ("rotary_dim", C.c_int32), ("pairing", C.c_int32), ("dtype", C.c_int32),
-                ("inv_freq", C.POINTER(C.c_double))]
+                ("inv_freq", C.POINTER(C.c_double)),
+                ("rotary_offset", C.c_int32), ("reserved_", C.c_int32)]
 
 
 class kvr_paged_dst(C.Structure):
@@ -133,10 +134,10 @@ def _ptr(x):
     raise TypeError(type(x))
 
 
-def model_desc(layers, kv_heads, head_dim, rotary_dim, pairing, dtype, inv_freq):
+def model_desc(layers, kv_heads, head_dim, rotary_dim, pairing, dtype, inv_freq, rotary_offset=0):
     """inv_freq: sequence / numpy array of rotary_dim/2 doubles (HOST).  Returns (desc, keepalive)."""
     arr = (C.c_double * len(inv_freq))(*[float(f) for f in inv_freq])
-    return kvr_model_desc(layers, kv_heads, head_dim, rotary_dim, pairing, dtype, arr), arr
+    return kvr_model_desc(layers, kv_heads, head_dim, rotary_dim, pairing, dtype, arr, rotary_offset, 0), arr
 
 
 def paged_dst(k_cache, v_cache, strides, num_blocks, block_size, block_table, num_seqs, max_blocks_per_seq,

@@ -85,7 +85,7 @@ def materialize_cpu(w):
     """(sources, k_cache, v_cache) as numpy bit arrays.  Config 0's keys are RoPE'd at
     old_start + t by the harness (BASELINE.json configs[0]) via the ORACLE's fp64 rotation."""
     from workloads import make_pool, make_sources
-    srcs = [(np_bits(k), np_bits(v)) for k, v in make_sources(w, "cpu")]
+    srcs = [(np_bits(k), None if v is None else np_bits(v)) for k, v in make_sources(w, "cpu")]
     if w.pre_rope_theta is not None:
         assert w.dtype == "bf16"
         out = []
@@ -100,7 +100,7 @@ def materialize_cpu(w):
             out.append((k, v))
         srcs = out
     kc, vc = make_pool(w, "cpu")
-    return srcs, np_bits(kc).copy(), np_bits(vc).copy()
+    return srcs, np_bits(kc).copy(), None if vc is None else np_bits(vc).copy()
 
 
 def run_oracle(w, srcs, k_cache, v_cache, n_threads=1, layer_begin=0, layer_end=None, segments=None):

@@ -29,7 +29,7 @@ def test_exports_match_header(kvr):
 
 def test_struct_layouts_match_header(kvr):
     # sizes implied by the field lists in include/kvr.h on LP64
-    assert C.sizeof(kvr.kvr_model_desc) == 32
+    assert C.sizeof(kvr.kvr_model_desc) == 32 + 8      # + rotary_offset, reserved_ (NEXT-3 adapters)
     assert C.sizeof(kvr.kvr_paged_dst) == 16 + 32 + 8 + 8 + 8 + 8
     assert C.sizeof(kvr.kvr_segment) == 16 + 24 + 20 + 4 + 16
     assert C.sizeof(kvr.kvr_tuning) == 64
@@ -39,11 +39,12 @@ def test_struct_layouts_match_header(kvr):
 
 def _call(kvr, **over):
     m, keep = kvr.model_desc(over.get("layers", 2), 2, over.get("head_dim", 64), over.get("rotary_dim", 64),
-                             over.get("pairing", 0), over.get("dtype", 0), [1.0] * (over.get("rotary_dim", 64) // 2))
+                             over.get("pairing", 0), over.get("dtype", 0), [1.0] * (over.get("rotary_dim", 64) // 2),
+                             rotary_offset=over.get("rotary_offset", 0))
     base = 1 << 20
-    d = kvr.paged_dst(base, base * 2, over.get("strides", (16 * 4 * 2 * 64, 4 * 2 * 64, 2 * 64, 64)), 16, 4, base * 3, 1,
+    d = kvr.paged_dst(base, over.get("v_cache", base * 2), over.get("strides", (16 * 4 * 2 * 64, 4 * 2 * 64, 2 * 64, 64)), 16, 4, base * 3, 1,
                       over.get("max_blocks", 8), k_scale=over.get("k_scale"))
-    s = kvr.segment(over.get("k_src", base * 4), base * 5, over.get("src_strides", (2 * 10 * 64, 10 * 64, 64)),
+    s = kvr.segment(over.get("k_src", base * 4), over.get("v_src", base * 5), over.get("src_strides", (2 * 10 * 64, 10 * 64, 64)),
                     over.get("len", 10), 0, over.get("new_start", 7), over.get("dst_seq", 0),
                     over.get("dst_token_start", 3))
     return kvr.kvr_validate(m, d, [s]), keep
@@ -66,6 +67,14 @@ def test_validation(kvr):
     assert _call(kvr, src_strides=(2 * 10 * 64, 10 * 64, 32))[0] == kvr.KVR_ERR_INVALID_ARG
     assert _call(kvr, strides=(16 * 4 * 2 * 64, 4 * 2 * 64, 2 * 64, 68))[0] == kvr.KVR_ERR_ALIGNMENT
     assert _call(kvr, new_start=-1)[0] == kvr.KVR_ERR_INVALID_ARG
+    # NEXT-3 adapters (kvr.h): rotary window inside the row; K-only calls are all-or-none
+    assert _call(kvr, rotary_dim=32, rotary_offset=32)[0] == kvr.KVR_OK
+    assert _call(kvr, rotary_dim=32, rotary_offset=40)[0] == kvr.KVR_ERR_INVALID_ARG   # window past the row
+    assert _call(kvr, rotary_dim=32, rotary_offset=-8)[0] == kvr.KVR_ERR_INVALID_ARG
+    assert _call(kvr, rotary_dim=32, rotary_offset=4)[0] == kvr.KVR_ERR_ALIGNMENT      # 8 bytes
+    assert _call(kvr, v_cache=None, v_src=None)[0] == kvr.KVR_OK
+    assert _call(kvr, v_cache=None)[0] == kvr.KVR_ERR_INVALID_ARG
+    assert _call(kvr, v_src=None)[0] == kvr.KVR_ERR_INVALID_ARG
 
 
 def test_bytes_moved_is_linear(kvr):

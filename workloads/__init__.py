@@ -7,6 +7,6 @@ position maps, frequency tables -- all of which are *inputs* of the kvr_* calls)
 and draws K/V values from seeded generators.  See DESIGN.md "Input recipe".
 """
 from .configs import (  # noqa: F401
-    S0, SegmentSpec, Workload, config, config_small, inv_freq_llama3, inv_freq_mrope_temporal, inv_freq_standard,
+    ADAPTERS, S0, SegmentSpec, Workload, adapter_config, adapter_small, config, config_small, inv_freq_llama3, inv_freq_mrope_temporal, inv_freq_standard,
     make_pool, make_sources, make_workload, pos_map_with_gaps, SENTINEL_BF16, SENTINEL_FP8,
 )

@@ -111,6 +111,8 @@ class Workload:
     k_scale_src: Optional[np.ndarray] = None   # None = same as k_scale
     dst_head_pad: int = 0        # extra elements after each (token, head) row in the pool (stride tests)
     pre_rope_theta: Optional[float] = None     # config 0: K is RoPE'd at old_start + t by the harness
+    rotary_offset: int = 0       # first rotary dim of a row ([latent | k_pe] caches: the latent width)
+    has_v: bool = True           # False: a single cached tensor per token (MLA latent cache), no V pool
     notes: dict = field(default_factory=dict)
 
     @property
@@ -174,7 +176,8 @@ def _draw(w: Workload, seg: SegmentSpec, seg_idx: int, which: str, device) -> to
 
 def make_sources(w: Workload, device="cpu"):
     """[(k_src, v_src)] per segment, each [layers, heads, len, dim(+pad)] of bit patterns."""
-    return [(_draw(w, s, i, "k", device), _draw(w, s, i, "v", device)) for i, s in enumerate(w.segments)]
+    return [(_draw(w, s, i, "k", device), _draw(w, s, i, "v", device) if w.has_v else None)
+            for i, s in enumerate(w.segments)]
 
 
 def make_pool(w: Workload, device="cpu"):
@@ -185,7 +188,7 @@ def make_pool(w: Workload, device="cpu"):
         val = SENTINEL_FP8
     n = w.pool_elems()
     return (torch.full((n,), val, dtype=_torch_bits_dtype(w), device=device),
-            torch.full((n,), val, dtype=_torch_bits_dtype(w), device=device))
+            torch.full((n,), val, dtype=_torch_bits_dtype(w), device=device) if w.has_v else None)
 
 
 # --------------------------------------------------------------------- builders
@@ -209,11 +212,11 @@ def _table_rows(num_blocks: int, rows: List[int], seed: int, unallocated_prefix:
 def make_workload(*, name, layers, kv_heads, head_dim, rotary_dim=None, pairing="neox", dtype="bf16",
                   theta=1e4, inv_freq=None, block_size=16, layout="NHD", seed=S0,
                   seq_segments, num_blocks=None, slack=1.25, scales_differ=False,
-                  dst_head_pad=0, pre_rope_theta=None) -> Workload:
+                  dst_head_pad=0, pre_rope_theta=None, rotary_offset=0, has_v=True) -> Workload:
     """seq_segments: list (one per destination sequence) of lists of dicts with keys
     len, dst_token_start and optionally old_start, new_start, pos_map, src_row_pad.
     new_start defaults to dst_token_start, old_start to 0."""
-    rotary_dim = rotary_dim or head_dim
+    rotary_dim = rotary_dim or (head_dim - rotary_offset)
     if inv_freq is None:
         inv_freq = inv_freq_standard(theta, rotary_dim)
     segs, rows, prefix = [], [], []
@@ -241,7 +244,8 @@ def make_workload(*, name, layers, kv_heads, head_dim, rotary_dim=None, pairing=
                     pairing=pairing, dtype=dtype, inv_freq=np.asarray(inv_freq, dtype=np.float64),
                     block_size=block_size, num_blocks=num_blocks, layout=layout, block_table=table,
                     segments=segs, seed=seed, k_scale=k_scale, k_scale_src=k_scale_src,
-                    dst_head_pad=dst_head_pad, pre_rope_theta=pre_rope_theta)
+                    dst_head_pad=dst_head_pad, pre_rope_theta=pre_rope_theta, rotary_offset=rotary_offset,
+                    has_v=has_v)
 
 
 def _compose_offsets(lengths, total, seed):
@@ -318,3 +322,48 @@ def config_small(c: int, layout: str = "NHD") -> Workload:
     if c == 0:
         return config(0, layout)
     return config(c, layout, layers={1: 3, 2: 2, 3: 2, 4: 3}[c], shrink={1: 8, 2: 16, 3: 16, 4: 32}[c])
+
+
+# ------------------------------------------------------------- NEXT-3 / NEXT-4 adapter workloads
+
+ADAPTERS = ("mla-dsv2-lite", "image-kv-qwen25vl-7b", "image-kv-qwen3vl-8b")
+
+
+def adapter_config(name: str, layout: str = "NHD", layers: Optional[int] = None, shrink: int = 1) -> Workload:
+    """Shapes of the paper's attention-variant adapters (PAPER.md:205, :215, :514 Fig. 22; Table 2 :306, :308).
+    Synthetic, seeded; only shapes are taken from the models the paper names.
+
+    mla-dsv2-lite         DeepSeek-V2-Lite-shaped latent cache: 27 layers, one cached row per token =
+                          [latent c_t (512) | k_pe (64)], no V tensor; only k_pe rotates (interleaved pairs,
+                          theta 1e4); one 8192-token skill precompiled at 0 and spliced at 2000; block_size 64.
+    image-kv-qwen25vl-7b  Qwen2.5-VL-7B-shaped image KV: 28 layers, 4 kv heads, D 128, SECTIONED M-RoPE (16, 24, 24),
+                          theta 1e6; 32 cached images of 1296 soft tokens each moved by Delta = 161 temporal positions
+                           into 32 sequences; only the 16 temporal pairs rotate.
+    image-kv-qwen3vl-8b   Qwen3-VL-8B-shaped: 36 layers, 8 kv heads, D 128, INTERLEAVED M-RoPE (24, 20, 20), theta 5e6;
+                          same 32 images.
+    """
+    seed = S0 + 100 + ADAPTERS.index(name)
+    if name == "mla-dsv2-lite":
+        n = 8192 // shrink
+        return make_workload(name=name, layers=layers or 27, kv_heads=1, head_dim=576, rotary_dim=64, rotary_offset=512,
+                             pairing="gptj", theta=1e4, block_size=64, layout=layout, seed=seed, has_v=False,
+                             num_blocks=2 * ((2000 + n + 63) // 64),
+                             seq_segments=[[dict(len=n, dst_token_start=2000, new_start=2000)]])
+    if name in ("image-kv-qwen25vl-7b", "image-kv-qwen3vl-8b"):
+        q3 = name.endswith("qwen3vl-8b")
+        sections, theta = ((24, 20, 20), 5e6) if q3 else ((16, 24, 24), 1e6)
+        inv = inv_freq_mrope_temporal(theta, 128, sections, interleaved=q3)
+        n_img = 32 if shrink == 1 else max(2, 32 // shrink)
+        n_tok = 1296 // shrink
+        rng = np.random.default_rng(seed + 4000)
+        seqs = []
+        for _ in range(n_img):
+            at = int(rng.integers(0, 2048 // shrink + 1))          # text before the image in its new trajectory
+            seqs.append([dict(len=n_tok, dst_token_start=at, old_start=at, new_start=at + 161)])
+        return make_workload(name=name, layers=layers or (36 if q3 else 28), kv_heads=8 if q3 else 4, head_dim=128,
+                             inv_freq=inv, block_size=16, layout=layout, seed=seed, seq_segments=seqs)
+    raise ValueError(name)
+
+
+def adapter_small(name: str, layout: str = "NHD") -> Workload:
+    return adapter_config(name, layout, layers=2, shrink=8)
