@@ -286,7 +286,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   P.any_pos_map = any_map; P.scales_differ = scales_differ;
 
   // ---- work decomposition: (segment, chunk of <= cg destination tokens, group of lpu layers) ----
-  auto decompose = [&](int cg, int lpu_request, int hsplit_request) {
+  auto decompose = [&](int cg, int lpu_request, int hsplit_request, bool ring) {
     P.cg = cg;
     // head split (ring kernel only): must divide the number of head groups of a unit
     int hsplit = 1;
@@ -315,7 +315,19 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       chunks_total += o.n_chunks;
     }
     int lpu = lpu_request;
-    if (lpu <= 0) {
+    if (lpu <= 0 && ring) {
+      // Ring kernel: a unit should hold enough tiles to amortise its decode in the producer warp (~8 tiles = 64 KB)
+      // and no more -- units are handed out in (layer, chunk) order, so with few layers per unit the CTAs that run
+      // concurrently read neighbouring source rows of one layer (DRAM page locality: +3 % on configs[2] against
+      // 11 layers per unit) and the tail is short.  With a position map the per-chunk angle table is rebuilt per
+      // unit, so a unit holds ~24 tiles there.
+      const int tiles_per_layer = (m.kv_heads / ring_heads_per_tile(P)) / hsplit;
+      const int want = any_map ? 24 : 8;
+      lpu = (want + tiles_per_layer - 1) / tiles_per_layer;
+      if (lpu > m.layers) lpu = m.layers;
+      // small calls: prefer more, smaller units so that every SM gets one (latency, not bandwidth, is the bound)
+      while (lpu > 1 && chunks_total * ((m.layers + lpu - 1) / lpu) * hsplit < (int64_t)4 * c->sm_count) lpu = (lpu + 1) / 2;
+    } else if (lpu <= 0) {
       if (any_map) lpu = m.layers;   // the per-token angle table is built once per chunk and reused by all layers
       else {
         int64_t target = (int64_t)c->sm_count * 32;
@@ -348,7 +360,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       cg_limit = (int)(16384 / ((int64_t)m.head_dim * E));
       cg_limit = cg_limit < 1 ? 1 : (cg_limit > 16 ? 16 : cg_limit);
     }
-    decompose(chunk_granularity(d->block_size, cg_limit), tu.layers_per_unit, tu.hsplit);
+    decompose(chunk_granularity(d->block_size, cg_limit), tu.layers_per_unit, tu.hsplit, true);
     bool ok = ring_supported(P, slot.host, &why);
     if (!ok && path == 2) { c->last_err = std::string("ring kernel unsupported: ") + (why ? why : ""); return KVR_ERR_UNSUPPORTED; }
     path = ok ? 2 : 1;
@@ -357,7 +369,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     // generic kernel: chunk table [cg][R/2] float4 must fit 48 KB of static-limit shared memory
     int limit = (int)(47 * 1024 / ((m.rotary_dim / 2) * 16 + 4));
     if (limit < 1) return KVR_ERR_UNSUPPORTED;
-    decompose(chunk_granularity(d->block_size, limit < 16 ? limit : 16), tu.layers_per_unit, 1);
+    decompose(chunk_granularity(d->block_size, limit < 16 ? limit : 16), tu.layers_per_unit, 1, false);
   }
 
   if (n <= kInlineSegs) {

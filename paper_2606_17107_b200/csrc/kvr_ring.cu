@@ -225,8 +225,10 @@ __device__ __forceinline__ void requant_fp8(uint4& A, float s_src, float inv_dst
 }
 
 // ------------------------------------------------------------------------------- the kernel
-template <int DTYPE, int PAIRING, bool MAP>
-__global__ void __launch_bounds__(kMaxThreads, 1)
+// MAXT = 256: the default launch shape (<= 8 warps, 2 CTAs per SM) gets 128 registers per thread and no spills;
+// MAXT = kMaxThreads: the wide shapes the tuning knobs allow (up to 16 consumer warps, or 3+ CTAs per SM).
+template <int DTYPE, int PAIRING, bool MAP, int MAXT>
+__global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1))
 kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ RingParams RP) {
   using G = Geo<DTYPE, PAIRING>;
   constexpr int E = (DTYPE == 0) ? 2 : 1;
@@ -246,6 +248,17 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
   // memory as soon as a CTA of this grid exits) and run this prologue while our tail drains; it touches no global
   // memory until griddepcontrol.wait has seen the previous grid complete and flush.
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  // Before the dependency wait the producer may only touch kernel parameters and the context's own immutable
+  // inv_freq copy: with the descriptors inline it already knows the segment of its first (statically assigned)
+  // unit and builds that segment's angle table (fp64 sincos), taking it off the critical path of the launch.
+  int pre_si = -1;
+  if (!MAP && warp == NW && P.n_segs <= kInlineSegs && (int64_t)blockIdx.x * P.grab < P.total_units) {
+    pre_si = find_segment(P.inline_segs, P.n_segs, (int64_t)blockIdx.x * P.grab);
+    float4* tab = reinterpret_cast<float4*>(smem + RP.off_tab + RP.tab_stride);       // table buffer 1
+    const int64_t delta = P.inline_segs[pre_si].delta;
+    for (int p = lane; p < RP.half_R; p += 32) tab[tab_pos<G::PPV>(p, RP.NV)] = angle_entry(delta, P.inv_freq[p]);
+    __syncwarp();
+  }
   asm volatile("griddepcontrol.wait;" ::: "memory");
   if (DTYPE == 1)
     for (int i = threadIdx.x; i < RP.n_scales; i += blockDim.x) s_scales[i] = P.k_scale_dst[i];
@@ -261,6 +274,7 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     uint32_t phase = 0;
     int tb = 0, gen = 0;           // current table buffer / generation
     int64_t cur_key = -1;          // segment (segment mode) or unit (map mode) the current table belongs to
+    if (pre_si >= 0) { tb = 1; gen = 1; cur_key = pre_si; }   // built before the dependency wait
     uint32_t lu_i[2] = {0, 0}, lu_phase[2] = {0, 0};   // last tile that used each table buffer
     int lu_stage[2] = {0, 0};
     bool lu_valid[2] = {false, false};
@@ -299,15 +313,17 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         d_blk = P.block_table[(int64_t)s->dst_seq * P.max_blocks + ch.blk_index];
       }
     };
+    // The first grab is static (CTA b takes units [b G, (b+1) G)): no round trip to the counter before the first
+    // load is in flight.  The counter hands out the units from gridDim.x * G on.
     unsigned long long nxt = 0;
-    if (lane == 0) nxt = atomicAdd(P.sched, (unsigned long long)G);
-    int64_t base = (int64_t)__shfl_sync(FULL, nxt, 0);
+    const int64_t dyn0 = (int64_t)gridDim.x * G;
+    int64_t base = (int64_t)blockIdx.x * G;
     if (lane == 0) nxt = atomicAdd(P.sched, (unsigned long long)G);
     int d_si, d_t0, d_ntok, d_off, d_lg, d_blk;
     decode(base, d_si, d_t0, d_ntok, d_off, d_lg, d_blk);
     for (;;) {
       if (base >= P.total_units) break;
-      const int64_t base_n = (int64_t)__shfl_sync(FULL, nxt, 0);
+      const int64_t base_n = dyn0 + (int64_t)__shfl_sync(FULL, nxt, 0);
       if (lane == 0 && base_n < P.total_units) nxt = atomicAdd(P.sched, (unsigned long long)G);
       int n_si, n_t0, n_ntok, n_off, n_lg, n_blk;
       decode(base_n, n_si, n_t0, n_ntok, n_off, n_lg, n_blk);
@@ -330,14 +346,30 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
             mbar_wait(s_empty + 8u * (nb ? lu_stage[1] : lu_stage[0]), nb ? lu_phase[1] : lu_phase[0], 1);   // its last reader may still be in flight
           __syncwarp();
           float4* tab = reinterpret_cast<float4*>(smem + RP.off_tab + nb * RP.tab_stride);
-          const int rows = MAP ? n_tok : 1;
-          for (int idx = lane; idx < rows * RP.half_R; idx += 32) {
-            const int t = idx / RP.half_R, p = idx - t * RP.half_R;
-            const int64_t delta = (MAP && sg.pos_map)
-                                      ? (int64_t)sg.pos_map[t0 + t] - ((int64_t)sg.old_start + t0 + t)
-                                      : (int64_t)sg.delta;
-            tab[t * RP.half_R + tab_pos<G::PPV>(p, RP.NV)] = angle_entry(delta, P.inv_freq[p]);
-            if (MAP && p == 0) reinterpret_cast<int32_t*>(tab + RP.cg * RP.half_R)[t] = (delta == 0);
+          if (MAP) {
+            // Per-token shifts, deduplicated into RUNS of equal Delta (a position map is contiguous except at its
+            // gaps, so a chunk of <= 32 tokens holds a handful of distinct shifts): one table row per run, and a
+            // per-token word that names the token's row (-1: Delta_t == 0, the row is a byte copy).
+            long long d = 0;
+            if (lane < n_tok)
+              d = sg.pos_map ? (long long)sg.pos_map[t0 + lane] - ((long long)sg.old_start + t0 + lane) : (long long)sg.delta;
+            const long long dprev = __shfl_up_sync(FULL, d, 1);
+            const unsigned heads_mask = __ballot_sync(FULL, lane < n_tok && (lane == 0 || d != dprev));
+            const int n_runs = __popc(heads_mask);
+            if (lane < n_tok)
+              reinterpret_cast<int32_t*>(tab + RP.cg * RP.half_R)[lane] =
+                  (d == 0) ? -1 : (__popc(heads_mask & (0xFFFFFFFFu >> (31 - lane))) - 1);
+            const int total = n_runs * RP.half_R;
+            for (int base_idx = 0; base_idx < total; base_idx += 32) {
+              const int idx = base_idx + lane;
+              const int r = idx < total ? idx / RP.half_R : 0, p = idx - r * RP.half_R;
+              const int src_lane = (int)__fns(heads_mask, 0, r + 1);            // first token of run r
+              const long long delta = __shfl_sync(FULL, d, src_lane);
+              if (idx < total) tab[r * RP.half_R + tab_pos<G::PPV>(p, RP.NV)] = angle_entry((int64_t)delta, P.inv_freq[p]);
+            }
+          } else {
+            for (int p = lane; p < RP.half_R; p += 32)
+              tab[tab_pos<G::PPV>(p, RP.NV)] = angle_entry((int64_t)sg.delta, P.inv_freq[p]);
           }
           __syncwarp();
           tb = nb; gen += 1; cur_key = key;
@@ -468,7 +500,7 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
   va += RP.ro_v; vb += RP.ro_v;       // table positions above are relative to the window; addresses are not
   float4 T4[DTYPE == 0 ? G::NT : 1];
   float2 T2[DTYPE == 1 ? G::NT : 1];
-  int my_gen = -1;
+  int my_gen = -1, my_run = -1;
   const bool dst_rows_packed = (P.d_st == P.head_dim);
 
   int stage = warp % S;
@@ -542,9 +574,11 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         uint4 B = lds128(ks + t * sm_st + vb * 16);
         bool rot_row = rotate;
         if (MAP) {
-          rot_row = reinterpret_cast<const int32_t*>(smem + RP.off_tab + m.tab * RP.tab_stride + RP.cg * RP.half_R * 16)[t] == 0;
-          if (rot_row && (rot_a || rot_b)) {
-            const uint32_t trow = tab + t * RP.half_R * 16;
+          const int run = reinterpret_cast<const int32_t*>(smem + RP.off_tab + m.tab * RP.tab_stride + RP.cg * RP.half_R * 16)[t];
+          rot_row = run >= 0;
+          if (rot_row && (rot_a || rot_b) && (run != my_run || m.gen != my_gen)) {   // cos/sin registers follow the run
+            my_run = run; my_gen = m.gen;
+            const uint32_t trow = tab + run * RP.half_R * 16;
 #pragma unroll
             for (int k = 0; k < G::NT; ++k) {
               float4 e = lds128f(trow + tpos[k] * 16);
@@ -641,11 +675,11 @@ bool ring_supported(const CallParams& P, const SegDev* segs, const char** why) {
   return w == nullptr;
 }
 
-template <int DTYPE, int PAIRING, bool MAP>
+template <int DTYPE, int PAIRING, bool MAP, int MAXT>
 static cudaError_t launch_inst(const CallParams& P, const RingParams& RP, int grid, int block, int smem, cudaStream_t st, bool pdl) {
   static int configured = 0;   // per instantiation
   if (configured < smem) {
-    cudaError_t e = cudaFuncSetAttribute(kvr_ring_kernel<DTYPE, PAIRING, MAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaError_t e = cudaFuncSetAttribute(kvr_ring_kernel<DTYPE, PAIRING, MAP, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     configured = smem;
   }
@@ -655,7 +689,7 @@ static cudaError_t launch_inst(const CallParams& P, const RingParams& RP, int gr
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = at; lc.numAttrs = pdl ? 1 : 0;
-  return cudaLaunchKernelEx(&lc, kvr_ring_kernel<DTYPE, PAIRING, MAP>, P, RP);
+  return cudaLaunchKernelEx(&lc, kvr_ring_kernel<DTYPE, PAIRING, MAP, MAXT>, P, RP);
 }
 
 cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_count, cudaStream_t stream,
@@ -727,7 +761,10 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   const int block = (RP.NW + 1) * 32;
   *grid_out = (int)g; *block_out = block; *smem_out = smem;
   const bool map = P.any_pos_map != 0;
-#define KVR_LAUNCH(D, PR, M) return launch_inst<D, PR, M>(P, RP, (int)g, block, smem, stream, cfg.pdl != 2)
+  const bool small = block <= 256 && ctas <= 2;
+#define KVR_LAUNCH(D, PR, M)                                                                             \
+  return small ? launch_inst<D, PR, M, 256>(P, RP, (int)g, block, smem, stream, cfg.pdl != 2)            \
+               : launch_inst<D, PR, M, kMaxThreads>(P, RP, (int)g, block, smem, stream, cfg.pdl != 2)
   if (P.dtype == 0) {
     if (P.pairing == 0) { if (map) KVR_LAUNCH(0, 0, true); else KVR_LAUNCH(0, 0, false); }
     else { if (map) KVR_LAUNCH(0, 1, true); else KVR_LAUNCH(0, 1, false); }
