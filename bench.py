@@ -54,9 +54,14 @@ def parse_args():
                     "mla-dsv2-lite | image-kv-qwen25vl-7b | image-kv-qwen3vl-8b; device-timed and e2e only")
     ap.add_argument("--layout", default="NHD", choices=["NHD", "HND"])
     ap.add_argument("--impl", default="kvr", choices=["kvr", "reference"])
-    ap.add_argument("--op", default="splice", choices=["splice", "inplace"],
+    ap.add_argument("--latency", action="store_true",
+                    help="also report launch-to-launch latency and CUDA-graph replay time per call, rotating over 8 "
+                         "buffer sets (SURVEY.md 8(d); always on for --config 0)")
+    ap.add_argument("--op", default="splice", choices=["splice", "inplace", "span"],
                     help="splice = kvr_reposition_splice (the BASELINE.json metric); inplace = kvr_reposition_inplace "
-                         "(SURVEY.md 8(f) NEXT-1: re-float resident chunks, 2*B1 bytes per token; device-timed only)")
+                         "(SURVEY.md 8(f) NEXT-1: re-float resident chunks, 2*B1 bytes per token; device-timed only); "
+                         "span = kvr_write_span over the same rows (Delta = 0: byte copies with the same access pattern "
+                         "= this library's own copy ceiling, SURVEY.md H1)")
     ap.add_argument("--e2e-steps", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -213,6 +218,44 @@ def run_reference(args):
     return 0
 
 
+def latency_probe(w, device, ctx, stream, sets=8, reps=64):
+    """Per-call latency of kvr_reposition_splice on `w` (meant for configs[0], 262 KB: launch-bound), rotating over
+    `sets` independent source/pool sets so no call finds its lines in L2 from the call before:
+    launch_to_launch_us = stream of back-to-back calls (CUDA events); graph_replay_us = the same calls captured once
+    in a CUDA graph and replayed."""
+    import torch
+    from paper_2606_17107_b200.harness import DeviceWorkload
+    dws = [DeviceWorkload(w, device) for _ in range(sets)]
+    for d in dws:
+        d.run(ctx, stream=stream)
+    torch.cuda.synchronize(device)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def burst():
+        for i in range(sets * reps):
+            dws[i % sets].run(ctx, stream=stream)
+    burst()
+    torch.cuda.synchronize(device)
+    ev0.record(stream); burst(); ev1.record(stream)
+    torch.cuda.synchronize(device)
+    l2l = ev0.elapsed_time(ev1) * 1e3 / (sets * reps)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(stream):
+        with torch.cuda.graph(graph, stream=stream):
+            burst()
+        graph.replay()
+        torch.cuda.synchronize(device)
+        ev0.record(stream)
+        for _ in range(5):
+            graph.replay()
+        ev1.record(stream)
+    torch.cuda.synchronize(device)
+    rep_us = ev0.elapsed_time(ev1) * 1e3 / (5 * sets * reps)
+    assert ctx.last_device_status()[0] == 0
+    return {"launch_to_launch_us": l2l, "graph_replay_us": rep_us, "buffer_sets": sets, "calls_per_graph": sets * reps,
+            "bytes_per_call": int(dws[0].bytes_moved())}
+
+
 # --------------------------------------------------------------------------------------- the kvr arm
 def run_kvr(args):
     import torch
@@ -251,6 +294,11 @@ def run_kvr(args):
         run_step = lambda: dw.run_inplace(ctx, spans, stream=stream)
         args.no_e2e = args.no_cpu_baseline = True
 
+    if args.op == "span":
+        spans_w = dw.write_spans()
+        run_step = lambda: ctx.write_span(dw.dst, spans_w, stream=stream)
+        args.no_e2e = args.no_cpu_baseline = True
+
     # ---- device-resident timing ----
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     sampler = ClockSampler(device)             # NVML init happens here, before the warm-up, not after it
@@ -286,6 +334,10 @@ def run_kvr(args):
     peak, peak_src = measured_peak()
     achieved = bytes_per_step / (seconds / steps) / 1e9      # this rank's kernel: one launch per step
 
+    latency = None
+    if (args.latency or (not args.workload and args.config == 0)) and args.op == "splice" and rep.world == 1:
+        latency = latency_probe(w, device, ctx, stream)
+
     # ---- end to end: sources in pinned host memory, through kvr_reposition_splice_host ----
     e2e = None
     if not args.no_e2e:
@@ -320,7 +372,8 @@ def run_kvr(args):
     ctx.close()
     if rep.rank == 0:
         line = {
-            "metric": METRIC if args.op == "splice" else "KV tokens repositioned in place/sec",
+            "metric": {"splice": METRIC, "inplace": "KV tokens repositioned in place/sec",
+                       "span": "KV tokens overwritten (Delta = 0 copy)/sec"}[args.op],
             "value": agg["per_second"], "unit": UNIT, "n_gpus": rep.world, "steps": steps,
             "warmup": warmup, "ms_per_step": agg["seconds"] / steps * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -340,6 +393,8 @@ def run_kvr(args):
             "e2e": e2e,
             "cpu_baseline": cpu,
         }
+        if latency is not None:
+            line["latency"] = latency
         print(json.dumps(line), flush=True)
     rep.close()
     return 0

@@ -131,7 +131,10 @@ typedef struct {
   int32_t grab;            /* units a CTA draws from the dynamic scheduler per atomic (1..32)               */
   int32_t pdl;             /* programmatic dependent launch of the ring kernel: 0 auto (on), 1 on, 2 off            */
   int32_t hsplit;          /* split a unit's heads into this many units (finer tail); 0 auto                        */
-  int32_t reserved[6];
+  int32_t chunk_tokens;    /* ring kernel: upper bound on the tokens of a chunk (default 16); the chunk is the largest
+                              divisor of block_size below it                                                          */
+  int32_t tile_bytes;      /* ring kernel: a tile takes the fewest heads whose K run reaches this size (default 4096) */
+  int32_t reserved[4];
 } kvr_tuning;
 
 /* Creates a context on CUDA device `cuda_device` (must be compute capability 10.x).  Allocates a few

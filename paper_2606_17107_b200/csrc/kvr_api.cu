@@ -176,6 +176,9 @@ kvr_status kvr_create(kvr_ctx** out, const kvr_model_desc* model, int cuda_devic
   if (e == cudaSuccess) e = cudaMemset(c->d_sched, 0, 2 * sizeof(unsigned long long));
   for (int i = 0; i < kSlots && e == cudaSuccess; ++i)
     e = cudaEventCreateWithFlags(&c->slots[i].ev, cudaEventDisableTiming);
+  // every staging slot is usable from the first call on (a call under stream capture cannot allocate)
+  for (int i = 0; i < kSlots && e == cudaSuccess; ++i)
+    if (slot_reserve(c, c->slots[i], kInitialSegCap) != KVR_OK) e = cudaErrorMemoryAllocation;
   cudaSetDevice(prev);
   if (e != cudaSuccess) {
     kvr_destroy(c);
@@ -349,7 +352,8 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   int path = tu.path;
   const char* why = nullptr;
   if (path == 0 || path == 2) {
-    int cg_limit = 16;
+    int cg_limit = (tu.chunk_tokens > 0 && tu.chunk_tokens < 16) ? tu.chunk_tokens : 16;
+    P.tile_min_bytes = tu.tile_bytes;
     if (inplace && d->stride_token != m.head_dim) {
       // token-major pool, in place: a tile is cg tokens x ALL heads (one contiguous run); keep it near 8 KB
       cg_limit = (int)(8192 / ((int64_t)m.kv_heads * m.head_dim * E));

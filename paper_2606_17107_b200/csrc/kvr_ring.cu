@@ -645,7 +645,7 @@ int ring_heads_per_tile(const CallParams& P) {
   const int rowB = P.head_dim * (P.dtype == 0 ? 2 : 1);
   if (P.inplace && P.d_st != P.head_dim && P.d_sh == P.head_dim && P.d_st == (int64_t)P.heads * P.head_dim) return P.heads;
   for (int h = 1; h <= P.heads; ++h)
-    if (P.heads % h == 0 && h * P.cg * rowB >= 4096) return h;
+    if (P.heads % h == 0 && h * P.cg * rowB >= (P.tile_min_bytes > 0 ? P.tile_min_bytes : 4096)) return h;
   return P.heads;
 }
 

@@ -261,3 +261,64 @@ def test_host_sources_entry_point(c, layout):
     run_oracle(w, srcs, kc, vc)
     assert np.array_equal(np_bits(dw.v_cache), vc)
     assert k_distance(w, np_bits(dw.k_cache), kc).max() <= K_TOL[w.dtype]
+
+
+# ------------------------------------------------------------------ CUDA graph capture; cost linear in L
+def test_cuda_graph_capture_and_replay_matches_the_oracle():
+    """include/kvr.h: a call with inline descriptors (<= 8 segments) enqueues nothing but its kernel and may be
+    captured in a CUDA graph; replaying the graph onto a re-sentinelled pool gives the oracle's bytes again."""
+    from paper_2606_17107_b200 import kvr
+    from paper_2606_17107_b200.harness import DeviceWorkload
+    from workloads import make_pool
+    w = config_small(2, "NHD")
+    srcs, kc, vc = materialize_cpu(w)
+    dw = DeviceWorkload(w, "cuda:0", sources=[(torch_bits(k), torch_bits(v)) for k, v in srcs])
+    stream = torch.cuda.Stream()
+    with kvr.Context(dw.model) as ctx:
+        dw.run(ctx, stream=stream)                         # warm: staging slots allocated outside the capture
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(stream):
+            with torch.cuda.graph(graph, stream=stream):
+                dw.run(ctx, stream=stream)
+            k0, v0 = make_pool(w, "cuda:0")
+            dw.k_cache.copy_(k0); dw.v_cache.copy_(v0)     # wipe what the warm-up call wrote
+            for _ in range(3):
+                graph.replay()
+        torch.cuda.synchronize()
+        assert ctx.last_device_status()[0] == 0
+    run_oracle(w, srcs, kc, vc)
+    assert np.array_equal(np_bits(dw.v_cache), vc)
+    assert k_distance(w, np_bits(dw.k_cache), kc).max() <= K_TOL[w.dtype]
+
+
+def test_time_is_linear_in_tokens():
+    """'transplant is O(L)'.  Device time of the configs[1] shape (8 layers) against L fits a line
+    through (almost) the origin: R^2 > 0.99 (SURVEY.md 8(c) pins, last row)."""
+    from paper_2606_17107_b200 import kvr
+    from paper_2606_17107_b200.harness import DeviceWorkload
+    Ls, ts = [2048, 4096, 8192, 16384, 32768], []
+    for L in Ls:
+        w = make_workload(name="lin", layers=8, kv_heads=8, head_dim=128, theta=1e6, block_size=16, seed=3,
+                          seq_segments=[[dict(len=L, dst_token_start=2000, new_start=2000)]])
+        dw = DeviceWorkload(w, "cuda:0")
+        assert dw.bytes_moved() == 4 * 8 * 8 * 128 * 2 * L
+        stream = torch.cuda.Stream()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with kvr.Context(dw.model) as ctx:
+            for _ in range(200):
+                dw.run(ctx, stream=stream)
+            torch.cuda.synchronize()
+            e0.record(stream)
+            for _ in range(50):
+                dw.run(ctx, stream=stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            assert ctx.last_device_status()[0] == 0
+        ts.append(e0.elapsed_time(e1) / 50)
+        del dw
+    x, y = np.array(Ls, dtype=np.float64), np.array(ts)
+    slope, icpt = np.polyfit(x, y, 1)
+    r2 = 1 - ((y - (slope * x + icpt)) ** 2).sum() / ((y - y.mean()) ** 2).sum()
+    assert r2 > 0.99, (ts, r2)
+    assert abs(icpt) < 0.015, (icpt, ts)                # ms: the line passes near the origin (a launch's fixed cost)
