@@ -134,7 +134,9 @@ typedef struct {
   int32_t chunk_tokens;    /* ring kernel: upper bound on the tokens of a chunk (default 16); the chunk is the largest
                               divisor of block_size below it                                                          */
   int32_t tile_bytes;      /* ring kernel: a tile takes the fewest heads whose K run reaches this size (default 4096) */
-  int32_t reserved[4];
+  int32_t gather;          /* ring kernel, dense token-major pools: tiles of all heads x few tokens, several consumer
+                              warps per tile (see kvr_ring.cu): 0 auto (on), 1 on, 2 off                              */
+  int32_t reserved[3];
 } kvr_tuning;
 
 /* Creates a context on CUDA device `cuda_device` (must be compute capability 10.x).  Allocates a few
@@ -178,7 +180,9 @@ KVR_API uint64_t kvr_last_h2d_bytes(const kvr_ctx* ctx);
  * delta_t = pos_map[t] - (old_start + t)) exactly as in kvr_reposition_splice and written back to the slot it was
  * read from.  V is position-free and is neither read nor written: pool->v_cache may be NULL.
  * fp8: pool->k_scale is both the source and the destination scale.  delta_t == 0 leaves the row's bytes alone.
- * Traffic is 2 * layers*kv_heads*head_dim*esz bytes per token (kvr_inplace_bytes_moved), half of a re-splice.
+ * Traffic is 2 * layers*kv_heads*head_dim*esz bytes per token (kvr_inplace_bytes_moved), half of a re-splice; with
+ * rotary_offset != 0 (a [latent | k_pe] cache) only the rotary window is read and written: 2 * layers*kv_heads*
+ * rotary_dim*esz bytes per token.
  * Spans of one call must not overlap (undefined).  Same asynchrony, validation and error rules as the splice:
  * host-detectable faults are rejected before any launch; an invalid block-table entry skips its tokens and
  * raises the sticky device status. */

@@ -325,7 +325,8 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       // 11 layers per unit) and the tail is short.  With a position map the per-chunk angle table is rebuilt per
       // unit, so a unit holds ~24 tiles there.
       const int tiles_per_layer = (m.kv_heads / ring_heads_per_tile(P)) / hsplit;
-      const int want = any_map ? 24 : 8;
+      const int want = P.gather ? (any_map ? 6 : 2)      // gather tiles are 32 KB: the same 64 KB / 192 KB per unit
+                                : (any_map ? 24 : 8);
       lpu = (want + tiles_per_layer - 1) / tiles_per_layer;
       if (lpu > m.layers) lpu = m.layers;
       // small calls: prefer more, smaller units so that every SM gets one (latency, not bandwidth, is the bound)
@@ -354,6 +355,28 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   if (path == 0 || path == 2) {
     int cg_limit = (tu.chunk_tokens > 0 && tu.chunk_tokens < 16) ? tu.chunk_tokens : 16;
     P.tile_min_bytes = tu.tile_bytes;
+    // GATHER mode (kvr_ring.cu): dense token-major (NHD) pool, several heads, power-of-two rows, not in place:
+    // a tile = all heads x cg tokens with K (and V) <= 16 KB each, so that a token's H*D destination row is written
+    // by one warp in one burst.  tuning.gather: 0 auto (on), 1 on, 2 off.
+    P.gather = 0;
+    {
+      const int64_t rowB = (int64_t)m.head_dim * E;
+      const bool pow2_row = rowB >= 32 && rowB <= 1024 && (rowB & (rowB - 1)) == 0 && m.rotary_offset == 0;
+      const bool dense_nhd = d->stride_head == m.head_dim && d->stride_token == (int64_t)m.kv_heads * m.head_dim;
+      const int64_t tile_target = tu.tile_bytes > 0 ? tu.tile_bytes : 16384;      // K bytes of a gather tile
+      int64_t lim = tile_target / (m.kv_heads * rowB);
+      const int cg_g = chunk_granularity(d->block_size, (int)(lim > 16 ? 16 : lim));
+      // auto: only where it was measured to pay (B200): bf16, and all heads of a FULL chunk fit the tile, so
+      // the source runs are not shortened (kv_heads * head_dim <= 512 elements: +4.6 % on configs[4], +2 % on the 4-head
+      // image-KV shape).  With 8 heads of 128 the chunk halves to 8 tokens (2 KB source runs): a wash (+-1 %).  fp8: -7 %.
+      const bool pays = m.dtype == KVR_BF16 && cg_g == chunk_granularity(d->block_size, 16);
+      if (tu.gather != 2 && (tu.gather == 1 || pays) && tu.chunk_tokens <= 0 && (tu.tile_bytes <= 0 || tu.gather == 1) &&
+          tu.hsplit <= 1 && !inplace && pow2_row && dense_nhd && m.kv_heads > 1 && m.kv_heads * rowB <= 8192 && cg_g >= 2) {
+        P.gather = 1;
+        cg_limit = cg_g;
+        P.tile_min_bytes = (int32_t)(m.kv_heads * cg_g * rowB);
+      }
+    }
     if (inplace && d->stride_token != m.head_dim) {
       // token-major pool, in place: a tile is cg tokens x ALL heads (one contiguous run); keep it near 8 KB
       cg_limit = (int)(8192 / ((int64_t)m.kv_heads * m.head_dim * E));
@@ -598,7 +621,9 @@ uint64_t kvr_inplace_bytes_moved(const kvr_model_desc* m, const kvr_resident_spa
   if (!m || (n > 0 && !spans)) return 0;
   uint64_t tokens = 0;
   for (int32_t i = 0; i < n; ++i) tokens += spans[i].len > 0 ? (uint64_t)spans[i].len : 0u;
-  return 2ull * (uint64_t)m->layers * (uint64_t)m->kv_heads * (uint64_t)m->head_dim * (uint64_t)elt_bytes(m->dtype) * tokens;
+  // a [latent | k_pe] row (rotary_offset != 0): only the k_pe window is read and written, the latent stays put
+  const uint64_t width = m->rotary_offset != 0 ? (uint64_t)m->rotary_dim : (uint64_t)m->head_dim;
+  return 2ull * (uint64_t)m->layers * (uint64_t)m->kv_heads * width * (uint64_t)elt_bytes(m->dtype) * tokens;
 }
 
 // ---- NEXT-2: span overwrite = the delta == 0 splice (R21) ----

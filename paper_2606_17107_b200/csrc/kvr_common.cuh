@@ -65,7 +65,7 @@ struct CallParams {
   int32_t grab;                // units handed out per atomic
   int32_t hsplit;              // ring kernel: a (chunk, layer group) is split into hsplit units over its head groups
   int32_t tile_min_bytes;      // ring kernel: a tile takes the fewest heads whose K run reaches this many bytes
-  int32_t pad1_;
+  int32_t gather;              // ring kernel: gather mode (dense token-major pool; a tile = all heads of a few tokens)
   int32_t no_v;                // V is neither read nor written (in-place calls; K-only [latent | k_pe] caches)
   int32_t inplace;             // kvr_reposition_inplace: K rows are read from the pool slot they are written back to; no V
   SegDev inline_segs[kInlineSegs];

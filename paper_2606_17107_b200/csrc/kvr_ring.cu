@@ -42,6 +42,11 @@ struct RingParams {
                                           // rest of the row is moved by a plain 16-byte copy loop
   int nv_slot;                            // vectors the lane slots are laid over: nv, or nr in window mode
   int ro_v;                               // rotary_offset in 16-byte vectors
+  int gather;                             // GATHER mode (see wpg)
+  int wpg;                                // GATHER mode (dense token-major pools): a tile holds ALL heads of a few tokens and
+                                          // wpg consumer warps share it, each taking whole token rows, tokens outer / heads
+                                          // inner, so that a token's H*D row reaches L2 (and DRAM) as one contiguous burst
+                                          // instead of H pieces written by H different warps at different times; 1 otherwise
   int ip_mode;                            // in-place source runs: 0 one run per head (d_st == head_dim), 1 one run for the
                                           // whole tile (token-major pool, all heads in the tile), 2 one copy per row
 };
@@ -228,7 +233,7 @@ __device__ __forceinline__ void requant_fp8(uint4& A, float s_src, float inv_dst
 // MAXT = 256: the default launch shape (<= 8 warps, 2 CTAs per SM) gets 128 registers per thread and no spills;
 // MAXT = kMaxThreads: the wide shapes the tuning knobs allow (up to 16 consumer warps, or 3+ CTAs per SM).
 template <int DTYPE, int PAIRING, bool MAP, int MAXT>
-__global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1))
+__global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1))   // 256 x 2, 448 x 1: 128 registers; 544 x 1: 96
 kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ RingParams RP) {
   using G = Geo<DTYPE, PAIRING>;
   constexpr int E = (DTYPE == 0) ? 2 : 1;
@@ -241,7 +246,7 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
   const int S = RP.S, NW = RP.NW;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < S; ++s) { mbar_init(s_full + 8u * s, 1); mbar_init(s_empty + 8u * s, 1); }
+    for (int s = 0; s < S; ++s) { mbar_init(s_full + 8u * s, 1); mbar_init(s_empty + 8u * s, (uint32_t)RP.wpg); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   // Programmatic dependent launch: let the next launch on this stream bring its CTAs up (they take an SM's shared
@@ -452,8 +457,8 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       base = base_n;
       d_si = n_si; d_t0 = n_t0; d_ntok = n_ntok; d_off = n_off; d_lg = n_lg; d_blk = n_blk;
     }
-    // one DONE tile per consumer warp, through the same ring (NW <= S, so the stages are distinct)
-    if (lane < NW) {
+    // one DONE tile per consumer warp (per group of wpg warps), through the same ring (NW / wpg <= S: distinct stages)
+    if (lane < NW / RP.wpg) {
       int my_stage = stage + lane;
       uint32_t my_phase = phase;
       if (my_stage >= S) { my_stage -= S; my_phase ^= 1u; }
@@ -503,8 +508,66 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
   int my_gen = -1, my_run = -1;
   const bool dst_rows_packed = (P.d_st == P.head_dim);
 
-  int stage = warp % S;
-  uint32_t phase = (uint32_t)(warp / S) & 1u;
+  const int wpg = RP.wpg, wsub = warp % wpg, stage_step = NW / wpg;
+  int stage = (warp / wpg) % S;
+  uint32_t phase = (uint32_t)((warp / wpg) / S) & 1u;
+
+  // one K row-slot of this lane: load, rotate (or requantise), store
+  auto k_row = [&](const TileMeta& m, uint32_t tab, bool rotate, uint32_t ks, uint8_t* kd, int t, int sm_st,
+                   float s_src, float inv_dst, bool requant) {
+    uint4 A = lds128(ks + t * sm_st + va * 16);
+    uint4 B = lds128(ks + t * sm_st + vb * 16);
+    bool rot_row = rotate;
+    if (MAP) {
+      const int run = reinterpret_cast<const int32_t*>(smem + RP.off_tab + m.tab * RP.tab_stride + RP.cg * RP.half_R * 16)[t];
+      rot_row = run >= 0;
+      if (rot_row && (rot_a || rot_b) && (run != my_run || m.gen != my_gen)) {   // cos/sin registers follow the run
+        my_run = run; my_gen = m.gen;
+        const uint32_t trow = tab + run * RP.half_R * 16;
+#pragma unroll
+        for (int k = 0; k < G::NT; ++k) {
+          float4 e = lds128f(trow + tpos[k] * 16);
+          if (DTYPE == 0) T4[k] = e; else T2[k] = make_float2(e.x, e.z);
+        }
+      }
+    }
+    if constexpr (DTYPE == 0) {
+      if (rot_row) {
+        if constexpr (PAIRING == 0) { if (rot_a) rot_bf16_neox(A, B, T4); }
+        else { if (rot_a) rot_bf16_gptj(A, T4); if (rot_b) rot_bf16_gptj(B, T4 + G::PPV); }
+      }
+    } else if (rot_row || requant) {
+      if (requant) {
+        if constexpr (PAIRING == 0) {
+          if (rot_a) rot_fp8_neox<true>(A, B, T2, s_src, inv_dst, rot_row);
+          else { requant_fp8(A, s_src, inv_dst); requant_fp8(B, s_src, inv_dst); }
+        } else {
+          if (rot_a) rot_fp8_gptj<true>(A, T2, s_src, inv_dst, rot_row); else requant_fp8(A, s_src, inv_dst);
+          if (rot_b) rot_fp8_gptj<true>(B, T2 + G::PPV, s_src, inv_dst, rot_row); else requant_fp8(B, s_src, inv_dst);
+        }
+      } else {                       // equal scales (then rot_row holds): they cancel
+        if constexpr (PAIRING == 0) {
+          if (rot_a) rot_fp8_neox<false>(A, B, T2, 1.0f, 1.0f, true);
+        } else {
+          if (rot_a) rot_fp8_gptj<false>(A, T2, 1.0f, 1.0f, true);
+          if (rot_b) rot_fp8_gptj<false>(B, T2 + G::PPV, 1.0f, 1.0f, true);
+        }
+      }
+    }
+    uint8_t* row = kd + (int64_t)t * P.d_st * E;
+    stg128(row + va * 16, A);
+    stg128(row + vb * 16, B);
+  };
+  auto head_scales = [&](const TileMeta& m, int hh, float& s_src, float& inv_dst, bool& requant) {
+    s_src = 1.0f; inv_dst = 1.0f; requant = false;
+    if (DTYPE == 1) {
+      const float s_dst = s_scales[m.scale_idx + hh];
+      s_src = P.scales_differ ? seg_array(P)[m.seg].k_scale_src[m.scale_idx + hh] : s_dst;
+      requant = (s_src != s_dst);
+      inv_dst = __frcp_rn(s_dst);
+    }
+  };
+
   for (;; ) {
     mbar_wait(s_full + 8u * stage, phase, 4);
     const TileMeta m = meta[stage];
@@ -516,6 +579,18 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     // ---- V (step a6): bytes unchanged ----
     if (RP.no_v) {
       // in-place: V is position-free and already where it belongs
+    } else if (RP.gather) {
+      // gather mode: this warp's tokens leave by one bulk (TMA) store per (token, head) row, heads innermost, so the
+      // rows of a token arrive back to back and form one contiguous H*D run of the dense token-major pool
+      for (int t0 = wsub * rpi; t0 < n_tok; t0 += rpi * wpg) {
+        const int rows = min(rpi, n_tok - t0) * RP.hpt;
+        for (int idx = lane; idx < rows; idx += 32) {
+          const int tt = t0 + idx / RP.hpt, hh = idx % RP.hpt;
+          bulk_s2g(P.v_cache + (m.dst_off + (int64_t)tt * P.d_st + (int64_t)hh * P.d_sh) * E,
+                   sv + (hh * RP.cg + tt) * RP.rowB, (uint32_t)RP.rowB);
+        }
+      }
+      bulk_commit();
     } else if (RP.v_bulk == 2) {
       // token-major pool: one bulk store per (head, token) row, lane r issues row r (n_tok <= 32)
       for (int hh = 0; hh < RP.hpt; ++hh)
@@ -558,61 +633,22 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     }
     const int sm_sh = (m.flags & kFlagTokMajor) ? RP.rowB : RP.cg * RP.rowB;        // stage strides of a head / a token
     const int sm_st = (m.flags & kFlagTokMajor) ? RP.hpt * RP.rowB : RP.rowB;
+    if (RP.gather) {
+      // gather mode: tokens outer, heads inner -- a pass of this warp completes rpi whole token rows
+      for (int t = rsub + wsub * rpi; t < n_tok; t += rpi * wpg)
+        for (int hh = 0; hh < RP.hpt; ++hh) {
+          float s_src, inv_dst; bool requant;
+          head_scales(m, hh, s_src, inv_dst, requant);
+          k_row(m, tab, rotate, sk + hh * sm_sh, P.k_cache + (m.dst_off + (int64_t)hh * P.d_sh) * E, t, sm_st,
+                s_src, inv_dst, requant);
+        }
+    } else
     for (int hh = 0; hh < RP.hpt; ++hh) {
       const uint32_t ks = sk + hh * sm_sh;
       uint8_t* kd = P.k_cache + (m.dst_off + (int64_t)hh * P.d_sh) * E;
-      float s_src = 1.0f, inv_dst = 1.0f;
-      bool requant = false;
-      if (DTYPE == 1) {
-        const float s_dst = s_scales[m.scale_idx + hh];
-        s_src = P.scales_differ ? seg_array(P)[m.seg].k_scale_src[m.scale_idx + hh] : s_dst;
-        requant = (s_src != s_dst);
-        inv_dst = __frcp_rn(s_dst);
-      }
-      for (int t = rsub; t < n_tok; t += rpi) {
-        uint4 A = lds128(ks + t * sm_st + va * 16);
-        uint4 B = lds128(ks + t * sm_st + vb * 16);
-        bool rot_row = rotate;
-        if (MAP) {
-          const int run = reinterpret_cast<const int32_t*>(smem + RP.off_tab + m.tab * RP.tab_stride + RP.cg * RP.half_R * 16)[t];
-          rot_row = run >= 0;
-          if (rot_row && (rot_a || rot_b) && (run != my_run || m.gen != my_gen)) {   // cos/sin registers follow the run
-            my_run = run; my_gen = m.gen;
-            const uint32_t trow = tab + run * RP.half_R * 16;
-#pragma unroll
-            for (int k = 0; k < G::NT; ++k) {
-              float4 e = lds128f(trow + tpos[k] * 16);
-              if (DTYPE == 0) T4[k] = e; else T2[k] = make_float2(e.x, e.z);
-            }
-          }
-        }
-        if constexpr (DTYPE == 0) {
-          if (rot_row) {
-            if constexpr (PAIRING == 0) { if (rot_a) rot_bf16_neox(A, B, T4); }
-            else { if (rot_a) rot_bf16_gptj(A, T4); if (rot_b) rot_bf16_gptj(B, T4 + G::PPV); }
-          }
-        } else if (rot_row || requant) {
-          if (requant) {
-            if constexpr (PAIRING == 0) {
-              if (rot_a) rot_fp8_neox<true>(A, B, T2, s_src, inv_dst, rot_row);
-              else { requant_fp8(A, s_src, inv_dst); requant_fp8(B, s_src, inv_dst); }
-            } else {
-              if (rot_a) rot_fp8_gptj<true>(A, T2, s_src, inv_dst, rot_row); else requant_fp8(A, s_src, inv_dst);
-              if (rot_b) rot_fp8_gptj<true>(B, T2 + G::PPV, s_src, inv_dst, rot_row); else requant_fp8(B, s_src, inv_dst);
-            }
-          } else {                       // equal scales (then rot_row holds): they cancel
-            if constexpr (PAIRING == 0) {
-              if (rot_a) rot_fp8_neox<false>(A, B, T2, 1.0f, 1.0f, true);
-            } else {
-              if (rot_a) rot_fp8_gptj<false>(A, T2, 1.0f, 1.0f, true);
-              if (rot_b) rot_fp8_gptj<false>(B, T2 + G::PPV, 1.0f, 1.0f, true);
-            }
-          }
-        }
-        uint8_t* row = kd + (int64_t)t * P.d_st * E;
-        stg128(row + va * 16, A);
-        stg128(row + vb * 16, B);
-      }
+      float s_src, inv_dst; bool requant;
+      head_scales(m, hh, s_src, inv_dst, requant);
+      for (int t = rsub; t < n_tok; t += rpi) k_row(m, tab, rotate, ks, kd, t, sm_st, s_src, inv_dst, requant);
       if (RP.win) {
         // window mode: everything outside the rotary window (the MLA latent) is position-free -- 16-byte copies
         const int npass = nv - nr, total = n_tok * npass;
@@ -626,13 +662,13 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         }
       }
     }
-    if (RP.v_bulk == 2 || (RP.v_bulk && lane == 0)) bulk_wait_read0();   // V bytes have left shared memory
+    if (RP.v_bulk == 2 || (RP.gather && !RP.no_v) || (RP.v_bulk && lane == 0)) bulk_wait_read0();   // V bytes have left shared memory
     __syncwarp();
     if (lane == 0) mbar_arrive(s_empty + 8u * stage);
-    stage += NW;
+    stage += stage_step;
     if (stage >= S) { stage -= S; phase ^= 1u; }
   }
-  if (RP.v_bulk == 2 || (RP.v_bulk && lane == 0)) bulk_wait_all0();
+  if (RP.v_bulk == 2 || (RP.gather && !RP.no_v) || (RP.v_bulk && lane == 0)) bulk_wait_all0();
   (void)dst_rows_packed;
 }
 
@@ -741,9 +777,17 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   int S = cfg.stages > 0 ? cfg.stages : 64;
   while (S > 2 && layout(S) > budget) --S;
   if (layout(S) > budget) return cudaErrorInvalidConfiguration;
-  if (S < RP.NW) RP.NW = S;
-  S -= S % RP.NW;   // stage s is always served by consumer warp s % NW: successive phases of one mbarrier are then
-                    // ordered by one warp's program order (a warp two phases ahead would pass a parity wait early)
+  // Stage ownership: consumer warp w serves stages (w / wpg) + k * (NW / wpg); S is a multiple of NW / wpg, so the
+  // successive phases of one mbarrier are ordered by one warp's program order (a warp two phases ahead would pass a
+  // parity wait early).  wpg > 1 only in gather mode, when the ring holds fewer (large) stages than consumer warps.
+  RP.gather = P.gather ? 1 : 0;
+  RP.wpg = 1;
+  if (S >= RP.NW) {
+    S -= S % RP.NW;
+  } else {
+    if (RP.gather) RP.wpg = RP.NW / S;      // >= 1; NW <= 16 is kept
+    RP.NW = S * RP.wpg;
+  }
   RP.S = S;
   const int smem = layout(S);
   // V out of shared memory: 1 = one bulk store per (head, chunk) run (needs d_st == head_dim), 2 = one bulk store per
@@ -753,7 +797,7 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   else if (cfg.v_bulk_store == 3) RP.v_bulk = 2;
   else if (cfg.v_bulk_store == 1) RP.v_bulk = runs ? 1 : 2;
   else RP.v_bulk = runs ? 1 : 0;
-  if (RP.no_v) RP.v_bulk = 0;
+  if (RP.no_v || RP.gather) RP.v_bulk = 0;
   int64_t g = (int64_t)sm_count * ctas;
   if (cfg.max_ctas > 0 && g > cfg.max_ctas) g = cfg.max_ctas;
   if (g > P.total_units) g = P.total_units;
@@ -761,9 +805,10 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   const int block = (RP.NW + 1) * 32;
   *grid_out = (int)g; *block_out = block; *smem_out = smem;
   const bool map = P.any_pos_map != 0;
-  const bool small = block <= 256 && ctas <= 2;
+  const bool small = block <= 256 && ctas <= 2, mid = block <= 448 && ctas == 1;
 #define KVR_LAUNCH(D, PR, M)                                                                             \
   return small ? launch_inst<D, PR, M, 256>(P, RP, (int)g, block, smem, stream, cfg.pdl != 2)            \
+         : mid ? launch_inst<D, PR, M, 448>(P, RP, (int)g, block, smem, stream, cfg.pdl != 2)            \
                : launch_inst<D, PR, M, kMaxThreads>(P, RP, (int)g, block, smem, stream, cfg.pdl != 2)
   if (P.dtype == 0) {
     if (P.pairing == 0) { if (map) KVR_LAUNCH(0, 0, true); else KVR_LAUNCH(0, 0, false); }

@@ -322,3 +322,25 @@ def test_time_is_linear_in_tokens():
     r2 = 1 - ((y - (slope * x + icpt)) ** 2).sum() / ((y - y.mean()) ** 2).sum()
     assert r2 > 0.99, (ts, r2)
     assert abs(icpt) < 0.015, (icpt, ts)                # ms: the line passes near the origin (a launch's fixed cost)
+
+
+# ------------------------------------------------------------------ gather mode of the ring kernel (dense NHD pools)
+@pytest.mark.parametrize("tuning", [dict(gather=1), dict(gather=2), dict(gather=1, consumer_warps=4),
+                                    dict(gather=1, max_ctas=2, stages=2, consumer_warps=6),
+                                    dict(gather=1, max_ctas=3, stages=3, consumer_warps=9, ctas_per_sm=1),
+                                    dict(gather=1, tile_bytes=32768, ctas_per_sm=1, consumer_warps=12),
+                                    dict(gather=1, tile_bytes=4096, consumer_warps=5)])
+@pytest.mark.parametrize("c", [0, 1, 2, 3, 4])
+def test_gather_mode(c, tuning):
+    """Tiles of all heads x few tokens shared by several consumer warps (tokens outer, heads inner, V by row-wise
+    bulk stores): forced on and off on every config; few CTAs and short rings exercise the shared-stage hand-shake."""
+    check_parity(config_small(c, "NHD"), "ring", **tuning)
+
+
+@pytest.mark.parametrize("bs", [2, 8, 16, 24, 128])
+@pytest.mark.parametrize("heads,D,dtype", [(4, 128, "bf16"), (2, 64, "bf16"), (6, 128, "bf16"), (8, 128, "fp8")])
+def test_gather_mode_ragged_blocks(bs, heads, D, dtype):
+    w = make_workload(name="gbs", layers=2, kv_heads=heads, head_dim=D, theta=1e6, block_size=bs, seed=6, dtype=dtype,
+                      seq_segments=[[dict(len=333, dst_token_start=bs + 3, new_start=2000), dict(len=1, dst_token_start=0)],
+                                    [dict(len=77, dst_token_start=1, new_start=9)]])
+    check_parity(w, "ring", gather=1)
