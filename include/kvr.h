@@ -135,7 +135,7 @@ typedef struct {
                               divisor of block_size below it                                                          */
   int32_t tile_bytes;      /* ring kernel: a tile takes the fewest heads whose K run reaches this size (default 4096) */
   int32_t gather;          /* ring kernel, dense token-major pools: tiles of all heads x few tokens, several consumer
-                              warps per tile (see kvr_ring.cu): 0 auto (on), 1 on, 2 off                              */
+                              warps per tile (see kvr_ring.cu): 0 auto, 1 on, 2 off, 3 on with K and V in tiles of their own                            */
   int32_t reserved[3];
 } kvr_tuning;
 

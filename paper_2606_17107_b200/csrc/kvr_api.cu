@@ -324,7 +324,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       // concurrently read neighbouring source rows of one layer (DRAM page locality: +3 % on configs[2] against
       // 11 layers per unit) and the tail is short.  With a position map the per-chunk angle table is rebuilt per
       // unit, so a unit holds ~24 tiles there.
-      const int tiles_per_layer = (m.kv_heads / ring_heads_per_tile(P)) / hsplit;
+      const int tiles_per_layer = ((m.kv_heads / ring_heads_per_tile(P)) / hsplit) * (P.gather == 2 ? 2 : 1);
       const int want = P.gather ? (any_map ? 6 : 2)      // gather tiles are 32 KB: the same 64 KB / 192 KB per unit
                                 : (any_map ? 24 : 8);
       lpu = (want + tiles_per_layer - 1) / tiles_per_layer;
@@ -363,16 +363,24 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       const int64_t rowB = (int64_t)m.head_dim * E;
       const bool pow2_row = rowB >= 32 && rowB <= 1024 && (rowB & (rowB - 1)) == 0 && m.rotary_offset == 0;
       const bool dense_nhd = d->stride_head == m.head_dim && d->stride_token == (int64_t)m.kv_heads * m.head_dim;
-      const int64_t tile_target = tu.tile_bytes > 0 ? tu.tile_bytes : 16384;      // K bytes of a gather tile
+      // A gather stage is <= 32 KB: K and V of all heads of a full chunk together if they fit (mode 1), else K and V
+      // in tiles of their own (mode 2, "split": a full chunk of ONE tensor), else a shorter chunk (mode 1).
+      const int cg_full = chunk_granularity(d->block_size, 16);
+      const int64_t chunk_bytes = (int64_t)m.kv_heads * cg_full * rowB;          // one tensor, all heads, a full chunk
+      int mode = 1;
+      int64_t tile_target = tu.tile_bytes > 0 ? tu.tile_bytes : 16384;             // K bytes of a gather tile
+      // (mode 2 is never chosen automatically: on B200 it measured +1.5 % on configs[1] and -1 % on configs[2] for 8 heads
+      //  of 128 bf16, -12 % in fp8: a V-only stage has no arithmetic to hide its row stores behind.)
+      (void)chunk_bytes;
+      if (tu.gather == 3) { mode = 2; if (tu.tile_bytes <= 0) tile_target = 32768; }
       int64_t lim = tile_target / (m.kv_heads * rowB);
       const int cg_g = chunk_granularity(d->block_size, (int)(lim > 16 ? 16 : lim));
-      // auto: only where it was measured to pay (B200): bf16, and all heads of a FULL chunk fit the tile, so
-      // the source runs are not shortened (kv_heads * head_dim <= 512 elements: +4.6 % on configs[4], +2 % on the 4-head
-      // image-KV shape).  With 8 heads of 128 the chunk halves to 8 tokens (2 KB source runs): a wash (+-1 %).  fp8: -7 %.
-      const bool pays = m.dtype == KVR_BF16 && cg_g == chunk_granularity(d->block_size, 16);
-      if (tu.gather != 2 && (tu.gather == 1 || pays) && tu.chunk_tokens <= 0 && (tu.tile_bytes <= 0 || tu.gather == 1) &&
-          tu.hsplit <= 1 && !inplace && pow2_row && dense_nhd && m.kv_heads > 1 && m.kv_heads * rowB <= 8192 && cg_g >= 2) {
-        P.gather = 1;
+      // auto: only where it was measured to pay (B200): bf16 and source runs that are not shortened.
+      const bool pays = m.dtype == KVR_BF16 && cg_g == cg_full;
+      if (tu.gather != 2 && (tu.gather == 1 || tu.gather == 3 || pays) && tu.chunk_tokens <= 0 &&
+          (tu.tile_bytes <= 0 || tu.gather == 1 || tu.gather == 3) && tu.hsplit <= 1 && !inplace && pow2_row && dense_nhd &&
+          m.kv_heads > 1 && m.kv_heads * rowB <= 8192 && cg_g >= 2) {
+        P.gather = (mode == 2 && d->v_cache) ? 2 : 1;
         cg_limit = cg_g;
         P.tile_min_bytes = (int32_t)(m.kv_heads * cg_g * rowB);
       }

@@ -43,6 +43,7 @@ struct RingParams {
   int nv_slot;                            // vectors the lane slots are laid over: nv, or nr in window mode
   int ro_v;                               // rotary_offset in 16-byte vectors
   int gather;                             // GATHER mode (see wpg)
+  int split;                              // gather tiles hold K or V alone (all heads of a FULL chunk of one tensor)
   int wpg;                                // GATHER mode (dense token-major pools): a tile holds ALL heads of a few tokens and
                                           // wpg consumer warps share it, each taking whole token rows, tokens outer / heads
                                           // inner, so that a token's H*D row reaches L2 (and DRAM) as one contiguous burst
@@ -63,6 +64,7 @@ struct __align__(16) TileMeta {
 static_assert(sizeof(TileMeta) == 32, "TileMeta layout");
 
 constexpr int kFlagDone = 1, kFlagRotate = 2, kFlagTokMajor = 4;   // TokMajor: the stage is laid out [token][head][dim]
+constexpr int kFlagKOnly = 8, kFlagVOnly = 16;                       // split gather tiles: the stage holds K or V alone
 constexpr int kMaxThreads = 32 * 17;
 
 // ------------------------------------------------------------------------------- PTX helpers
@@ -280,8 +282,7 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     int tb = 0, gen = 0;           // current table buffer / generation
     int64_t cur_key = -1;          // segment (segment mode) or unit (map mode) the current table belongs to
     if (pre_si >= 0) { tb = 1; gen = 1; cur_key = pre_si; }   // built before the dependency wait
-    uint32_t lu_i[2] = {0, 0}, lu_phase[2] = {0, 0};   // last tile that used each table buffer
-    int lu_stage[2] = {0, 0};
+    uint32_t lu_i[2] = {0, 0};     // last tile that used each table buffer
     bool lu_valid[2] = {false, false};
     int cur_si = -1;
     SegDev sg{};                   // current segment, held in registers
@@ -347,8 +348,16 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         const int64_t key = MAP ? (base + j) : (int64_t)si;
         if (key != cur_key) {
           const int nb = tb ^ 1;
-          if (lane == 0 && (nb ? lu_valid[1] : lu_valid[0]) && (nb ? lu_i[1] : lu_i[0]) + (uint32_t)S >= i)   // tiles <= i-1-S are known released
-            mbar_wait(s_empty + 8u * (nb ? lu_stage[1] : lu_stage[0]), nb ? lu_phase[1] : lu_phase[0], 1);   // its last reader may still be in flight
+          // Buffer nb was last read by the tiles up to lu_i[nb].  Consumer warps take their stages in order, so once
+          // the newest tile of EACH warp (group) among those is released, every older one is: wait for the last
+          // NW / wpg tiles up to lu_i (tile j sits in stage j % S, use j / S); tiles <= i-1-S are known released.
+          if (nb ? lu_valid[1] : lu_valid[0]) {
+            const uint32_t last = nb ? lu_i[1] : lu_i[0];
+            if ((uint32_t)lane < (uint32_t)(NW / RP.wpg) && (uint32_t)lane <= last) {
+              const uint32_t j = last - (uint32_t)lane;
+              if (j + (uint32_t)S >= i) mbar_wait(s_empty + 8u * (j % (uint32_t)S), (j / (uint32_t)S) & 1u, 1);
+            }
+          }
           __syncwarp();
           float4* tab = reinterpret_cast<float4*>(smem + RP.off_tab + nb * RP.tab_stride);
           if (MAP) {
@@ -385,7 +394,8 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
           const int lgi = lg / P.hsplit, hpart = lg - lgi * P.hsplit;     // layer group, head part of this unit
           const int l0 = lgi * P.lpu, l1 = min(P.layers, l0 + P.lpu);
           const int hg_per = hgroups / P.hsplit;
-          const int n_tiles = (l1 - l0) * hg_per;
+          const int kinds = RP.split ? 2 : 1;                            // split: a K tile, then a V tile
+          const int n_tiles = (l1 - l0) * hg_per * kinds;
           const bool inplace = P.inplace != 0;
           const int flags = ((MAP || sg.delta != 0) ? kFlagRotate : 0) | ((inplace && RP.ip_mode == 1) ? kFlagTokMajor : 0);
           const uint32_t run_bytes = (uint32_t)(n_tok * RP.rowB);
@@ -396,7 +406,8 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
           for (int tb0 = 0; tb0 < n_tiles; tb0 += pass) {
             const int n = min(pass, n_tiles - tb0);
             if (lane < n) {
-              const int t = tb0 + lane;
+              const int t = (tb0 + lane) / kinds;
+              const int kind = RP.split ? (tb0 + lane) - t * kinds : -1;      // 0: K tile, 1: V tile, -1: both
               const int l = l0 + t / hg_per, h0 = (hpart * hg_per + t % hg_per) * RP.hpt;
               int my_stage = stage + lane;
               uint32_t my_phase = phase;
@@ -405,12 +416,14 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
               mbar_wait(s_empty + 8u * my_stage, my_phase ^ 1u, 2);
               TileMeta m;
               m.dst_off = (int64_t)l * P.d_sl + dst_chunk + (int64_t)h0 * P.d_sh;
-              m.n_tok = n_tok; m.flags = flags; m.tab = tb; m.gen = gen;
+              m.n_tok = n_tok; m.tab = tb; m.gen = gen;
+              m.flags = flags | (kind == 0 ? kFlagKOnly : 0) | (kind == 1 ? kFlagVOnly : 0);
               m.scale_idx = l * P.heads + h0; m.seg = si;
               meta[my_stage] = m;
-              mbar_arrive_expect_tx(bar, (RP.no_v ? 1u : 2u) * RP.hpt * run_bytes);
+              mbar_arrive_expect_tx(bar, ((RP.no_v || RP.split) ? 1u : 2u) * RP.hpt * run_bytes);
               const uint32_t sk = s_base + RP.off_stage + (uint32_t)my_stage * RP.stage_bytes;
-              const uint32_t sv = sk + RP.tile_bytes;
+              const uint32_t sv = RP.split ? sk : sk + RP.tile_bytes;
+              const bool ld_k = kind != 1, ld_v = kind != 0 && !RP.no_v;
               if (inplace) {
                 // the tile's source IS its destination: K rows already resident in the paged pool (R20)
                 const uint8_t* src = P.k_cache + m.dst_off * E;
@@ -430,12 +443,12 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
                 const int64_t src_off = ((int64_t)l * sg.sl + (int64_t)(h0 + hh) * sg.sh + src_chunk) * E;
                 const uint32_t so = (uint32_t)(hh * RP.cg * RP.rowB);
                 if (packed_rows) {
-                  bulk_g2s(sk + so, sg.k_src + src_off, run_bytes, bar, pol);
-                  if (!RP.no_v) bulk_g2s(sv + so, sg.v_src + src_off, run_bytes, bar, pol);
+                  if (ld_k) bulk_g2s(sk + so, sg.k_src + src_off, run_bytes, bar, pol);
+                  if (ld_v) bulk_g2s(sv + so, sg.v_src + src_off, run_bytes, bar, pol);
                 } else {
                   for (int r = 0; r < n_tok; ++r) {
-                    bulk_g2s(sk + so + r * RP.rowB, sg.k_src + src_off + (int64_t)r * sg.st * E, RP.rowB, bar, pol);
-                    if (!RP.no_v) bulk_g2s(sv + so + r * RP.rowB, sg.v_src + src_off + (int64_t)r * sg.st * E, RP.rowB, bar, pol);
+                    if (ld_k) bulk_g2s(sk + so + r * RP.rowB, sg.k_src + src_off + (int64_t)r * sg.st * E, RP.rowB, bar, pol);
+                    if (ld_v) bulk_g2s(sv + so + r * RP.rowB, sg.v_src + src_off + (int64_t)r * sg.st * E, RP.rowB, bar, pol);
                   }
                 }
               }
@@ -447,10 +460,8 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
           }
           // the unit's last tile is the last reader of table buffer tb
           if (n_tiles > 0) {
-            const int ls = (stage == 0) ? S - 1 : stage - 1;
-            const uint32_t lp = (stage == 0) ? (phase ^ 1u) : phase;
-            if (tb) { lu_i[1] = i - 1u; lu_stage[1] = ls; lu_phase[1] = lp; lu_valid[1] = true; }
-            else { lu_i[0] = i - 1u; lu_stage[0] = ls; lu_phase[0] = lp; lu_valid[0] = true; }
+            if (tb) { lu_i[1] = i - 1u; lu_valid[1] = true; }
+            else { lu_i[0] = i - 1u; lu_valid[0] = true; }
           }
         }
       }
@@ -573,11 +584,11 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     const TileMeta m = meta[stage];
     if (m.flags & kFlagDone) break;
     const uint32_t sk = s_base + RP.off_stage + (uint32_t)stage * RP.stage_bytes;
-    const uint32_t sv = sk + RP.tile_bytes;
+    const uint32_t sv = RP.split ? sk : sk + RP.tile_bytes;
     const int n_tok = m.n_tok;
 
     // ---- V (step a6): bytes unchanged ----
-    if (RP.no_v) {
+    if (RP.no_v || (m.flags & kFlagKOnly)) {
       // in-place: V is position-free and already where it belongs
     } else if (RP.gather) {
       // gather mode: this warp's tokens leave by one bulk (TMA) store per (token, head) row, heads innermost, so the
@@ -633,7 +644,9 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     }
     const int sm_sh = (m.flags & kFlagTokMajor) ? RP.rowB : RP.cg * RP.rowB;        // stage strides of a head / a token
     const int sm_st = (m.flags & kFlagTokMajor) ? RP.hpt * RP.rowB : RP.rowB;
-    if (RP.gather) {
+    if (m.flags & kFlagVOnly) {
+      // split gather tile holding V alone: nothing to rotate
+    } else if (RP.gather) {
       // gather mode: tokens outer, heads inner -- a pass of this warp completes rpi whole token rows
       for (int t = rsub + wsub * rpi; t < n_tok; t += rpi * wpg)
         for (int hh = 0; hh < RP.hpt; ++hh) {
@@ -755,7 +768,8 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   const int hpt = ring_heads_per_tile(P);
   RP.hpt = hpt;
   RP.tile_bytes = hpt * RP.cg * RP.rowB;
-  RP.stage_bytes = (RP.no_v ? 1 : 2) * RP.tile_bytes;
+  RP.split = (P.gather == 2 && !RP.no_v) ? 1 : 0;
+  RP.stage_bytes = ((RP.no_v || RP.split) ? 1 : 2) * RP.tile_bytes;
   const int ctas = cfg.ctas_per_sm > 0 ? cfg.ctas_per_sm : 2;
   RP.NW = cfg.consumer_warps > 0 ? cfg.consumer_warps : 6;
   if (RP.NW > 16) RP.NW = 16;

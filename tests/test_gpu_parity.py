@@ -329,7 +329,9 @@ def test_time_is_linear_in_tokens():
                                     dict(gather=1, max_ctas=2, stages=2, consumer_warps=6),
                                     dict(gather=1, max_ctas=3, stages=3, consumer_warps=9, ctas_per_sm=1),
                                     dict(gather=1, tile_bytes=32768, ctas_per_sm=1, consumer_warps=12),
-                                    dict(gather=1, tile_bytes=4096, consumer_warps=5)])
+                                    dict(gather=1, tile_bytes=4096, consumer_warps=5),
+                                    dict(gather=3), dict(gather=3, max_ctas=2, stages=2, consumer_warps=4),
+                                    dict(gather=3, max_ctas=3, stages=5, consumer_warps=10, ctas_per_sm=1)])
 @pytest.mark.parametrize("c", [0, 1, 2, 3, 4])
 def test_gather_mode(c, tuning):
     """Tiles of all heads x few tokens shared by several consumer warps (tokens outer, heads inner, V by row-wise
@@ -344,3 +346,4 @@ def test_gather_mode_ragged_blocks(bs, heads, D, dtype):
                       seq_segments=[[dict(len=333, dst_token_start=bs + 3, new_start=2000), dict(len=1, dst_token_start=0)],
                                     [dict(len=77, dst_token_start=1, new_start=9)]])
     check_parity(w, "ring", gather=1)
+    check_parity(w, "ring", gather=3)
