@@ -52,6 +52,10 @@
  * tests/test_oracle_inplace.py: the pi/2 closed form through brute-force slot
  * enumeration, Delta = 0 leaves every byte, untouched slots and pass-through dims
  * keep their bytes, Delta then -Delta, and the RoPE identity through the pool.
+ * kvr_oracle_reposition_splice_ex / _inplace_ex (reading R23, the MLA [latent | k_pe] row) are
+ * pinned by tests/test_oracle_adapters.py: the pi/2 closed form at the window's offset pair indices, a numpy RoPE of
+ * the k_pe sub-vector with exact-rational rounding, latent bytes equal, the RoPE identity through bf16,
+ * exact-rational fp8 requantisation of the latent under a scale change, in-place == splice.
  * Nothing in this file is "parity unpinned".
  *
  * Build: gcc -O2 -std=c11 -fopenmp -shared -fPIC (oracle/build.py).  No
