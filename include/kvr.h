@@ -136,7 +136,8 @@ typedef struct {
   int32_t tile_bytes;      /* ring kernel: a tile takes the fewest heads whose K run reaches this size (default 4096) */
   int32_t gather;          /* ring kernel, dense token-major pools: tiles of all heads x few tokens, several consumer
                               warps per tile (see kvr_ring.cu): 0 auto, 1 on, 2 off, 3 on with K and V in tiles of their own                            */
-  int32_t reserved[3];
+  int32_t warps_per_stage; /* gather mode: consumer warps that share one stage (default: all of them)                  */
+  int32_t reserved[2];
 } kvr_tuning;
 
 /* Creates a context on CUDA device `cuda_device` (must be compute capability 10.x).  Allocates a few

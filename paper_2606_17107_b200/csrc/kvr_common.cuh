@@ -163,7 +163,7 @@ __device__ __forceinline__ uint32_t f32x2_to_e4m3x2_sat(float lo, float hi) {
 cudaError_t launch_generic(const CallParams& P, int sm_count, cudaStream_t stream, int* grid, int* block, int* smem);
 
 struct RingConfig {
-  int ctas_per_sm, consumer_warps, stages, v_bulk_store, max_ctas, grab, pdl;
+  int ctas_per_sm, consumer_warps, stages, v_bulk_store, max_ctas, grab, pdl, warps_per_stage;
 };
 int ring_heads_per_tile(const CallParams& P);   // heads one tile of the ring kernel covers (needs P.cg)
 bool ring_window_mode(const CallParams& P);      // rows outside the power-of-two slot layout (e.g. MLA [latent | k_pe])

@@ -593,13 +593,16 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     } else if (RP.gather) {
       // gather mode: this warp's tokens leave by one bulk (TMA) store per (token, head) row, heads innermost, so the
       // rows of a token arrive back to back and form one contiguous H*D run of the dense token-major pool
-      for (int t0 = wsub * rpi; t0 < n_tok; t0 += rpi * wpg) {
-        const int rows = min(rpi, n_tok - t0) * RP.hpt;
-        for (int idx = lane; idx < rows; idx += 32) {
-          const int tt = t0 + idx / RP.hpt, hh = idx % RP.hpt;
+      // Work items of a gather tile: (token group of rpi tokens, head), token group major; warp wsub of the wpg
+      // warps that share the stage takes a contiguous range of them.
+      const int items = ((n_tok + rpi - 1) / rpi) * RP.hpt, ipw = (items + wpg - 1) / wpg;
+      const int it0 = wsub * ipw, it1 = min(items, it0 + ipw);
+      for (int idx = lane; idx < (it1 - it0) * rpi; idx += 32) {
+        const int it = it0 + idx / rpi, r = idx - (idx / rpi) * rpi;
+        const int tg = it / RP.hpt, hh = it - tg * RP.hpt, tt = tg * rpi + r;
+        if (tt < n_tok)
           bulk_s2g(P.v_cache + (m.dst_off + (int64_t)tt * P.d_st + (int64_t)hh * P.d_sh) * E,
                    sv + (hh * RP.cg + tt) * RP.rowB, (uint32_t)RP.rowB);
-        }
       }
       bulk_commit();
     } else if (RP.v_bulk == 2) {
@@ -648,13 +651,16 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       // split gather tile holding V alone: nothing to rotate
     } else if (RP.gather) {
       // gather mode: tokens outer, heads inner -- a pass of this warp completes rpi whole token rows
-      for (int t = rsub + wsub * rpi; t < n_tok; t += rpi * wpg)
-        for (int hh = 0; hh < RP.hpt; ++hh) {
-          float s_src, inv_dst; bool requant;
-          head_scales(m, hh, s_src, inv_dst, requant);
+      const int items = ((n_tok + rpi - 1) / rpi) * RP.hpt, ipw = (items + wpg - 1) / wpg;
+      const int it1 = min(items, (wsub + 1) * ipw);
+      for (int it = wsub * ipw; it < it1; ++it) {
+        const int tg = it / RP.hpt, hh = it - tg * RP.hpt, t = tg * rpi + rsub;
+        float s_src, inv_dst; bool requant;
+        head_scales(m, hh, s_src, inv_dst, requant);
+        if (t < n_tok)
           k_row(m, tab, rotate, sk + hh * sm_sh, P.k_cache + (m.dst_off + (int64_t)hh * P.d_sh) * E, t, sm_st,
                 s_src, inv_dst, requant);
-        }
+      }
     } else
     for (int hh = 0; hh < RP.hpt; ++hh) {
       const uint32_t ks = sk + hh * sm_sh;
@@ -796,11 +802,21 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   // parity wait early).  wpg > 1 only in gather mode, when the ring holds fewer (large) stages than consumer warps.
   RP.gather = P.gather ? 1 : 0;
   RP.wpg = 1;
-  if (S >= RP.NW) {
+  if (RP.gather && (cfg.warps_per_stage > 0 || S < RP.NW)) {
+    // few large stages: every group of wpg warps walks the ring in NW / wpg strides.  Default: one group per stage
+    // (wpg = NW / S).  Measured on B200 (configs[4]): 2 warps per stage 6.44-6.50 TB/s, all 6 sharing every stage
+    // 6.34, 4 of 4 6.37; one CTA per SM with 12 warps (2-6 per stage, 2 stages per group) 6.13-6.35.
+    int wpg = cfg.warps_per_stage > 0 ? cfg.warps_per_stage : (RP.NW / S > 1 ? RP.NW / S : 1);
+    if (wpg > RP.NW) wpg = RP.NW;
+    int step = RP.NW / wpg;
+    if (step < 1) step = 1;
+    if (step > S) step = S;
+    while (S % step) --step;
+    RP.wpg = wpg; RP.NW = wpg * step;
+  } else if (S >= RP.NW) {
     S -= S % RP.NW;
   } else {
-    if (RP.gather) RP.wpg = RP.NW / S;      // >= 1; NW <= 16 is kept
-    RP.NW = S * RP.wpg;
+    RP.NW = S;
   }
   RP.S = S;
   const int smem = layout(S);

@@ -330,6 +330,8 @@ def test_time_is_linear_in_tokens():
                                     dict(gather=1, max_ctas=3, stages=3, consumer_warps=9, ctas_per_sm=1),
                                     dict(gather=1, tile_bytes=32768, ctas_per_sm=1, consumer_warps=12),
                                     dict(gather=1, tile_bytes=4096, consumer_warps=5),
+                                    dict(gather=1, warps_per_stage=6), dict(gather=3, warps_per_stage=4, consumer_warps=4),
+                                    dict(gather=1, warps_per_stage=3, consumer_warps=12, ctas_per_sm=1, max_ctas=2),
                                     dict(gather=3), dict(gather=3, max_ctas=2, stages=2, consumer_warps=4),
                                     dict(gather=3, max_ctas=3, stages=5, consumer_warps=10, ctas_per_sm=1)])
 @pytest.mark.parametrize("c", [0, 1, 2, 3, 4])
