@@ -154,6 +154,13 @@ def _oracle_sample(c, layout, k_steps_total, get_sources, cpu_work_target_s=15.0
     t0 = time.perf_counter()
     orc.splice_workload(w1, s1, kc, vc, n_threads=threads)
     per_layer = time.perf_counter() - t0
+    # the canonical single-thread oracle on the same one-layer sample, if it ends within ~20 s
+    single = None
+    if per_layer * threads < 20.0:
+        t0 = time.perf_counter()
+        orc.splice_workload(w1, s1, kc, vc, n_threads=1)
+        single = full.tokens / ((time.perf_counter() - t0) * full.layers)
+    _oracle_sample.single_thread_value = single
     per_step_target = min(cpu_work_target_s / threads, wall_cap_s / max(1, k_steps_total))
     ls = int(max(1, min(full.layers, per_step_target / max(per_layer, 1e-9))))
     ls = max(ls, min(full.layers, -(-threads // full.kv_heads)))     # enough (layer, head) units for every thread
@@ -367,7 +374,9 @@ def run_kvr(args):
     cpu = None
     if rep.world == 1 and not args.no_cpu_baseline:
         v, per_step, threads, sample, _ = time_oracle(args.config, args.layout, 1, 0, cpu_sources_from_device(dw))
-        cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample}
+        cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+               "single_thread_value": getattr(_oracle_sample, "single_thread_value", None),
+               "single_thread_sample": "layer 0 of every segment, one thread, scaled linearly to all layers"}
 
     ctx.close()
     if rep.rank == 0:
