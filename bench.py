@@ -51,7 +51,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
     ap.add_argument("--workload", default="", help="an adapter workload instead of --config (SURVEY.md 8(f) NEXT-3/4): "
-                    "mla-dsv2-lite | image-kv-qwen25vl-7b | image-kv-qwen3vl-8b; device-timed and e2e only")
+                    "mla-dsv2-lite | image-kv-qwen25vl-7b | image-kv-qwen3vl-8b | compose-qwen3-8b; device-timed and e2e only")
     ap.add_argument("--layout", default="NHD", choices=["NHD", "HND"])
     ap.add_argument("--impl", default="kvr", choices=["kvr", "reference"])
     ap.add_argument("--latency", action="store_true",

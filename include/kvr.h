@@ -109,12 +109,20 @@ typedef struct {
  * delta_t = pos_map[t] - (old_start + t), and new_start is ignored.
  * k_scale_src: DEVICE fp32 [layers*kv_heads] source K scales (fp8 only); NULL = same as destination.
  * Two segments that write the same slot, or a source that aliases the destination, are undefined. */
+/* flags: KVR_SEG_PRE_ROPE (NEXT-4, "splice fused with the suffix-prefill KV write"; "TTFT is a
+ * re-rotation pass plus the suffix"): the segment's keys are not yet position-encoded -- the suffix keys a model has
+ * just projected -- i.e. EVERY source token sits at position old_start (0 for plain pre-RoPE keys: RoPE at 0 is the
+ * identity) and token t goes to its target position new_start + t (or pos_map[t]): delta_t = target_t - old_start.
+ * One kvr_reposition_splice call can thus carry the spliced skills (delta per segment), repaired seam tokens
+ * (delta = 0) and the fresh suffix (RoPE applied on the way into the cache): K is never materialised twice. */
+#define KVR_SEG_PRE_ROPE 1
 typedef struct {
   const void* k_src;
   const void* v_src;
   int64_t src_stride_layer, src_stride_head, src_stride_token; /* elements */
   int32_t len, old_start, new_start;
   int32_t dst_seq, dst_token_start;
+  int32_t flags; /* 0 or KVR_SEG_PRE_ROPE (occupies what used to be padding: the struct size is unchanged) */
   const int32_t* pos_map;
   const float* k_scale_src;
 } kvr_segment;

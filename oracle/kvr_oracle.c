@@ -74,6 +74,12 @@
 #define KVRO_FP8_E4M3 1
 #define KVRO_PAIR_NEOX_HALF 0
 #define KVRO_PAIR_GPTJ_INTERLEAVED 1
+/* Reading R24 (NEXT-4, "splice fused with the suffix-prefill KV write"; "TTFT is a
+ * re-rotation pass plus the suffix"): a segment whose keys are NOT yet position-encoded -- freshly projected suffix
+ * keys -- is a segment all of whose tokens sit at position old_start (0 for plain pre-RoPE keys, since RoPE at 0 is
+ * the identity); token t is rotated to its target position new_start + t (or pos_map[t]):
+ * Delta_t = target_t - old_start.  Everything else (pairing, rounding, slots, V) is unchanged. */
+#define KVRO_SEG_PRE_ROPE 1
 
 /* ------------------------------------------------------------------ codecs */
 
@@ -208,7 +214,7 @@ static int splice_core(
     const void* k_src, const void* v_src,
     int64_t src_stride_layer, int64_t src_stride_head, int64_t src_stride_token,
     int len, int old_start, int new_start, int dst_seq, int dst_token_start,
-    const int32_t* pos_map, const float* k_scale_src,
+    const int32_t* pos_map, const float* k_scale_src, int seg_flags,
     /* control */
     int layer_begin, int layer_end, int n_threads) {
   if (!inv_freq || !k_cache || !block_table || !k_src) return KVRO_ERR_INVALID_ARG;
@@ -223,7 +229,7 @@ static int splice_core(
   if (len <= 0 || dst_seq < 0 || dst_seq >= num_seqs || dst_token_start < 0) return KVRO_ERR_INVALID_ARG;
   if ((int64_t)dst_token_start + len > (int64_t)max_blocks_per_seq * block_size) return KVRO_ERR_INVALID_ARG;
   if (layer_begin < 0 || layer_end > layers || layer_begin > layer_end) return KVRO_ERR_INVALID_ARG;
-  if (n_threads < 1) return KVRO_ERR_INVALID_ARG;
+  if (n_threads < 1 || (seg_flags & ~KVRO_SEG_PRE_ROPE)) return KVRO_ERR_INVALID_ARG;
 
   const int esz = (dtype == KVRO_BF16) ? 2 : 1;
   const int32_t* table_row = block_table + (int64_t)dst_seq * max_blocks_per_seq;
@@ -245,6 +251,8 @@ static int splice_core(
         /* step 1: the position shift of this token */
         int64_t delta = pos_map ? (int64_t)pos_map[t] - ((int64_t)old_start + t)
                                 : (int64_t)new_start - (int64_t)old_start;
+        if (seg_flags & KVRO_SEG_PRE_ROPE) /* reading R24: every source token sits at old_start, token t goes to target_t */
+          delta = (pos_map ? (int64_t)pos_map[t] : (int64_t)new_start + t) - (int64_t)old_start;
         /* step 7: the slot */
         int64_t j = (int64_t)dst_token_start + t;
         int64_t blk = table_row[j / block_size];
@@ -322,7 +330,7 @@ int kvr_oracle_reposition_splice(
                      stride_layer, stride_block, stride_token, stride_head, num_blocks, block_size, block_table,
                      num_seqs, max_blocks_per_seq, k_scale_dst, k_src, v_src, src_stride_layer, src_stride_head,
                      src_stride_token, len, old_start, new_start, dst_seq, dst_token_start, pos_map, k_scale_src,
-                     layer_begin, layer_end, n_threads);
+                     0, layer_begin, layer_end, n_threads);
 }
 
 /*
@@ -343,13 +351,13 @@ int kvr_oracle_reposition_splice_ex(
     const void* k_src, const void* v_src,
     int64_t src_stride_layer, int64_t src_stride_head, int64_t src_stride_token,
     int len, int old_start, int new_start, int dst_seq, int dst_token_start,
-    const int32_t* pos_map, const float* k_scale_src,
+    const int32_t* pos_map, const float* k_scale_src, int seg_flags,
     int layer_begin, int layer_end, int n_threads) {
   return splice_core(layers, kv_heads, head_dim, rotary_dim, rotary_offset, pairing, dtype, inv_freq, k_cache,
                      v_cache, stride_layer, stride_block, stride_token, stride_head, num_blocks, block_size,
                      block_table, num_seqs, max_blocks_per_seq, k_scale_dst, k_src, v_src, src_stride_layer,
                      src_stride_head, src_stride_token, len, old_start, new_start, dst_seq, dst_token_start,
-                     pos_map, k_scale_src, layer_begin, layer_end, n_threads);
+                     pos_map, k_scale_src, seg_flags, layer_begin, layer_end, n_threads);
 }
 
 /* ------------------------------------------------- in-place reposition (NEXT-1) */

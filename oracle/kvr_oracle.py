@@ -17,6 +17,7 @@ from . import build as _build
 BF16, FP8_E4M3 = 0, 1
 NEOX_HALF, GPTJ_INTERLEAVED = 0, 1
 OK, ERR_INVALID_ARG, ERR_OUT_OF_RANGE = 0, -1, -4
+SEG_PRE_ROPE = 1
 
 _lib = None
 
@@ -51,7 +52,7 @@ def lib():
             [C.c_void_p, C.c_void_p] + [C.c_int64] * 4 + [C.c_int, C.c_int] +
             [C.c_void_p, C.c_int, C.c_int, C.c_void_p] +
             [C.c_void_p, C.c_void_p] + [C.c_int64] * 3 + [C.c_int] * 5 +
-            [C.c_void_p, C.c_void_p] +
+            [C.c_void_p, C.c_void_p, C.c_int] +                   # pos_map, k_scale_src, seg_flags
             [C.c_int] * 3)
         _lib.kvr_oracle_reposition_inplace_ex.restype = C.c_int
         _lib.kvr_oracle_reposition_inplace_ex.argtypes = (
@@ -135,7 +136,7 @@ def reposition_splice(*, layers, kv_heads, head_dim, rotary_dim, pairing, dtype,
                       k_src, v_src, src_stride_layer, src_stride_head, src_stride_token,
                       len, old_start, new_start, dst_seq, dst_token_start,
                       pos_map=None, k_scale_src=None,
-                      layer_begin=0, layer_end=None, n_threads=1, rotary_offset=0):
+                      layer_begin=0, layer_end=None, n_threads=1, rotary_offset=0, pre_rope=False):
     """Splices ONE segment into (k_cache, v_cache) in place.  Returns the status code.
     rotary_offset != 0 or v_cache is None / v_src is None (a [latent | k_pe] cache, reading R23) go through
     kvr_oracle_reposition_splice_ex."""
@@ -146,7 +147,7 @@ def reposition_splice(*, layers, kv_heads, head_dim, rotary_dim, pairing, dtype,
     num_seqs, max_blocks = block_table.shape
     if layer_end is None:
         layer_end = layers
-    if rotary_offset != 0 or v_cache is None or v_src is None:
+    if rotary_offset != 0 or v_cache is None or v_src is None or pre_rope:
         return lib().kvr_oracle_reposition_splice_ex(
             layers, kv_heads, head_dim, rotary_dim, rotary_offset, pairing, dtype, _ptr(inv_freq),
             _ptr(k_cache, edt, True), _ptr(v_cache, edt, True),
@@ -154,7 +155,7 @@ def reposition_splice(*, layers, kv_heads, head_dim, rotary_dim, pairing, dtype,
             _ptr(block_table, np.int32), num_seqs, max_blocks, _ptr(k_scale_dst, np.float32),
             _ptr(k_src, edt), _ptr(v_src, edt), src_stride_layer, src_stride_head, src_stride_token,
             len, old_start, new_start, dst_seq, dst_token_start,
-            _ptr(pos_map, np.int32), _ptr(k_scale_src, np.float32),
+            _ptr(pos_map, np.int32), _ptr(k_scale_src, np.float32), SEG_PRE_ROPE if pre_rope else 0,
             layer_begin, layer_end, n_threads)
     return lib().kvr_oracle_reposition_splice(
         layers, kv_heads, head_dim, rotary_dim, pairing, dtype, _ptr(inv_freq),
@@ -231,7 +232,7 @@ def splice_workload(w, srcs, k_cache, v_cache, n_threads=1, layer_begin=0, layer
             len=seg.len, old_start=seg.old_start, new_start=seg.new_start, dst_seq=seg.dst_seq,
             dst_token_start=seg.dst_token_start, pos_map=seg.pos_map, k_scale_src=w.k_scale_src,
             layer_begin=layer_begin, layer_end=layer_end, n_threads=n_threads,
-            rotary_offset=getattr(w, "rotary_offset", 0))
+            rotary_offset=getattr(w, "rotary_offset", 0), pre_rope=getattr(seg, "pre_rope", False))
         if status != OK:
             raise RuntimeError(f"oracle: segment {i} -> status {status}")
 

@@ -74,6 +74,7 @@ kvr_status check_call(const kvr_model_desc* m, const kvr_paged_dst* d, const kvr
     for (int64_t x : ss)
       if ((x * E) % 16 != 0) return KVR_ERR_ALIGNMENT;
     if (s.pos_map && (reinterpret_cast<uintptr_t>(s.pos_map) & 3u)) return KVR_ERR_ALIGNMENT;
+    if (s.flags & ~KVR_SEG_PRE_ROPE) return KVR_ERR_INVALID_ARG;
   }
   return KVR_OK;
 }
@@ -283,7 +284,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
 
   bool any_map = false, scales_differ = false;
   for (int32_t i = 0; i < n; ++i) {
-    any_map |= segs[i].pos_map != nullptr;
+    any_map |= segs[i].pos_map != nullptr || (segs[i].flags & KVR_SEG_PRE_ROPE);   // per-token shifts
     scales_differ |= (m.dtype == KVR_FP8_E4M3 && segs[i].k_scale_src && segs[i].k_scale_src != d->k_scale);
   }
   P.any_pos_map = any_map; P.scales_differ = scales_differ;
@@ -314,7 +315,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       o.dst_seq = s.dst_seq; o.dst_token_start = s.dst_token_start;
       o.first_q = s.dst_token_start / cg;
       o.n_chunks = (int32_t)(((int64_t)s.dst_token_start + s.len - 1) / cg - o.first_q + 1);
-      o.index = i; o.pad_ = 0;
+      o.index = i; o.pre_rope = (s.flags & KVR_SEG_PRE_ROPE) ? 1 : 0;
       chunks_total += o.n_chunks;
     }
     int lpu = lpu_request;

@@ -31,7 +31,7 @@ struct SegDev {
   int32_t first_q;             // dst_token_start / cg
   int32_t n_chunks;            // chunks of <= cg tokens, aligned to cg in destination token space
   int32_t index;               // position in the caller's array (for the status word)
-  int32_t pad_;
+  int32_t pre_rope;            // KVR_SEG_PRE_ROPE: every source token sits at old_start (kvr.h)
 };
 
 constexpr int kInlineSegs = 8;    // calls with <= this many segments carry their descriptors in the kernel parameters
@@ -98,6 +98,12 @@ __device__ __forceinline__ Chunk chunk_of(const SegDev& s, int32_t c, int32_t cg
   ch.blk_index = (int32_t)(lo / block_size);
   ch.off = (int32_t)(lo % block_size);
   return ch;
+}
+
+// Position shift of token i of a segment (kvr.h): new position minus old position.
+__device__ __forceinline__ long long token_delta(const SegDev& s, int i) {
+  if (s.pre_rope) return (s.pos_map ? (long long)s.pos_map[i] : (long long)s.old_start + s.delta + i) - (long long)s.old_start;
+  return s.pos_map ? (long long)s.pos_map[i] - ((long long)s.old_start + i) : (long long)s.delta;
 }
 
 __device__ __forceinline__ void report_bad_block(int32_t* status, int32_t seg_index, int32_t token) {

@@ -34,8 +34,7 @@ __global__ void __launch_bounds__(256) kvr_generic_kernel(const __grid_constant_
     __syncthreads();  // previous unit's table no longer in use
     for (int idx = threadIdx.x; idx < ch.n_tok * half; idx += blockDim.x) {
       int t = idx / half, i = idx % half;
-      int64_t delta = s.pos_map ? (int64_t)s.pos_map[ch.t0 + t] - ((int64_t)s.old_start + ch.t0 + t)
-                                : (int64_t)s.delta;
+      int64_t delta = token_delta(s, ch.t0 + t);
       tab[t * half + i] = angle_entry(delta, P.inv_freq[i]);
       if (i == 0) is_copy[t] = (delta == 0);
     }

@@ -345,7 +345,10 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
           continue;
         }
         // ---- angle table (step a1) ----
-        const int64_t key = MAP ? (base + j) : (int64_t)si;
+        // per-token shifts (position map, pre-RoPE keys): a table per unit; a constant shift: a table per segment,
+        // also inside a call that has per-token segments elsewhere (its per-token words then all name row 0)
+        const bool per_token = MAP && (sg.pos_map != nullptr || sg.pre_rope != 0);
+        const int64_t key = per_token ? ((base + j) | (1ll << 62)) : (int64_t)si;
         if (key != cur_key) {
           const int nb = tb ^ 1;
           // Buffer nb was last read by the tiles up to lu_i[nb].  Consumer warps take their stages in order, so once
@@ -360,13 +363,16 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
           }
           __syncwarp();
           float4* tab = reinterpret_cast<float4*>(smem + RP.off_tab + nb * RP.tab_stride);
-          if (MAP) {
+          if (MAP && !per_token) {
+            for (int p = lane; p < RP.half_R; p += 32)
+              tab[tab_pos<G::PPV>(p, RP.NV)] = angle_entry((int64_t)sg.delta, P.inv_freq[p]);
+            if (lane < RP.cg) reinterpret_cast<int32_t*>(tab + RP.cg * RP.half_R)[lane] = (sg.delta == 0) ? -1 : 0;
+          } else if (MAP) {
             // Per-token shifts, deduplicated into RUNS of equal Delta (a position map is contiguous except at its
             // gaps, so a chunk of <= 32 tokens holds a handful of distinct shifts): one table row per run, and a
             // per-token word that names the token's row (-1: Delta_t == 0, the row is a byte copy).
             long long d = 0;
-            if (lane < n_tok)
-              d = sg.pos_map ? (long long)sg.pos_map[t0 + lane] - ((long long)sg.old_start + t0 + lane) : (long long)sg.delta;
+            if (lane < n_tok) d = token_delta(sg, t0 + lane);
             const long long dprev = __shfl_up_sync(FULL, d, 1);
             const unsigned heads_mask = __ballot_sync(FULL, lane < n_tok && (lane == 0 || d != dprev));
             const int n_runs = __popc(heads_mask);

@@ -43,7 +43,8 @@ class DeviceWorkload:
             self.k_cache, self.v_cache = _make_pool(w, self.device)
         self.segs = kvr.segment_array([
             kvr.segment(k, v, w.src_strides(s), s.len, s.old_start, s.new_start, s.dst_seq, s.dst_token_start,
-                        pos_map=pm, k_scale_src=self.k_scale_src)
+                        pos_map=pm, k_scale_src=self.k_scale_src,
+                        flags=kvr.KVR_SEG_PRE_ROPE if getattr(s, "pre_rope", False) else 0)
             for s, (k, v), pm in zip(w.segments, self.sources, self.pos_maps)])
         self.dst = self.dst_for(self.k_cache, self.v_cache) if make_pool else None
 
@@ -94,7 +95,8 @@ class DeviceWorkload:
         self.host_k_scale_src = None if self.k_scale_src is None else self.k_scale_src.cpu().pin_memory()
         self.host_segs = kvr.segment_array([
             kvr.segment(k, v, w.src_strides(s), s.len, s.old_start, s.new_start, s.dst_seq, s.dst_token_start,
-                        pos_map=pm, k_scale_src=self.host_k_scale_src)
+                        pos_map=pm, k_scale_src=self.host_k_scale_src,
+                        flags=kvr.KVR_SEG_PRE_ROPE if getattr(s, "pre_rope", False) else 0)
             for s, (k, v), pm in zip(w.segments, self.host_sources, self.host_pos_maps)])
         return self.host_segs
 

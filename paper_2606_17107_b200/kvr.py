@@ -15,6 +15,7 @@ KVR_OK, KVR_ERR_INVALID_ARG, KVR_ERR_UNSUPPORTED, KVR_ERR_ALIGNMENT = 0, -1, -2,
 KVR_ERR_OUT_OF_RANGE, KVR_ERR_CUDA, KVR_ERR_NOMEM = -4, -5, -6
 KVR_BF16, KVR_FP8_E4M3 = 0, 1
 KVR_PAIR_NEOX_HALF, KVR_PAIR_GPTJ_INTERLEAVED = 0, 1
+KVR_SEG_PRE_ROPE = 1
 PATH_AUTO, PATH_GENERIC, PATH_RING = 0, 1, 2
 
 
@@ -40,7 +41,7 @@ class kvr_segment(C.Structure):
                 ("src_stride_layer", C.c_int64), ("src_stride_head", C.c_int64),
                 ("src_stride_token", C.c_int64),
                 ("len", C.c_int32), ("old_start", C.c_int32), ("new_start", C.c_int32),
-                ("dst_seq", C.c_int32), ("dst_token_start", C.c_int32),
+                ("dst_seq", C.c_int32), ("dst_token_start", C.c_int32), ("flags", C.c_int32),
                 ("pos_map", C.c_void_p), ("k_scale_src", C.c_void_p)]
 
 
@@ -149,10 +150,10 @@ def paged_dst(k_cache, v_cache, strides, num_blocks, block_size, block_table, nu
 
 
 def segment(k_src, v_src, src_strides, len, old_start, new_start, dst_seq, dst_token_start, pos_map=None,
-            k_scale_src=None):
+            k_scale_src=None, flags=0):
     sl, sh, st = src_strides
     return kvr_segment(_ptr(k_src), _ptr(v_src), sl, sh, st, len, old_start, new_start, dst_seq,
-                       dst_token_start, _ptr(pos_map), _ptr(k_scale_src))
+                       dst_token_start, flags, _ptr(pos_map), _ptr(k_scale_src))
 
 
 def resident_span(seq, token_start, len, old_start, new_start, pos_map=None):

@@ -46,7 +46,7 @@ def _call(kvr, **over):
                       over.get("max_blocks", 8), k_scale=over.get("k_scale"))
     s = kvr.segment(over.get("k_src", base * 4), over.get("v_src", base * 5), over.get("src_strides", (2 * 10 * 64, 10 * 64, 64)),
                     over.get("len", 10), 0, over.get("new_start", 7), over.get("dst_seq", 0),
-                    over.get("dst_token_start", 3))
+                    over.get("dst_token_start", 3), flags=over.get("flags", 0))
     return kvr.kvr_validate(m, d, [s]), keep
 
 
@@ -75,6 +75,9 @@ def test_validation(kvr):
     assert _call(kvr, v_cache=None, v_src=None)[0] == kvr.KVR_OK
     assert _call(kvr, v_cache=None)[0] == kvr.KVR_ERR_INVALID_ARG
     assert _call(kvr, v_src=None)[0] == kvr.KVR_ERR_INVALID_ARG
+    # NEXT-4: segment flags (the field sits in former padding: the struct size asserted above is unchanged)
+    assert _call(kvr, flags=kvr.KVR_SEG_PRE_ROPE)[0] == kvr.KVR_OK
+    assert _call(kvr, flags=2)[0] == kvr.KVR_ERR_INVALID_ARG
 
 
 def test_bytes_moved_is_linear(kvr):

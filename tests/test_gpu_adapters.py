@@ -130,7 +130,7 @@ def test_mla_host_sources_and_write_span():
 
 
 @pytest.mark.parametrize("name,layers", [("mla-dsv2-lite", [0, 26]), ("image-kv-qwen25vl-7b", [0, 27]),
-                                         ("image-kv-qwen3vl-8b", [35])])
+                                         ("image-kv-qwen3vl-8b", [35]), ("compose-qwen3-8b", [17])])
 def test_adapter_full_size_sampled_layers(name, layers):
     """The launch configuration bench.py times (full-size workload, auto dispatch); the oracle checks sampled layers."""
     from paper_2606_17107_b200 import kvr
@@ -158,3 +158,25 @@ def test_adapter_full_size_sampled_layers(name, layers):
         assert k_distance(w, gk, kc).max() <= K_TOL[w.dtype], (name, l)
         if vc is not None:
             assert np.array_equal(bits_to_numpy(dw.v_cache[l * s_l:(l + 1) * s_l]), vc), (name, l, "V")
+
+
+# ------------------------------------------------------------------ NEXT-4: skills + seam token + fresh suffix in ONE call
+def _compose(dtype="bf16", layout="NHD", pairing="neox", with_map=False, D=128, heads=4):
+    """Two sequences; each gets a precompiled skill, and then -- in the same call -- a repaired seam token (Delta = 0
+    row) and/or the freshly projected suffix keys (KVR_SEG_PRE_ROPE), optionally at mapped positions with gaps."""
+    pm = (3000 + np.cumsum(np.r_[0, 1 + (np.arange(76) % 7 == 0) * 5])).astype(np.int32) if with_map else None
+    return make_workload(
+        name="compose", layers=3, kv_heads=heads, head_dim=D, pairing=pairing, dtype=dtype, theta=1e6, block_size=16,
+        layout=layout, seed=61, slack=1.5,
+        seq_segments=[[dict(len=300, dst_token_start=20, new_start=20),                                # skill
+                       dict(len=1, dst_token_start=320, new_start=0),                                  # seam row, Delta = 0
+                       dict(len=77, dst_token_start=321, new_start=321, pre_rope=True, pos_map=pm)],   # suffix
+                      [dict(len=130, dst_token_start=5, new_start=161),
+                       dict(len=40, dst_token_start=135, new_start=135, pre_rope=True)]])
+
+
+@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("dtype,layout,pairing,with_map,heads", [("bf16", "NHD", "neox", False, 4), ("bf16", "HND", "gptj", True, 8),
+                                                              ("fp8", "NHD", "neox", True, 8), ("bf16", "NHD", "neox", True, 2)])
+def test_compose_skill_seam_and_fresh_suffix_in_one_call(dtype, layout, pairing, with_map, heads, path):
+    check_parity(_compose(dtype, layout, pairing, with_map, heads=heads), path)

@@ -204,3 +204,48 @@ def test_k_only_bytes_and_arg_rules():
     assert orc.reposition_splice(**common, v_cache=None, v_src=None, rotary_offset=32) == orc.OK
     assert orc.reposition_splice(**common, v_cache=kc.copy(), v_src=None, rotary_offset=32) != orc.OK   # all-or-none
     assert orc.reposition_splice(**common, v_cache=None, v_src=None, rotary_offset=40) != orc.OK       # window past row
+
+
+# ------------------------------------------------------------------ NEXT-4: fresh suffix keys (pre-RoPE) in the same call (R24)
+@pytest.mark.parametrize("with_map", [False, True])
+@pytest.mark.parametrize("pairing", ["neox", "gptj"])
+def test_pre_rope_segment_is_rope_at_the_target_positions(pairing, with_map):
+    """A KVR_SEG_PRE_ROPE segment holds keys that are not position-encoded yet; the splice must leave, in the slots,
+    exactly RoPE(k, target_t) -- the textbook formula in numpy, rounded once (exact rational rounding) -- with
+    target_t = new_start + t or pos_map[t].  A plain segment in the same workload keeps its ordinary meaning."""
+    D, R = 32, 16
+    pm = np.array([700, 701, 705, 706, 900, 901, 902], dtype=np.int32) if with_map else None
+    w = make_workload(name="pre", layers=2, kv_heads=2, head_dim=D, rotary_dim=R, pairing=pairing, theta=1e4,
+                      block_size=4, seed=51,
+                      seq_segments=[[dict(len=9, dst_token_start=2, new_start=161),                       # a skill
+                                     dict(len=7, dst_token_start=11, new_start=170, pre_rope=True, pos_map=pm)]])
+    srcs, kc, vc = materialize_cpu(w)
+    run_oracle(w, srcs, kc, vc)
+    for (si, l, h, t), o in brute_force_offsets(w).items():
+        seg, src = w.segments[si], srcs[si][0][l, h, t, :D]
+        x = src.view(ml_dtypes.bfloat16).astype(np.float64)[None, :]
+        if seg.pre_rope:
+            target = int(pm[t]) if with_map else seg.new_start + t
+            y = rope_direct_np(x, [target], w.inv_freq, R, pairing)[0]              # RoPE of the raw key at its position
+        else:
+            y = rope_direct_np(x, [seg.new_start - seg.old_start], w.inv_freq, R, pairing)[0]
+        exp = np.array([bf16_exact(float(v)) for v in y], dtype=np.uint16)
+        exp[R:] = src[R:]
+        assert np.array_equal(kc[o:o + D], exp), (si, l, h, t)
+        assert np.array_equal(vc[o:o + D], srcs[si][1][l, h, t, :D])
+
+
+def test_pre_rope_equals_per_token_map_of_an_ordinary_segment():
+    """Delta_t = target_t - old_start: the same bytes as an ordinary segment whose position map is target_t + t
+    (old_start = 0), i.e. the flag is only a convenience over the per-token map."""
+    w1 = make_workload(name="a", layers=1, kv_heads=2, head_dim=32, theta=1e4, block_size=4, seed=52,
+                       seq_segments=[[dict(len=10, dst_token_start=3, new_start=40, pre_rope=True)]])
+    w2 = make_workload(name="a", layers=1, kv_heads=2, head_dim=32, theta=1e4, block_size=4, seed=52,
+                       seq_segments=[[dict(len=10, dst_token_start=3, new_start=40,
+                                           pos_map=(40 + 2 * np.arange(10)).astype(np.int32))]])
+    s1, k1, v1 = materialize_cpu(w1)
+    s2, k2, v2 = materialize_cpu(w2)
+    assert np.array_equal(s1[0][0], s2[0][0])
+    run_oracle(w1, s1, k1, v1)
+    run_oracle(w2, s2, k2, v2)
+    assert np.array_equal(k1, k2) and np.array_equal(v1, v2)

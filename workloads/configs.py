@@ -89,6 +89,7 @@ class SegmentSpec:
     dst_token_start: int
     pos_map: Optional[np.ndarray] = None   # int32 [len]: new position of token t
     src_row_pad: int = 0                   # extra elements after each source token row (stride tests)
+    pre_rope: bool = False                 # keys not yet position-encoded (fresh suffix keys): all tokens at old_start
 
 
 @dataclass
@@ -230,7 +231,7 @@ def make_workload(*, name, layers, kv_heads, head_dim, rotary_dim=None, pairing=
             segs.append(SegmentSpec(len=d["len"], old_start=d.get("old_start", 0),
                                     new_start=d.get("new_start", d["dst_token_start"]), dst_seq=q,
                                     dst_token_start=d["dst_token_start"], pos_map=d.get("pos_map"),
-                                    src_row_pad=d.get("src_row_pad", 0)))
+                                    src_row_pad=d.get("src_row_pad", 0), pre_rope=d.get("pre_rope", False)))
     if num_blocks is None:
         num_blocks = int(np.ceil(slack * sum(rows)))
     table = _table_rows(num_blocks, rows, seed + 3000, prefix)
@@ -326,7 +327,7 @@ def config_small(c: int, layout: str = "NHD") -> Workload:
 
 # ------------------------------------------------------------- NEXT-3 / NEXT-4 adapter workloads
 
-ADAPTERS = ("mla-dsv2-lite", "image-kv-qwen25vl-7b", "image-kv-qwen3vl-8b")
+ADAPTERS = ("mla-dsv2-lite", "image-kv-qwen25vl-7b", "image-kv-qwen3vl-8b", "compose-qwen3-8b")
 
 
 def adapter_config(name: str, layout: str = "NHD", layers: Optional[int] = None, shrink: int = 1) -> Workload:
@@ -341,6 +342,10 @@ def adapter_config(name: str, layout: str = "NHD", layers: Optional[int] = None,
                            into 32 sequences; only the 16 temporal pairs rotate.
     image-kv-qwen3vl-8b   Qwen3-VL-8B-shaped: 36 layers, 8 kv heads, D 128, INTERLEAVED M-RoPE (24, 20, 20), theta 5e6;
                           same 32 images.
+    compose-qwen3-8b      NEXT-4, one call per composed context ("a re-rotation pass plus the suffix"),
+                          configs[1]'s shape: 16 requests, each = a 4096-token precompiled skill moved to 2000, one
+                          repaired seam token (Delta = 0 row) and a 512-token task suffix whose freshly
+                          projected keys are not position-encoded yet (pre_rope: RoPE applied on the way in).
     """
     seed = S0 + 100 + ADAPTERS.index(name)
     if name == "mla-dsv2-lite":
@@ -362,6 +367,14 @@ def adapter_config(name: str, layout: str = "NHD", layers: Optional[int] = None,
             seqs.append([dict(len=n_tok, dst_token_start=at, old_start=at, new_start=at + 161)])
         return make_workload(name=name, layers=layers or (36 if q3 else 28), kv_heads=8 if q3 else 4, head_dim=128,
                              inv_freq=inv, block_size=16, layout=layout, seed=seed, seq_segments=seqs)
+    if name == "compose-qwen3-8b":
+        n_req = 16 if shrink == 1 else max(2, 16 // shrink)
+        n, suf = 4096 // shrink, 512 // shrink
+        seqs = [[dict(len=n, dst_token_start=2000, new_start=2000),
+                 dict(len=1, dst_token_start=2000 + n, new_start=0),
+                 dict(len=suf, dst_token_start=2001 + n, new_start=2001 + n, pre_rope=True)] for _ in range(n_req)]
+        return make_workload(name=name, layers=layers or 36, kv_heads=8, head_dim=128, theta=1e6, block_size=16,
+                             layout=layout, seed=seed, seq_segments=seqs)
     raise ValueError(name)
 
 
