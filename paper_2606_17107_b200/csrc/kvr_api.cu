@@ -372,7 +372,6 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       int64_t tile_target = tu.tile_bytes > 0 ? tu.tile_bytes : 16384;             // K bytes of a gather tile
       // (mode 2 is never chosen automatically: on B200 it measured +1.5 % on configs[1] and -1 % on configs[2] for 8 heads
       //  of 128 bf16, -12 % in fp8: a V-only stage has no arithmetic to hide its row stores behind.)
-      (void)chunk_bytes;
       if (tu.gather == 3) { mode = 2; if (tu.tile_bytes <= 0) tile_target = 32768; }
       int64_t lim = tile_target / (m.kv_heads * rowB);
       const int cg_g = chunk_granularity(d->block_size, (int)(lim > 16 ? 16 : lim));
@@ -384,6 +383,12 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
         P.gather = (mode == 2 && d->v_cache) ? 2 : 1;
         cg_limit = cg_g;
         P.tile_min_bytes = (int32_t)(m.kv_heads * cg_g * rowB);
+        // forced, with a tile smaller than all heads of a full chunk: keep the full chunk and take a SUBSET of the heads
+        // per tile (a token then leaves as heads/hpt contiguous pieces instead of one)
+        if (tu.tile_bytes > 0 && tu.tile_bytes >= cg_full * rowB && tu.tile_bytes < chunk_bytes) {
+          cg_limit = cg_full;
+          P.tile_min_bytes = tu.tile_bytes;
+        }
       }
     }
     if (inplace && d->stride_token != m.head_dim) {

@@ -42,6 +42,7 @@ struct RingParams {
                                           // rest of the row is moved by a plain 16-byte copy loop
   int nv_slot;                            // vectors the lane slots are laid over: nv, or nr in window mode
   int ro_v;                               // rotary_offset in 16-byte vectors
+  int log_rpi;                            // log2(rows per warp pass)
   int gather;                             // GATHER mode (see wpg)
   int split;                              // gather tiles hold K or V alone (all heads of a FULL chunk of one tensor)
   int wpg;                                // GATHER mode (dense token-major pools): a tile holds ALL heads of a few tokens and
@@ -603,6 +604,18 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       // warps that share the stage takes a contiguous range of them.
       const int items = ((n_tok + rpi - 1) / rpi) * RP.hpt, ipw = (items + wpg - 1) / wpg;
       const int it0 = wsub * ipw, it1 = min(items, it0 + ipw);
+      if (RP.v_bulk == 0) {
+        // 16-byte warp copies, same item order (short rows -- fp8 -- make poor bulk stores)
+        const int per_item = rpi * nv, total = (it1 - it0) * per_item;
+#pragma unroll 4
+        for (int idx = lane; idx < total; idx += 32) {
+          const int it = it0 + idx / per_item, rem = idx % per_item;
+          const int tg = it / RP.hpt, hh = it - tg * RP.hpt, tt = tg * rpi + (rem >> RP.log_nv), v = rem & (nv - 1);
+          if (tt < n_tok)
+            stg128(P.v_cache + (m.dst_off + (int64_t)tt * P.d_st + (int64_t)hh * P.d_sh) * E + v * 16,
+                   lds128(sv + (hh * RP.cg + tt) * RP.rowB + v * 16));
+        }
+      } else
       for (int idx = lane; idx < (it1 - it0) * rpi; idx += 32) {
         const int it = it0 + idx / rpi, r = idx - (idx / rpi) * rpi;
         const int tg = it / RP.hpt, hh = it - tg * RP.hpt, tt = tg * rpi + r;
@@ -657,15 +670,22 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       // split gather tile holding V alone: nothing to rotate
     } else if (RP.gather) {
       // gather mode: tokens outer, heads inner -- a pass of this warp completes rpi whole token rows
-      const int items = ((n_tok + rpi - 1) / rpi) * RP.hpt, ipw = (items + wpg - 1) / wpg;
-      const int it1 = min(items, (wsub + 1) * ipw);
-      for (int it = wsub * ipw; it < it1; ++it) {
-        const int tg = it / RP.hpt, hh = it - tg * RP.hpt, t = tg * rpi + rsub;
-        float s_src, inv_dst; bool requant;
-        head_scales(m, hh, s_src, inv_dst, requant);
-        if (t < n_tok)
-          k_row(m, tab, rotate, sk + hh * sm_sh, P.k_cache + (m.dst_off + (int64_t)hh * P.d_sh) * E, t, sm_st,
-                s_src, inv_dst, requant);
+      // (token group, head) items of this warp, token group major; the walk keeps running pointers (no divisions)
+      const int items = ((n_tok + rpi - 1) >> RP.log_rpi) * RP.hpt;
+      const int ipw = (wpg == 1) ? items : (items + wpg - 1) / wpg;
+      const int it0 = wsub * ipw, it1 = min(items, it0 + ipw);
+      int tg = (wpg == 1) ? 0 : it0 / RP.hpt, hh = it0 - tg * RP.hpt;
+      uint8_t* const kd0 = P.k_cache + m.dst_off * E;
+      const int64_t kd_step = P.d_sh * E;
+      uint32_t ks = sk + hh * sm_sh;
+      uint8_t* kd = kd0 + hh * kd_step;
+      int t = (tg << RP.log_rpi) + rsub;
+      for (int it = it0; it < it1; ++it) {
+        float s_src = 1.0f, inv_dst = 1.0f; bool requant = false;
+        if (DTYPE == 1) head_scales(m, hh, s_src, inv_dst, requant);
+        if (t < n_tok) k_row(m, tab, rotate, ks, kd, t, sm_st, s_src, inv_dst, requant);
+        ++hh; ks += sm_sh; kd += kd_step;
+        if (hh == RP.hpt) { hh = 0; ks = sk; kd = kd0; t += rpi; }
       }
     } else
     for (int hh = 0; hh < RP.hpt; ++hh) {
@@ -687,13 +707,13 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         }
       }
     }
-    if (RP.v_bulk == 2 || (RP.gather && !RP.no_v) || (RP.v_bulk && lane == 0)) bulk_wait_read0();   // V bytes have left shared memory
+    if (RP.v_bulk == 2 || (RP.v_bulk && lane == 0)) bulk_wait_read0();   // V bytes have left shared memory
     __syncwarp();
     if (lane == 0) mbar_arrive(s_empty + 8u * stage);
     stage += stage_step;
     if (stage >= S) { stage -= S; phase ^= 1u; }
   }
-  if (RP.v_bulk == 2 || (RP.gather && !RP.no_v) || (RP.v_bulk && lane == 0)) bulk_wait_all0();
+  if (RP.v_bulk == 2 || (RP.v_bulk && lane == 0)) bulk_wait_all0();
   (void)dst_rows_packed;
 }
 
@@ -766,7 +786,7 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   RP.ro_v = P.rotary_offset * E / 16;
   RP.nv = RP.rowB / 16; RP.log_nv = (RP.nv & (RP.nv - 1)) ? -1 : ilog2(RP.nv);
   RP.nv_slot = RP.win ? RP.nr : RP.nv;
-  RP.sp = RP.nv_slot / 2; RP.log_sp = ilog2(RP.sp); RP.rpi = 32 / RP.sp;
+  RP.sp = RP.nv_slot / 2; RP.log_sp = ilog2(RP.sp); RP.rpi = 32 / RP.sp; RP.log_rpi = ilog2(RP.rpi);
   RP.half_R = P.rotary_dim / 2;
   const int ppv = (P.pairing == 0) ? 16 / E : 8 / E;
   RP.NV = RP.half_R / ppv;
@@ -833,7 +853,9 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   else if (cfg.v_bulk_store == 3) RP.v_bulk = 2;
   else if (cfg.v_bulk_store == 1) RP.v_bulk = runs ? 1 : 2;
   else RP.v_bulk = runs ? 1 : 0;
-  if (RP.no_v || RP.gather) RP.v_bulk = 0;
+  if (RP.gather)   // gather mode: 2 = one bulk store per (token, head) row (default: measured faster), 0 = warp copies
+    RP.v_bulk = (cfg.v_bulk_store == 2) ? 0 : (cfg.v_bulk_store == 3 || cfg.v_bulk_store == 1) ? 2 : 2;
+  if (RP.no_v) RP.v_bulk = 0;
   int64_t g = (int64_t)sm_count * ctas;
   if (cfg.max_ctas > 0 && g > cfg.max_ctas) g = cfg.max_ctas;
   if (g > P.total_units) g = P.total_units;
