@@ -126,3 +126,26 @@ def test_product_does_not_import_oracle():
                 assert "kvr_oracle" not in text, f
     orc = open(os.path.join(ROOT, "oracle", "kvr_oracle.c")).read() + open(os.path.join(ROOT, "oracle", "kvr_oracle.py")).read()
     assert "kvr.h" not in orc.replace("include/kvr.h)", "") and "paper_2606_17107_b200 import" not in orc
+
+
+def test_header_is_valid_c99_and_struct_sizes_match_the_binding(kvr, tmp_path):
+    """include/kvr.h is a C header (extern "C" only under C++): it must compile as strict C99 on its own, and the
+    struct sizes the C compiler sees must be the ones the ctypes binding marshals."""
+    import os
+    import shutil
+    import subprocess
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("no gcc")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    src = tmp_path / "abi.c"
+    src.write_text(
+        '#include "kvr.h"\n#include <stdio.h>\n'
+        'int main(void) { printf("%zu %zu %zu %zu %zu %zu\\n", sizeof(kvr_model_desc), sizeof(kvr_paged_dst), '
+        'sizeof(kvr_segment), sizeof(kvr_tuning), sizeof(kvr_resident_span), sizeof(kvr_span)); return 0; }\n')
+    exe = tmp_path / "abi"
+    subprocess.run([gcc, "-std=c99", "-pedantic", "-Wall", "-Werror", "-I", os.path.join(root, "include"),
+                    str(src), "-o", str(exe)], check=True)
+    sizes = [int(x) for x in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()]
+    assert sizes == [C.sizeof(t) for t in (kvr.kvr_model_desc, kvr.kvr_paged_dst, kvr.kvr_segment, kvr.kvr_tuning,
+                                           kvr.kvr_resident_span, kvr.kvr_span)]
