@@ -32,12 +32,15 @@ __global__ void __launch_bounds__(256) kvr_generic_kernel(const __grid_constant_
     const int l0 = lg * P.lpu, l1 = min(P.layers, l0 + P.lpu);
 
     __syncthreads();  // previous unit's table no longer in use
-    for (int idx = threadIdx.x; idx < ch.n_tok * half; idx += blockDim.x) {
+    // per-token shifts (position map, pre-RoPE keys): one table row per token; a constant shift: one row for all
+    const bool per_token = s.pos_map != nullptr || s.pre_rope != 0;
+    const int tab_rows = per_token ? ch.n_tok : 1;
+    for (int idx = threadIdx.x; idx < tab_rows * half; idx += blockDim.x) {
       int t = idx / half, i = idx % half;
       int64_t delta = token_delta(s, ch.t0 + t);
       tab[t * half + i] = angle_entry(delta, P.inv_freq[i]);
-      if (i == 0) is_copy[t] = (delta == 0);
     }
+    for (int t = threadIdx.x; t < ch.n_tok; t += blockDim.x) is_copy[t] = (token_delta(s, ch.t0 + t) == 0);
     const int32_t blk = P.block_table[(int64_t)s.dst_seq * P.max_blocks + ch.blk_index];
     __syncthreads();
     if (blk < 0 || blk >= P.num_blocks) {
@@ -59,7 +62,7 @@ __global__ void __launch_bounds__(256) kvr_generic_kernel(const __grid_constant_
       uint8_t* dst = P.k_cache + ((int64_t)l * P.d_sl + (int64_t)h * P.d_sh + (int64_t)t * P.d_st + dst_base) * E;
       const uint8_t* src = P.inplace ? dst      // each pair is read and written by this one thread: aliasing-safe
                                      : s.k_src + ((int64_t)l * s.sl + (int64_t)h * s.sh + (int64_t)(ch.t0 + t) * s.st) * E;
-      float4 cs = tab[t * half + i];
+      float4 cs = tab[(per_token ? t : 0) * half + i];
       if (DTYPE == 0) {
         uint16_t ua = reinterpret_cast<const uint16_t*>(src)[ia], ub = reinterpret_cast<const uint16_t*>(src)[ib];
         if (!is_copy[t]) {

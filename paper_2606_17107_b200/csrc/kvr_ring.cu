@@ -696,14 +696,17 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       for (int t = rsub; t < n_tok; t += rpi) k_row(m, tab, rotate, ks, kd, t, sm_st, s_src, inv_dst, requant);
       if (RP.win) {
         // window mode: everything outside the rotary window (the MLA latent) is position-free -- 16-byte copies
-        const int npass = nv - nr, total = n_tok * npass;
-        for (int idx = lane; idx < total; idx += 32) {
-          const int t = idx / npass;
-          int v = idx - t * npass;
-          if (v >= RP.ro_v) v += nr;
-          uint4 A = lds128(ks + t * sm_st + v * 16);
-          if (DTYPE == 1 && requant) requant_fp8(A, s_src, inv_dst);
-          stg128(kd + (int64_t)t * P.d_st * E + v * 16, A);
+        const int npass = nv - nr;
+        for (int t = 0; t < n_tok; ++t) {
+          const uint32_t srow = ks + t * sm_st;
+          uint8_t* drow = kd + (int64_t)t * P.d_st * E;
+#pragma unroll 2
+          for (int j = lane; j < npass; j += 32) {
+            const int v = (j >= RP.ro_v) ? j + nr : j;
+            uint4 A = lds128(srow + v * 16);
+            if (DTYPE == 1 && requant) requant_fp8(A, s_src, inv_dst);
+            stg128(drow + v * 16, A);
+          }
         }
       }
     }
