@@ -1,23 +1,27 @@
 // kvr_ring.cu -- the FAST reposition+splice kernel for sm_100a: a persistent, warp-specialised
-// TMA ring.  HBM-bound by construction (no contraction => no tensor cores; DESIGN.md "Kernels").
+// TMA ring.  HBM-bound by construction (no contraction => no tensor cores; DESIGN.md 5).
 //
-//   producer warp   lane 0 walks this CTA's units (segment, chunk of <= cg destination tokens, layer
-//                   group), resolves the block-table entry (step a4), and for every tile
-//                   (layer, head group) of the unit arms an mbarrier with the byte count and issues
-//                   1-D bulk TMA loads  global -> shared  (cp.async.bulk, steps a2/a6-read) of the K
-//                   and V runs into the next ring stage, together with a 32-byte tile descriptor.
-//                   All 32 lanes evaluate the angle table  (fp64 sincos of Delta*inv_freq -> fp32
-//                   hi/lo, step a1)  into a small double-buffered shared table whenever the segment
-//                   (or, with a position map, the chunk) changes.
-//   consumer warps  each owns every NW-th tile: wait on the stage's "full" mbarrier, then
-//                   V: either one bulk TMA store  shared -> global  per destination run (head-major
-//                      pools) or 16-byte warp copies (token-major pools)             (step a6)
-//                   K: 16-byte shared loads, compensated fp32 rotation in registers with the
-//                      segment's cos/sin held in registers, 16-byte global stores to the paged slot
-//                                                                                     (steps a3, a5)
+//   producer warp   draws units (segment, chunk of <= cg destination tokens, layer group) -- the first grab is
+//                   static, the rest come from one global counter -- and decodes 32 of them at a time, lane j
+//                   resolving unit j's segment, chunk geometry and block-table entry (step a4) one grab ahead.
+//                   For every tile of a unit a lane arms the stage's "full" mbarrier with the byte count and
+//                   issues 1-D bulk TMA loads  global -> shared  (cp.async.bulk, steps a2 / a6-read) of the K
+//                   and V runs, together with a 32-byte tile descriptor; up to min(32, S) tiles per pass.
+//                   All 32 lanes evaluate the angle table  (fp64 sincos of Delta*inv_freq -> fp32 hi/lo,
+//                   step a1)  into a double-buffered shared table when the segment changes; with per-token
+//                   shifts (position map, pre-RoPE keys) per unit, deduplicated into runs of equal Delta.
+//   consumer warps  each owns every (NW/wpg)-th stage: wait on its "full" mbarrier, then
+//                   V: one bulk TMA store  shared -> global  per destination run (head-major pools) or per row
+//                      (gather mode), or 16-byte warp copies (token-major pools)                  (step a6)
+//                   K: 16-byte shared loads, compensated fp32 rotation in registers with the segment's
+//                      cos/sin held in registers, 16-byte global stores to the paged slot   (steps a3, a5)
 //                   then release the stage through its "empty" mbarrier.
+//   modes           in place (K rows read from the slot they are written back to), window (rows that are not a
+//                   power of two / rotary window at an offset: the MLA [latent | k_pe] row), gather (dense
+//                   token-major pools: all heads of a chunk per stage, several warps per stage), K-only.
 //
-// Units are drawn by the persistent CTAs (grid = SMs x CTAs/SM) from one global counter (dynamic scheduling).
+// Persistent grid = SMs x CTAs/SM; programmatic dependent launch overlaps a launch's prologue (and its first
+// angle table) with the tail of the previous one.
 #include <cstdio>
 
 #include "kvr_common.cuh"
@@ -524,7 +528,6 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
   float4 T4[DTYPE == 0 ? G::NT : 1];
   float2 T2[DTYPE == 1 ? G::NT : 1];
   int my_gen = -1, my_run = -1;
-  const bool dst_rows_packed = (P.d_st == P.head_dim);
 
   const int wpg = RP.wpg, wsub = warp % wpg, stage_step = NW / wpg;
   int stage = (warp / wpg) % S;
@@ -717,7 +720,6 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     if (stage >= S) { stage -= S; phase ^= 1u; }
   }
   if (RP.v_bulk == 2 || (RP.v_bulk && lane == 0)) bulk_wait_all0();
-  (void)dst_rows_packed;
 }
 
 // ------------------------------------------------------------------------------- host side
