@@ -349,3 +349,24 @@ def test_gather_mode_ragged_blocks(bs, heads, D, dtype):
                                     [dict(len=77, dst_token_start=1, new_start=9)]])
     check_parity(w, "ring", gather=1)
     check_parity(w, "ring", gather=3)
+
+
+@pytest.mark.parametrize("path", ["generic", "ring"])
+def test_thousands_of_tiny_segments(path):
+    """2600 segments in one call: descriptor staging grows past its initial capacity and the ring kernel's producer
+    searches the segments' unit prefix sums in global memory (more than fit its shared-memory copy)."""
+    rng = np.random.default_rng(12)
+    seqs = []
+    for q in range(4):
+        at, lst = 0, []
+        for _ in range(650):
+            at += int(rng.integers(0, 3))
+            n = int(rng.integers(1, 6))
+            lst.append(dict(len=n, dst_token_start=at, new_start=int(rng.integers(0, 50000)),
+                            old_start=int(rng.integers(0, 50000))))
+            at += n
+        seqs.append(lst)
+    w = make_workload(name="tiny-segs", layers=2, kv_heads=2, head_dim=64, theta=1e6, block_size=16, seed=12,
+                      seq_segments=seqs)
+    assert len(w.segments) == 2600
+    check_parity(w, path)
