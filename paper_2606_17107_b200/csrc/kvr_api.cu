@@ -326,8 +326,11 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       // 11 layers per unit) and the tail is short.  With a position map the per-chunk angle table is rebuilt per
       // unit, so a unit holds ~24 tiles there.
       const int tiles_per_layer = ((m.kv_heads / ring_heads_per_tile(P)) / hsplit) * (P.gather == 2 ? 2 : 1);
-      const int want = P.gather ? (any_map ? 6 : 2)      // gather tiles are 32 KB: the same 64 KB / 192 KB per unit
-                                : (any_map ? 24 : 8);
+      // (with pre-RoPE keys every token has its own shift, nothing deduplicates: ~96 tiles per unit.  One value per
+      //  call: giving the constant-shift segments of such a call their own, smaller units measured slower.)
+      bool any_pre = false;
+      for (int32_t i = 0; i < n; ++i) any_pre |= (segs[i].flags & KVR_SEG_PRE_ROPE) != 0;
+      const int want = (any_pre ? 96 : any_map ? 24 : 8) / (P.gather ? 4 : 1);   // gather tiles are 32 KB, ordinary ones 8 KB
       lpu = (want + tiles_per_layer - 1) / tiles_per_layer;
       if (lpu > m.layers) lpu = m.layers;
       // small calls: prefer more, smaller units so that every SM gets one (latency, not bandwidth, is the bound)
