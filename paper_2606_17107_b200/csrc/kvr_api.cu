@@ -396,7 +396,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     }
     if (inplace && d->stride_token != m.head_dim) {
       // token-major pool, in place: a tile is cg tokens x ALL heads (one contiguous run); keep it near 8 KB
-      cg_limit = (int)(8192 / ((int64_t)m.kv_heads * m.head_dim * E));
+      cg_limit = (int)((tu.tile_bytes > 0 ? tu.tile_bytes : 8192) / ((int64_t)m.kv_heads * m.head_dim * E));
       cg_limit = cg_limit < 1 ? 1 : (cg_limit > 16 ? 16 : cg_limit);
     }
     if ((int64_t)m.head_dim * E > 1024) {
