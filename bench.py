@@ -390,8 +390,10 @@ def run_kvr(args):
                        "layout": args.layout,
                        "cache_dtype": CACHE_DTYPE[w.dtype], "tokens": tokens, "segments": len(w.segments),
                        "bytes_per_step": bytes_per_step, "parallelism": f"replicas x{rep.world}",
-                       "l2": f"inputs larger than L2 ({bytes_per_step // 2} B of sources + as many pool bytes "
-                             "per step vs 126 MB L2); no flush",
+                       "l2": (f"inputs larger than L2 ({bytes_per_step // 2} B of sources + as many pool bytes "
+                              "per step vs 126 MB L2); no flush") if bytes_per_step // 2 > 2 * 126e6 else
+                             (f"working set ({bytes_per_step} B per step) does NOT exceed the 126 MB L2 and is not flushed: "
+                              "a latency-bound case, not a bandwidth figure; see 'latency' (8 rotating buffer sets)"),
                        "kernel": {1: "kvr_generic_kernel", 2: "kvr_ring_kernel"}.get(info["path"], "?"),
                        "grid": info["grid"], "block": info["block"], "smem": info["smem"]},
             "gpu_launches": launches,
