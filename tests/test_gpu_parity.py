@@ -370,3 +370,13 @@ def test_thousands_of_tiny_segments(path):
                       seq_segments=seqs)
     assert len(w.segments) == 2600
     check_parity(w, path)
+
+
+@pytest.mark.parametrize("gather", [0, 1, 2])
+def test_k_only_call_on_an_ordinary_row(gather):
+    """v_cache = NULL / v_src = NULL on a power-of-two row (not an MLA window row): gather and plain tiles."""
+    w = make_workload(name="konly", layers=3, kv_heads=4, head_dim=128, theta=1e6, block_size=16, seed=9, has_v=False,
+                      seq_segments=[[dict(len=333, dst_token_start=19, new_start=2000), dict(len=1, dst_token_start=0)],
+                                    [dict(len=77, dst_token_start=1, new_start=9)]])
+    check_parity(w, "ring", gather=gather)
+    check_parity(w, "generic")
