@@ -266,6 +266,8 @@ def latency_probe(w, device, ctx, stream, sets=8, reps=64):
 # --------------------------------------------------------------------------------------- the kvr arm
 def run_kvr(args):
     import torch
+    from paper_2606_17107_b200 import build as _kbuild
+    _kbuild.build()        # no-op when the in-tree library is newer than its sources; never a CPU fallback
     from paper_2606_17107_b200 import kvr
     from paper_2606_17107_b200.harness import DeviceWorkload
     from paper_2606_17107_b200.replicas import Replicas, aggregate_throughput

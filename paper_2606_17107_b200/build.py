@@ -27,10 +27,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     extra = os.environ.get("KVR_NVCC_EXTRA", "").split()     # e.g. -DKVR_WATCHDOG_PRINT -DKVR_WATCHDOG_CYCLES=2000000000ll
+    tmp = f"{LIB}.tmp{os.getpid()}"
     cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
-          [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB + ".tmp"]
+          [os.path.join(CSRC, s) for s in SOURCES] + ["-o", tmp]
     subprocess.run(cmd, check=True)
-    os.replace(LIB + ".tmp", LIB)
+    os.replace(tmp, LIB)        # atomic: concurrent builders (one per rank) each install a complete file
     return LIB
 
 
