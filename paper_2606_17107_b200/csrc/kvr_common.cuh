@@ -120,6 +120,11 @@ __device__ __forceinline__ float4 angle_entry(int64_t delta, double inv_freq) {
   return make_float4(ch, cl, sh, sl);
 }
 
+__device__ __forceinline__ float4 angle_entry_cs(double c, double s) {
+  float ch = (float)c, sh = (float)s;
+  return make_float4(ch, (float)(c - (double)ch), sh, (float)(s - (double)sh));
+}
+
 // ---- compensated rotation (bf16 path) ---------------------------------------------------------
 // ra = a*c - b*s ; rb = b*c + a*s with c = t.x + t.y, s = t.z + t.w.
 __device__ __forceinline__ void rotate_comp(float a, float b, float4 t, float& ra, float& rb) {

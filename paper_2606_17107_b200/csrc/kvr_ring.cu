@@ -372,6 +372,26 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
             for (int p = lane; p < RP.half_R; p += 32)
               tab[tab_pos<G::PPV>(p, RP.NV)] = angle_entry((int64_t)sg.delta, P.inv_freq[p]);
             if (lane < RP.cg) reinterpret_cast<int32_t*>(tab + RP.cg * RP.half_R)[lane] = (sg.delta == 0) ? -1 : 0;
+          } else if (MAP && sg.pre_rope && sg.pos_map == nullptr) {
+            // Pre-RoPE keys at consecutive target positions: Delta_t = Delta_0 + t.  One fp64 sincos per pair for the
+            // first token and one for the step angle inv_freq[p]; the other tokens follow by the fp64 angle-addition
+            // recurrence (c, s) <- (c c1 - s s1, s c1 + c s1): <= 15 steps, error ~2e-15 against sincos of the product,
+            // i.e. at the resolution of the fp32 hi+lo pair the table stores.  ~4x cheaper than a
+            // sincos per (token, pair), which is what bounds a chunk whose every token has its own shift.
+            const long long d0 = token_delta(sg, t0);
+            for (int p = lane; p < RP.half_R; p += 32) {
+              const double f = P.inv_freq[p];
+              double s1, c1, sn, cs;
+              sincos(f, &s1, &c1);
+              sincos((double)d0 * f, &sn, &cs);
+              const int pos = tab_pos<G::PPV>(p, RP.NV);
+              for (int r = 0; r < n_tok; ++r) {
+                tab[r * RP.half_R + pos] = angle_entry_cs(cs, sn);
+                const double c2 = cs * c1 - sn * s1, s2 = sn * c1 + cs * s1;
+                cs = c2; sn = s2;
+              }
+            }
+            if (lane < n_tok) reinterpret_cast<int32_t*>(tab + RP.cg * RP.half_R)[lane] = (d0 + lane == 0) ? -1 : lane;
           } else if (MAP) {
             // Per-token shifts, deduplicated into RUNS of equal Delta (a position map is contiguous except at its
             // gaps, so a chunk of <= 32 tokens holds a handful of distinct shifts): one table row per run, and a
