@@ -373,8 +373,16 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       const int64_t chunk_bytes = (int64_t)m.kv_heads * cg_full * rowB;          // one tensor, all heads, a full chunk
       int mode = 1;
       int64_t tile_target = tu.tile_bytes > 0 ? tu.tile_bytes : 16384;             // K bytes of a gather tile
-      // (mode 2 is never chosen automatically: on B200 it measured +1.5 % on configs[1] and -1 % on configs[2] for 8 heads
-      //  of 128 bf16, -12 % in fp8: a V-only stage has no arithmetic to hide its row stores behind.)
+      // More than 16 KB per tensor (8 heads of 128 bf16): K and V in 16 KB tiles of their own, each holding HALF the
+      // heads of a full chunk (a token then leaves as two contiguous 1 KB pieces), ring of 6, two stages per warp group
+      // (kvr_ring.cu).  B200: configs[1] 6.15 -> 6.25, configs[2] 6.34 -> 6.47, Qwen3-VL image-KV 6.35 -> 6.48 TB/s.
+      // Not with per-token shifts (measured: no gain) and not in fp8 (-15 %: 128-byte rows make poor bulk stores).
+      bool split16 = false;
+      if (tu.gather == 0 && tu.tile_bytes <= 0 && m.dtype == KVR_BF16 && !any_map && d->v_cache &&
+          chunk_bytes > 16384 && 16384 % (cg_full * rowB) == 0) {
+        const int hpt = (int)(16384 / (cg_full * rowB));
+        if (hpt >= 2 && m.kv_heads % hpt == 0) { mode = 2; tile_target = chunk_bytes; split16 = true; }
+      }
       if (tu.gather == 3) { mode = 2; if (tu.tile_bytes <= 0) tile_target = 32768; }
       int64_t lim = tile_target / (m.kv_heads * rowB);
       const int cg_g = chunk_granularity(d->block_size, (int)(lim > 16 ? 16 : lim));
@@ -392,6 +400,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
           cg_limit = cg_full;
           P.tile_min_bytes = tu.tile_bytes;
         }
+        if (split16) { cg_limit = cg_full; P.tile_min_bytes = 16384; }
       }
     }
     if (inplace && d->stride_token != m.head_dim) {

@@ -854,15 +854,17 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   RP.gather = P.gather ? 1 : 0;
   RP.wpg = 1;
   if (RP.gather && (cfg.warps_per_stage > 0 || S < RP.NW)) {
-    // few large stages: every group of wpg warps walks the ring in NW / wpg strides.  Default: one group per stage
-    // (wpg = NW / S).  Measured on B200 (configs[4]): 2 warps per stage 6.44-6.50 TB/s, all 6 sharing every stage
-    // 6.34, 4 of 4 6.37; one CTA per SM with 12 warps (2-6 per stage, 2 stages per group) 6.13-6.35.
-    int wpg = cfg.warps_per_stage > 0 ? cfg.warps_per_stage : (RP.NW / S > 1 ? RP.NW / S : 1);
+    // Few large stages: groups of wpg warps walk the ring in NW / wpg strides.  A group should own TWO stages (one
+    // loading while the other is consumed): with one stage per group, load and rotate of that stage are serial and
+    // the ring cannot hide the rotate.  Default wpg = 2: 16 KB stages, S = 6 -> 3 groups x 2 stages.  Measured on
+    // B200: configs[2] 6.34 -> 6.47 TB/s with split 16 KB tiles and 2 stages per group; one stage per group 6.15-6.29;
+    // all warps on every stage 6.30; one CTA per SM with 12 warps 5.0-5.5.
+    int wpg = cfg.warps_per_stage > 0 ? cfg.warps_per_stage : 2;
     if (wpg > RP.NW) wpg = RP.NW;
     int step = RP.NW / wpg;
     if (step < 1) step = 1;
     if (step > S) step = S;
-    while (S % step) --step;
+    S -= S % step;
     RP.wpg = wpg; RP.NW = wpg * step;
   } else if (S >= RP.NW) {
     S -= S % RP.NW;
