@@ -835,7 +835,8 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   RP.tab_stride = ((tab_rows * RP.half_R * 16 + RP.cg * 4) + 127) & ~127;
   RP.n_scales = P.dtype == 1 ? P.layers * P.heads : 0;
   RP.n_ub = (P.n_segs > kInlineSegs && P.n_segs <= 2048) ? P.n_segs : 0;
-  const int budget = (227 * 1024) / ctas - 1024;          // per-CTA dynamic shared memory (1 KB reserved per CTA)
+  // per-CTA dynamic shared memory: 228 KB per SM, 1 KB reserved per resident CTA, at most 227 KB per CTA
+  const int budget = (ctas == 1) ? 227 * 1024 : (228 * 1024) / ctas - 1024;
   auto layout = [&](int S) {
     int off = 16 * S;
     off = (off + 31) & ~31; RP.off_meta = off; off += 32 * S;
