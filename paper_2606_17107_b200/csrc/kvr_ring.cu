@@ -628,15 +628,15 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       const int items = ((n_tok + rpi - 1) / rpi) * RP.hpt, ipw = (items + wpg - 1) / wpg;
       const int it0 = wsub * ipw, it1 = min(items, it0 + ipw);
       if (RP.v_bulk == 0) {
-        // 16-byte warp copies, whole token rows (hpt heads = hpt * nv vectors, contiguous in the dense pool); the
-        // warps of the stage take tokens round robin.  No divisions: a lane's (head, vector) are shifts of its index.
-        const int row_vecs = RP.hpt * nv, head_stride = RP.cg * RP.rowB;
-        for (int tt = wsub; tt < n_tok; tt += wpg) {
-          const uint32_t srow = sv + tt * RP.rowB;
-          uint8_t* drow = P.v_cache + (m.dst_off + (int64_t)tt * P.d_st) * E;
-#pragma unroll 2
-          for (int j = lane; j < row_vecs; j += 32)
-            stg128(drow + j * 16, lds128(srow + (j >> RP.log_nv) * head_stride + (j & (nv - 1)) * 16));
+        // 16-byte warp copies, same item order (short rows -- fp8 -- make poor bulk stores)
+        const int per_item = rpi * nv, total = (it1 - it0) * per_item;
+#pragma unroll 4
+        for (int idx = lane; idx < total; idx += 32) {
+          const int it = it0 + idx / per_item, rem = idx % per_item;
+          const int tg = it / RP.hpt, hh = it - tg * RP.hpt, tt = tg * rpi + (rem >> RP.log_nv), v = rem & (nv - 1);
+          if (tt < n_tok)
+            stg128(P.v_cache + (m.dst_off + (int64_t)tt * P.d_st + (int64_t)hh * P.d_sh) * E + v * 16,
+                   lds128(sv + (hh * RP.cg + tt) * RP.rowB + v * 16));
         }
       } else
       for (int idx = lane; idx < (it1 - it0) * rpi; idx += 32) {
