@@ -527,23 +527,21 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
   // this lane's slot: two 16-byte vectors (va, vb) of every row it visits (of its rotary window in window mode)
   int va, vb;
   bool rot_a, rot_b;
-  int tpos[G::NT];               // table positions of this lane's pairs (only used if rotary)
   if (PAIRING == 0) {
     const int half = nr >> 1;
     if (q < half) { va = q; vb = q + half; rot_a = rot_b = true; }
     else { va = nr + 2 * (q - half); vb = va + 1; rot_a = rot_b = false; }
-#pragma unroll
-    for (int k = 0; k < G::NT; ++k) tpos[k] = rot_a ? tab_pos<G::PPV>(va * G::EPV + k, RP.NV) : 0;
   } else {
     va = q; vb = q + (nvs >> 1);
     rot_a = va < nr; rot_b = vb < nr;
-#pragma unroll
-    for (int k = 0; k < G::NT; ++k) {
-      const int v = (k < G::PPV) ? va : vb;
-      const bool r = (k < G::PPV) ? rot_a : rot_b;
-      tpos[k] = r ? tab_pos<G::PPV>(v * G::PPV + (k % G::PPV), RP.NV) : 0;
-    }
   }
+  // Table position of this lane's k-th pair (tab_pos of pair va * EPV + k for NeoX, of pair v * PPV + k % PPV for
+  // GPT-J): affine in k, so it is recomputed where the table is read instead of being held in NT registers.
+  const int tp_a = rot_a ? va : 0, tp_b = rot_b ? vb : 0, tp_nv = RP.NV;
+  auto tpos = [&](int k) -> int {
+    if (PAIRING == 0) return rot_a ? tp_a + k * tp_nv : 0;
+    return (k < G::PPV) ? (rot_a ? tp_a + k * tp_nv : 0) : (rot_b ? tp_b + (k - G::PPV) * tp_nv : 0);
+  };
   va += RP.ro_v; vb += RP.ro_v;       // table positions above are relative to the window; addresses are not
   float4 T4[DTYPE == 0 ? G::NT : 1];
   float2 T2[DTYPE == 1 ? G::NT : 1];
@@ -567,7 +565,7 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         const uint32_t trow = tab + run * RP.half_R * 16;
 #pragma unroll
         for (int k = 0; k < G::NT; ++k) {
-          float4 e = lds128f(trow + tpos[k] * 16);
+          float4 e = lds128f(trow + tpos(k) * 16);
           if (DTYPE == 0) T4[k] = e; else T2[k] = make_float2(e.x, e.z);
         }
       }
@@ -682,7 +680,7 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       if (rot_a || rot_b) {
 #pragma unroll
         for (int k = 0; k < G::NT; ++k) {
-          float4 e = lds128f(tab + tpos[k] * 16);
+          float4 e = lds128f(tab + tpos(k) * 16);
           if (DTYPE == 0) T4[k] = e; else T2[k] = make_float2(e.x, e.z);
         }
       }
