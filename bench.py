@@ -2,19 +2,28 @@
 """bench.py -- KV tokens repositioned+spliced per second on B200 (BASELINE.json `metric`).
 
 A "step" is one pass of the whole hot path (SURVEY.md 8(a) a1..a6 = one kvr_reposition_splice call) over one
-BASELINE.json configuration of synthetic seeded input.  Default workload: configs[1] (Qwen3-8B-shaped, bf16,
-one 4096-token skill at new_start = 2000); `--config c` times another one with the same JSON contract.
+BASELINE.json configuration of synthetic seeded input.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c] [--impl kvr|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl kvr|reference] [--config c] [--layout NHD|HND]
 
-* value      whole-job KV tokens/s, inputs resident in HBM, timed with CUDA events on the launching stream,
-             barrier + synchronize on both sides, max over ranks (N > 1: independent replicas, "weak").
-* roofline   algorithmic bytes (4 * layers*kv_heads*head_dim*esz per KV token, DESIGN.md) / measured launch time
+Default (no --config): the HEADLINE is configs[4] (cfg4-long-partial-rotary, 12.9 GB per step, bf16 cache: the largest
+single-GPU configuration at the paper's cache precision; BASELINE.json's metric is not quoted on one configuration),
+token-major (NHD) pool, and the same JSON line carries `per_config`: configs[1..4] x {NHD, HND}, each timed in the
+same run (north_star: ">= 80 % of peak HBM bandwidth on configs 1-4").  `--config c` times that one configuration
+alone (what the ncu captures under profiles/ run).
+
+* value      whole-job KV tokens/s of the headline: EXACTLY K steps, inputs resident in HBM, CUDA events on the
+             launching stream, barrier + synchronize on both sides, max over ranks (N > 1: independent replicas).
+* per_config for every (config, layout): blocks of K steps repeated back to back until >= 0.25 s of device time;
+             median / best / spread over the blocks, GB/s of algorithmic bytes, fraction of the measured peak,
+             NVML clocks sampled during that configuration's timed region.
+* roofline   algorithmic bytes (4 * layers*kv_heads*head_dim*esz per KV token, DESIGN.md 5) / measured launch time
              against MEASURED_PEAKS.json `hbm_gbs` (the measured copy bandwidth of this pool's B200s).
 * e2e        the same metric through kvr_reposition_splice_host: sources in pinned HOST memory, the
              host->device copies and the device->host read of the status word inside the timed region.
 * cpu_baseline  the fp64 oracle (oracle/, as it stands) on this box's host cores over a bounded sample.
 * --impl reference  times the oracle alone (rank 0 only), same metric/config, JSON line with "impl": "reference".
+             That arm imports nothing of the product package (tests/test_bench_arms.py).
 """
 import argparse
 import json
@@ -29,13 +38,18 @@ if ROOT not in sys.path:
 
 METRIC = "KV tokens repositioned+spliced/sec"
 UNIT = "KV tokens/s"
+HEADLINE_CONFIG = 4                # largest single-GPU configuration with the paper's (bf16) cache precision
+SWEEP_CONFIGS = (1, 2, 3, 4)       # north_star: the bandwidth bar is on configs 1-4
+SWEEP_LAYOUTS = ("NHD", "HND")
 FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback ("of fallback")
 CACHE_DTYPE = {"bf16": "bf16", "fp8": "fp8-e4m3"}
+L2_BYTES = 126e6
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from one `ncu --set full`
-# capture of the bench command (profiles/, named per round); None until a capture of that config exists.
+# capture of the bench command (profiles/, named per round); None until a capture of that case exists.
+# Keys: "<workload>:<layout>" for the splice, "<workload>:<layout>:<op>" for the other ops.
 NCU_TRAFFIC_BYTES = {}
 try:
-    with open(os.path.join(ROOT, "profiles", "traffic.txt")) as _f:     # lines: "<workload name> <bytes> <source file>"
+    with open(os.path.join(ROOT, "profiles", "traffic.txt")) as _f:     # lines: "<key> <bytes> <source file>"
         for _line in _f:
             _p = _line.split()
             if len(_p) >= 2 and not _line.startswith("#"):
@@ -44,12 +58,17 @@ except OSError:
     pass
 
 
-def parse_args():
+def traffic_of(name, layout, op):
+    return NCU_TRAFFIC_BYTES.get(f"{name}:{layout}" + ("" if op == "splice" else f":{op}"))
+
+
+def parse_args(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=None)
-    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--config", type=int, default=None,
+                    help="index into BASELINE.json configs: time that one alone (default: headline configs[4] + sweep)")
     ap.add_argument("--workload", default="", help="an adapter workload instead of --config (SURVEY.md 8(f) NEXT-3/4): "
                     "mla-dsv2-lite | image-kv-qwen25vl-7b | image-kv-qwen3vl-8b | compose-qwen3-8b; device-timed and e2e only")
     ap.add_argument("--layout", default="NHD", choices=["NHD", "HND"])
@@ -62,11 +81,14 @@ def parse_args():
                          "(SURVEY.md 8(f) NEXT-1: re-float resident chunks, 2*B1 bytes per token; device-timed only); "
                          "span = kvr_write_span over the same rows (Delta = 0: byte copies with the same access pattern "
                          "= this library's own copy ceiling, SURVEY.md H1)")
+    ap.add_argument("--sweep", dest="sweep", action="store_true", default=None, help="force the per_config sweep")
+    ap.add_argument("--no-sweep", dest="sweep", action="store_false")
+    ap.add_argument("--min-device-s", type=float, default=0.25, help="device time per (config, layout) of the sweep")
     ap.add_argument("--e2e-steps", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--tune", default="", help="kvr_tuning overrides, e.g. ctas_per_sm=1,stages=12")
-    return ap.parse_args()
+    return ap.parse_args(argv)
 
 
 def measured_peak():
@@ -77,9 +99,33 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+def algorithmic_bytes(w):
+    """Bytes one step must move: read K, read V, write K, write V of every spliced token."""
+    return (4 if w.has_v else 2) * w.layers * w.kv_heads * w.head_dim * w.elt_bytes * w.tokens
+
+
+def config_block(w, op, config_index, layout, world):
+    """The `config` object of the JSON line: identical keys and values in the kvr arm and the reference arm."""
+    b = algorithmic_bytes(w)
+    return {"workload": w.name, "op": op, "config_index": config_index, "layout": layout,
+            "cache_dtype": CACHE_DTYPE[w.dtype], "tokens": w.tokens, "segments": len(w.segments),
+            "bytes_per_step": b, "parallelism": f"replicas x{world}",
+            "l2": (f"inputs larger than L2 ({b // 2} B of sources + as many pool bytes per step vs 126 MB L2); no flush")
+                  if b // 2 > 2 * L2_BYTES else
+                  (f"working set ({b} B per step) does NOT exceed the 126 MB L2 and is not flushed: a latency-bound "
+                   "case, not a bandwidth figure; see 'latency' (8 rotating buffer sets)")}
+
+
+def bits_to_numpy(t):
+    """Bit-pattern tensor (int16 for bf16, uint8 for fp8) -> contiguous numpy array (uint16 / uint8) on the host."""
+    import numpy as np
+    a = t.detach().cpu().contiguous().numpy()
+    return a.view(np.uint16) if a.dtype == np.int16 else a
+
+
 # --------------------------------------------------------------------------------------- clocks
 class ClockSampler:
-    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+    """Samples SM clock and throttle reasons through NVML while a timed region runs."""
     BAD = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20}
     NOTE = {"sw_power_cap": 0x4}
 
@@ -98,6 +144,9 @@ class ClockSampler:
             self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
         except Exception as e:      # noqa: BLE001 -- no NVML: the clocks object says so
             self.error = repr(e)
+
+    def reset(self):
+        self.samples, self.reasons, self._stop = [], 0, threading.Event()
 
     def sample(self):
         if self._h is None:
@@ -122,20 +171,23 @@ class ClockSampler:
         self._stop.set()
         self._t.join()
 
+    def bad(self):
+        return any(self.reasons & bit for bit in self.BAD.values())
+
     def summary(self):
         if not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable: " + getattr(self, "error", "no samples")]}
         s = sorted(self.samples)
         names = [n for n, bit in {**self.BAD, **self.NOTE}.items() if self.reasons & bit]
-        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": names, "samples": len(s)}
+        return {"sm_mhz": s[len(s) // 2], "sm_min_mhz": s[0], "sm_max_mhz": self.max_mhz, "reasons": names, "samples": len(s)}
 
 
 # --------------------------------------------------------------------------------------- oracle timing
 def _oracle_sample(c, layout, k_steps_total, get_sources, cpu_work_target_s=15.0, wall_cap_s=120.0):
     """Times the oracle, as it stands, on a bounded sample of config c: the first `ls` layers of every segment
-    (every head, token and element of them).  Returns (seconds per step over the sample, ls, layers, threads,
-    run_step) where run_step() performs one sample pass.  The sample is sized from one calibration layer so that
-    a step is ~cpu_work_target_s of CPU work and k_steps_total steps stay under wall_cap_s."""
+    (every head, token and element of them).  Returns (ls, layers, threads, run_step, full workload) where run_step()
+    performs one sample pass.  The sample is sized from one calibration layer so that a step is ~cpu_work_target_s
+    of CPU work and k_steps_total steps stay under wall_cap_s."""
     import numpy as np
     from oracle import kvr_oracle as orc
     from workloads import SENTINEL_BF16, SENTINEL_FP8, config
@@ -151,6 +203,7 @@ def _oracle_sample(c, layout, k_steps_total, get_sources, cpu_work_target_s=15.0
         return w, srcs, kc, vc
 
     w1, s1, kc, vc = make(1)
+    orc.splice_workload(w1, s1, kc, vc, n_threads=threads)        # untimed: page in the pool, start the thread team
     t0 = time.perf_counter()
     orc.splice_workload(w1, s1, kc, vc, n_threads=threads)
     per_layer = time.perf_counter() - t0
@@ -176,8 +229,6 @@ def _oracle_sample(c, layout, k_steps_total, get_sources, cpu_work_target_s=15.0
 
 
 def cpu_sources_from_device(dw):
-    from paper_2606_17107_b200.harness import bits_to_numpy
-
     def get(w, ls):
         return [(bits_to_numpy(k[:ls]), bits_to_numpy(v[:ls])) for k, v in dw.sources]
     return get
@@ -185,7 +236,6 @@ def cpu_sources_from_device(dw):
 
 def cpu_sources_fresh():
     def get(w, ls):
-        from paper_2606_17107_b200.harness import bits_to_numpy
         from workloads import make_sources
         return [(bits_to_numpy(k), bits_to_numpy(v)) for k, v in make_sources(w, "cpu")]
     return get
@@ -205,18 +255,19 @@ def time_oracle(c, layout, steps, warmup, get_sources):
 
 
 def run_reference(args):
+    """The oracle arm: imports oracle/ and workloads/ only -- nothing under paper_2606_17107_b200/."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
     steps = args.steps if args.steps is not None else 5
     warmup = args.warmup if args.warmup is not None else 1
-    value, per_step, threads, sample, full = time_oracle(args.config, args.layout, steps, warmup, cpu_sources_fresh())
+    c = args.config if args.config is not None else HEADLINE_CONFIG
+    value, per_step, threads, sample, full = time_oracle(c, args.layout, steps, warmup, cpu_sources_fresh())
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
         "warmup": warmup, "ms_per_step": per_step * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": full.name, "config_index": args.config, "layout": args.layout,
-                   "cache_dtype": CACHE_DTYPE[full.dtype], "tokens": full.tokens},
+        "config": config_block(full, "splice", c, args.layout, max(1, args.gpus)),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -264,6 +315,119 @@ def latency_probe(w, device, ctx, stream, sets=8, reps=64):
 
 
 # --------------------------------------------------------------------------------------- the kvr arm
+def _median(xs):
+    s = sorted(xs)
+    n = len(s)
+    return s[n // 2] if n % 2 else 0.5 * (s[n // 2 - 1] + s[n // 2])
+
+
+class Timer:
+    """Device timing of one (workload, layout, op) on one stream.  All numbers come from CUDA events recorded on
+    the launching stream; nothing is timed under a profiler."""
+
+    def __init__(self, device, stream, rep, sampler):
+        self.device, self.stream, self.rep, self.sampler = device, stream, rep, sampler
+
+    def warm(self, run_step, warmup):
+        """`warmup` untimed steps, then keep warming until the GPU has been busy for >= 0.3 s: an idle B200 sits at
+        ~120 MHz SM clock and needs tens of ms of load to reach its running clocks.  Returns (ramp steps, s/step)."""
+        import torch
+        for _ in range(warmup):
+            run_step()
+        torch.cuda.synchronize(self.device)
+        ramp, t_ramp = 0, time.perf_counter()
+        while time.perf_counter() - t_ramp < 0.3 and ramp < 100000:
+            for _ in range(8):
+                run_step()
+            ramp += 8
+            torch.cuda.synchronize(self.device)
+        return ramp, (time.perf_counter() - t_ramp) / max(1, ramp)
+
+    def exact_block(self, run_step, steps):
+        """EXACTLY `steps` steps bracketed by barrier + synchronize on both sides.  Returns seconds."""
+        import torch
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(self.device)
+        self.rep.barrier()
+        ev0.record(self.stream)
+        for _ in range(steps):
+            run_step()
+        ev1.record(self.stream)
+        self.sampler.sample()                  # the queue is still draining: a sample under load even for short runs
+        torch.cuda.synchronize(self.device)
+        self.rep.barrier()
+        return ev0.elapsed_time(ev1) * 1e-3
+
+    def blocks(self, run_step, steps, est_step_s, min_device_s, max_blocks=2000):
+        """Blocks of `steps` steps back to back (one event between blocks, no host sync inside) until the device has
+        been timed for >= min_device_s.  Returns the per-block seconds."""
+        import torch
+        block_s = max(steps * est_step_s, 1e-9)
+        n = int(min(max_blocks, max(3 if 3 * block_s < 2.0 else 1, -(-min_device_s // block_s))))
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(n + 1)]
+        torch.cuda.synchronize(self.device)
+        evs[0].record(self.stream)
+        for b in range(n):
+            for _ in range(steps):
+                run_step()
+            evs[b + 1].record(self.stream)
+        self.sampler.sample()
+        torch.cuda.synchronize(self.device)
+        return [evs[b].elapsed_time(evs[b + 1]) * 1e-3 for b in range(n)]
+
+
+def measure_case(kvr, timer, ctx_of, w, dw, op, steps, warmup, min_device_s, peak, headline):
+    """Times one (workload, layout, op).  Returns the per_config entry; with `headline` also the bracketed block."""
+    ctx = ctx_of(dw)
+    stream = timer.stream
+    bytes_per_step = dw.bytes_moved()
+    assert op != "splice" or bytes_per_step == algorithmic_bytes(w), (bytes_per_step, algorithmic_bytes(w))
+    run_step = lambda: dw.run(ctx, stream=stream)
+    if op == "inplace":
+        dw.run(ctx, stream=stream)                       # the chunks must be resident first (finite keys in the slots)
+        spans = dw.inplace_spans([161 + 7 * i for i in range(len(w.segments))])
+        bytes_per_step = kvr.kvr_inplace_bytes_moved(dw.model, spans)
+        run_step = lambda: dw.run_inplace(ctx, spans, stream=stream)
+    elif op == "span":
+        spans_w = dw.write_spans()
+        run_step = lambda: ctx.write_span(dw.dst, spans_w, stream=stream)
+
+    out = {}
+    for attempt in range(2):                   # a region that saw a thermal / hw slowdown is re-measured once
+        ramp, est = timer.warm(run_step, warmup)
+        st = ctx.last_device_status()
+        assert st[0] == kvr.KVR_OK, st
+        timer.sampler.reset()
+        launches0 = ctx.launch_count()
+        with timer.sampler:
+            exact_s = timer.exact_block(run_step, steps) if headline else None
+            launches_exact = ctx.launch_count() - launches0
+            blk = timer.blocks(run_step, steps, est, min_device_s)
+        out["remeasured"] = attempt > 0
+        if not timer.sampler.bad():
+            break
+    st = ctx.last_device_status()
+    assert st[0] == kvr.KVR_OK, st
+    info = ctx.last_launch_info()
+    per_step = [b / steps for b in blk]
+    med, best, worst = _median(per_step), min(per_step), max(per_step)
+    gbs = lambda s: bytes_per_step / s / 1e9
+    out.update({
+        "workload": w.name, "layout": w.layout, "op": op, "cache_dtype": CACHE_DTYPE[w.dtype], "tokens": w.tokens,
+        "segments": len(w.segments), "bytes_per_step": int(bytes_per_step),
+        "ms_per_step": med * 1e3, "best_ms_per_step": best * 1e3, "worst_ms_per_step": worst * 1e3,
+        "spread": (worst - best) / med, "blocks": len(blk), "steps_per_block": steps, "device_s": sum(blk),
+        "tokens_per_s": w.tokens / med,
+        "achieved": gbs(med), "best_achieved": gbs(best), "unit": "GB/s", "frac": gbs(med) / peak,
+        "best_frac": gbs(best) / peak, "gb_s_of_nominal_8000": gbs(med) / 8000.0,
+        "clocks": timer.sampler.summary(), "traffic": traffic_of(w.name, w.layout, op),
+        "kernel": {1: "kvr_generic_kernel", 2: "kvr_ring_kernel"}.get(info["path"], "?"),
+        "grid": info["grid"], "block": info["block"], "smem": info["smem"],
+        "warmup": warmup, "warmup_ramp_steps": ramp,
+    })
+    return out, exact_s, launches_exact, ctx
+
+
 def run_kvr(args):
     import torch
     from paper_2606_17107_b200 import build as _kbuild
@@ -279,72 +443,68 @@ def run_kvr(args):
     device = torch.device("cuda", local_rank)
     torch.cuda.set_device(device)
     rep = Replicas(backend="nccl", device=device)
-    steps = args.steps if args.steps is not None else 1000
-    warmup = max(3, args.warmup if args.warmup is not None else 50)
-
-    if args.workload:
-        from workloads import adapter_config
-        w = adapter_config(args.workload, args.layout)
-        args.no_cpu_baseline = True
-    else:
-        w = config(args.config, args.layout)
-    dw = DeviceWorkload(w, device)
-    tokens, bytes_per_step = w.tokens, dw.bytes_moved()
-    stream = torch.cuda.Stream(device=device)
-    ctx = kvr.Context(dw.model, device=local_rank)
-    if args.tune:
-        ctx.set_tuning(**{k: int(v) for k, v in (kv.split("=") for kv in args.tune.split(","))})
-
-    run_step = lambda: dw.run(ctx, stream=stream)
-    if args.op == "inplace":
-        dw.run(ctx, stream=stream)                       # the chunks must be resident first (finite keys in the slots)
-        spans = dw.inplace_spans([161 + 7 * i for i in range(len(w.segments))])
-        bytes_per_step = kvr.kvr_inplace_bytes_moved(dw.model, spans)
-        run_step = lambda: dw.run_inplace(ctx, spans, stream=stream)
-        args.no_e2e = args.no_cpu_baseline = True
-
-    if args.op == "span":
-        spans_w = dw.write_spans()
-        run_step = lambda: ctx.write_span(dw.dst, spans_w, stream=stream)
-        args.no_e2e = args.no_cpu_baseline = True
-
-    # ---- device-resident timing ----
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler = ClockSampler(device)             # NVML init happens here, before the warm-up, not after it
-    for _ in range(warmup):
-        run_step()
-    # An idle B200 sits at ~120 MHz SM clock and needs some tens of ms of load to reach its running clocks; a
-    # handful of sub-ms warm-up steps does not get it there.  Keep warming (untimed) until the GPU has been
-    # busy for >= 0.3 s, then go straight into the timed region.  `warmup` in the JSON line is the count done.
-    t_ramp = time.perf_counter()
-    while time.perf_counter() - t_ramp < 0.3 and warmup < 100000:
-        for _ in range(8):
-            run_step()
-        warmup += 8
-        torch.cuda.synchronize(device)
-    st = ctx.last_device_status()
-    assert st[0] == kvr.KVR_OK, st
-    torch.cuda.synchronize(device)
-    rep.barrier()
-    launches0 = ctx.launch_count()
-    with sampler:
-        ev0.record(stream)
-        for _ in range(steps):
-            run_step()
-        ev1.record(stream)
-        sampler.sample()                       # the queue is still draining: a sample under load even for short runs
-        torch.cuda.synchronize(device)
-    rep.barrier()
-    launches = ctx.launch_count() - launches0
-    seconds = ev0.elapsed_time(ev1) * 1e-3
-    agg = aggregate_throughput(rep, tokens * steps, seconds)
-    info = ctx.last_launch_info()
-    clocks = sampler.summary()
+    single = args.config is not None or bool(args.workload) or args.op != "splice"
+    steps = args.steps if args.steps is not None else (1000 if single else 20)
+    warmup = max(3, args.warmup if args.warmup is not None else (50 if single else 5))
+    sweep = args.sweep if args.sweep is not None else (not single and rep.world == 1)
+    head_c = args.config if args.config is not None else HEADLINE_CONFIG
     peak, peak_src = measured_peak()
+    stream = torch.cuda.Stream(device=device)
+    timer = Timer(device, stream, rep, ClockSampler(device))     # NVML init happens here, before any warm-up
+    tune = {k: int(v) for k, v in (kv.split("=") for kv in args.tune.split(","))} if args.tune else {}
+
+    ctxs = []
+
+    def ctx_of(dw):
+        ctx = kvr.Context(dw.model, device=local_rank)
+        if tune:
+            ctx.set_tuning(**tune)
+        ctxs.append(ctx)
+        return ctx
+
+    # ---- sweep: configs[1..4] x {NHD, HND}; the headline case is measured last and keeps its buffers ----
+    per_config, head = [], None
+    cases = []
+    if sweep:
+        for c in SWEEP_CONFIGS:
+            for lay in SWEEP_LAYOUTS:
+                if not (c == head_c and lay == args.layout):
+                    cases.append((c, lay))
+    cases.append((head_c, args.layout))
+    sources, sources_c = None, None
+    for c, lay in cases:
+        is_head = (c, lay) == (head_c, args.layout)
+        if args.workload and is_head:
+            from workloads import adapter_config
+            w = adapter_config(args.workload, lay)
+            args.no_cpu_baseline = True
+        else:
+            w = config(c, lay)
+        if sources_c != c:
+            sources, sources_c = None, c                 # frees the previous configuration's sources
+        dw = DeviceWorkload(w, device, sources=sources)   # the two layouts of a configuration share its sources
+        sources = dw.sources
+        entry, exact_s, launches, ctx = measure_case(kvr, timer, ctx_of, w, dw, args.op if is_head else "splice",
+                                                     steps, warmup, args.min_device_s, peak, headline=is_head)
+        entry["config_index"] = None if (args.workload and is_head) else c
+        per_config.append(entry)
+        if is_head:
+            head = (w, dw, ctx, entry, exact_s, launches)
+        else:
+            ctx.close()
+            del dw
+            torch.cuda.empty_cache()
+    per_config.sort(key=lambda e: (e["config_index"] if e["config_index"] is not None else -1, e["layout"]))
+
+    w, dw, ctx, entry, seconds, launches = head
+    if args.op != "splice":
+        args.no_e2e = args.no_cpu_baseline = True
+    tokens, bytes_per_step = w.tokens, entry["bytes_per_step"]
+    agg = aggregate_throughput(rep, tokens * steps, seconds)
     achieved = bytes_per_step / (seconds / steps) / 1e9      # this rank's kernel: one launch per step
 
     latency = None
-    if (args.latency or (not args.workload and args.config == 0)) and args.op == "splice" and rep.world == 1:
+    if (args.latency or (not args.workload and head_c == 0)) and args.op == "splice" and rep.world == 1:
         latency = latency_probe(w, device, ctx, stream)
 
     # ---- end to end: sources in pinned host memory, through kvr_reposition_splice_host ----
@@ -371,41 +531,46 @@ def run_kvr(args):
                "steps": e2e_steps, "ms_per_step": e_agg["seconds"] / e2e_steps * 1e3,
                "api": "kvr_reposition_splice_host (pinned host K/V sources -> staged H2D overlapped with the kernel) "
                       "+ kvr_last_device_status"}
+        dw.host_sources = dw.host_segs = None
 
-    # ---- oracle on the host cores (rank 0, N = 1 only) ----
+    # ---- oracle on the host cores (rank 0, N = 1 only): 1 warm-up + 3 timed passes over a bounded sample ----
     cpu = None
     if rep.world == 1 and not args.no_cpu_baseline:
-        v, per_step, threads, sample, _ = time_oracle(args.config, args.layout, 1, 0, cpu_sources_from_device(dw))
+        v, per_step, threads, sample, _ = time_oracle(head_c, args.layout, 3, 1, cpu_sources_from_device(dw))
         cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
                "single_thread_value": getattr(_oracle_sample, "single_thread_value", None),
                "single_thread_sample": "layer 0 of every segment, one thread, scaled linearly to all layers"}
 
-    ctx.close()
+    for c_ in ctxs:
+        c_.close()
     if rep.rank == 0:
+        cfg = config_block(w, args.op, None if args.workload else head_c, args.layout, rep.world)
+        cfg["bytes_per_step"] = int(bytes_per_step)
         line = {
             "metric": {"splice": METRIC, "inplace": "KV tokens repositioned in place/sec",
                        "span": "KV tokens overwritten (Delta = 0 copy)/sec"}[args.op],
             "value": agg["per_second"], "unit": UNIT, "n_gpus": rep.world, "steps": steps,
-            "warmup": warmup, "ms_per_step": agg["seconds"] / steps * 1e3, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": w.name, "op": args.op, "config_index": None if args.workload else args.config,
-                       "layout": args.layout,
-                       "cache_dtype": CACHE_DTYPE[w.dtype], "tokens": tokens, "segments": len(w.segments),
-                       "bytes_per_step": bytes_per_step, "parallelism": f"replicas x{rep.world}",
-                       "l2": (f"inputs larger than L2 ({bytes_per_step // 2} B of sources + as many pool bytes "
-                              "per step vs 126 MB L2); no flush") if bytes_per_step // 2 > 2 * 126e6 else
-                             (f"working set ({bytes_per_step} B per step) does NOT exceed the 126 MB L2 and is not flushed: "
-                              "a latency-bound case, not a bandwidth figure; see 'latency' (8 rotating buffer sets)"),
-                       "kernel": {1: "kvr_generic_kernel", 2: "kvr_ring_kernel"}.get(info["path"], "?"),
-                       "grid": info["grid"], "block": info["block"], "smem": info["smem"]},
+            "warmup": warmup, "warmup_ramp_steps": entry["warmup_ramp_steps"],
+            "ms_per_step": agg["seconds"] / steps * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": w.dtype if w.dtype == "bf16" else "fp8-e4m3",
+            "arithmetic": "fp32 registers (bf16: compensated rotate) on an fp64 sincos table; one rounding to the cache dtype",
+            "data": "synthetic", "config": cfg,
+            "launch": {"kernel": entry["kernel"], "grid": entry["grid"], "block": entry["block"], "smem": entry["smem"]},
             "gpu_launches": launches,
-            "clocks": clocks,
+            "clocks": entry["clocks"],
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC_BYTES.get(w.name if args.op == "splice" else w.name + ":inplace"), "peak_source": peak_src,
-                         "gb_s_of_nominal_8000": achieved / 8000.0},
+                         "traffic": entry["traffic"], "peak_source": peak_src,
+                         "gb_s_of_nominal_8000": achieved / 8000.0,
+                         "median_achieved": entry["achieved"], "best_achieved": entry["best_achieved"],
+                         "spread": entry["spread"], "blocks": entry["blocks"]},
             "e2e": e2e,
             "cpu_baseline": cpu,
         }
+        if sweep or len(per_config) > 1:
+            line["per_config"] = per_config
+        else:
+            line["timing"] = {k: entry[k] for k in ("ms_per_step", "best_ms_per_step", "worst_ms_per_step", "spread",
+                                                     "blocks", "steps_per_block", "device_s", "remeasured")}
         if latency is not None:
             line["latency"] = latency
         print(json.dumps(line), flush=True)
