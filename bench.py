@@ -87,6 +87,9 @@ def parse_args(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--layers", type=int, default=None,
+                    help="profiling aid: keep only the first N layers of the configuration (same kernel, tiles and "
+                         "per-layer access pattern, less memory for ncu to save and restore); never a bench number")
     ap.add_argument("--tune", default="", help="kvr_tuning overrides, e.g. ctas_per_sm=1,stages=12")
     return ap.parse_args(argv)
 
@@ -479,7 +482,7 @@ def run_kvr(args):
             w = adapter_config(args.workload, lay)
             args.no_cpu_baseline = True
         else:
-            w = config(c, lay)
+            w = config(c, lay, layers=args.layers)
         if sources_c != c:
             sources, sources_c = None, c                 # frees the previous configuration's sources
         dw = DeviceWorkload(w, device, sources=sources)   # the two layouts of a configuration share its sources
@@ -546,6 +549,8 @@ def run_kvr(args):
     if rep.rank == 0:
         cfg = config_block(w, args.op, None if args.workload else head_c, args.layout, rep.world)
         cfg["bytes_per_step"] = int(bytes_per_step)
+        if args.layers is not None:
+            cfg["layers_override"] = args.layers           # a profiling run, not a bench number
         line = {
             "metric": {"splice": METRIC, "inplace": "KV tokens repositioned in place/sec",
                        "span": "KV tokens overwritten (Delta = 0 copy)/sec"}[args.op],

@@ -26,7 +26,9 @@
  *     K', V are written at element offset  l*stride_layer + blk*stride_block + off*stride_token + h*stride_head
  * Delta_t == 0 copies the K row byte for byte.  In KVR_FP8_E4M3 mode K is dequantised with the
  * source scale, rotated, and requantised (round-to-nearest-even, saturating to +-448) with the
- * destination scale; V bytes are always copied unchanged.
+ * destination scale; where the two scales of a (layer, head) are the same number they cancel exactly
+ * ((q s cos - q' s sin) / s = q cos - q' sin) and every kernel rotates the e4m3 codes as they are.
+ * V bytes are always copied unchanged.
  *
  * Every step above runs in hand-written CUDA kernels; there is no CPU fallback.  All entry points
  * return kvr_status and never throw.  Nothing here synchronises the device except where stated.
@@ -163,7 +165,13 @@ KVR_API kvr_status kvr_validate(const kvr_model_desc* model, const kvr_paged_dst
  * default stream), the reposition + splice of n_segs segments into dst.  Asynchronous: returns once the
  * work is enqueued; there is no device synchronisation.  Host-detectable faults are rejected before any
  * launch and leave the destination untouched.  Calls on one context must be issued to one stream at a
- * time (the context owns per-call staging).  Every destination byte not addressed keeps its value. */
+ * time (the context owns per-call staging).  Every destination byte not addressed keeps its value.
+ * CUDA graphs: a call with at most 8 segments carries its descriptors in the kernel parameters, enqueues nothing
+ * but its kernel and may be captured (stream capture) and replayed; the pointers it was given must stay valid for
+ * every replay.  A call with more than 8 segments stages its descriptors through context-owned pinned memory that
+ * later calls reuse, so under capture it is refused with KVR_ERR_UNSUPPORTED before anything is enqueued (split it
+ * into calls of <= 8 segments to capture it).  The same rule holds for kvr_reposition_inplace and kvr_write_span
+ * (spans); kvr_reposition_splice_host is never capturable. */
 KVR_API kvr_status kvr_reposition_splice(kvr_ctx* ctx, const kvr_paged_dst* dst, const kvr_segment* segs,
                                          int32_t n_segs, void* cuda_stream);
 

@@ -99,6 +99,7 @@ struct kvr_ctx {
   int device = 0, sm_count = 0;
   Slot slots[kSlots];
   int next_slot = 0;
+  SegDev inline_scratch[kInlineSegs];   // host-side descriptors of calls that carry them in the kernel parameters
   kvr_tuning tuning{};
   uint64_t launches = 0;
   int last_path = 0, last_grid = 0, last_block = 0, last_smem = 0;
@@ -251,17 +252,29 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   KVR_CUDA(c, cudaStreamIsCapturing(stream, &cap));
   const bool capturing = cap != cudaStreamCaptureStatusNone;
 
-  Slot& slot = c->slots[c->next_slot];
-  c->next_slot = (c->next_slot + 1) % kSlots;
-  if (slot.pending && !capturing) {
-    KVR_CUDA(c, cudaEventSynchronize(slot.ev));   // the call that used this slot 8 calls ago
-    slot.pending = false;
+  // Descriptors.  Calls with <= kInlineSegs segments carry them in the kernel parameters: they are built in a
+  // context-owned host scratch array, enqueue nothing but the kernel and may be captured in a CUDA graph.  Larger calls
+  // stage them through a ring of pinned slots + one H2D copy; a captured copy node would read its pinned slot again at
+  // every replay, long after later calls have overwritten it, so such calls are refused under capture (kvr.h).
+  const bool inline_descs = n <= kInlineSegs;
+  if (capturing && !inline_descs) {
+    c->last_err = "more than 8 segments (spans) per call cannot be captured in a CUDA graph";
+    return KVR_ERR_UNSUPPORTED;
   }
-  if ((size_t)n > slot.cap) {
-    if (capturing) return KVR_ERR_UNSUPPORTED;    // cannot allocate under stream capture; warm the context first
-    st = slot_reserve(c, slot, (size_t)n);
-    if (st != KVR_OK) return st;
+  Slot* slot_p = nullptr;
+  if (!inline_descs) {
+    slot_p = &c->slots[c->next_slot];
+    c->next_slot = (c->next_slot + 1) % kSlots;
+    if (slot_p->pending) {
+      KVR_CUDA(c, cudaEventSynchronize(slot_p->ev));   // the call that used this slot kSlots calls ago
+      slot_p->pending = false;
+    }
+    if ((size_t)n > slot_p->cap) {
+      st = slot_reserve(c, *slot_p, (size_t)n);
+      if (st != KVR_OK) return st;
+    }
   }
+  SegDev* const host_descs = inline_descs ? c->inline_scratch : slot_p->host;
 
   kvr_model_desc m = c->model;
   m.layers = nl;
@@ -279,7 +292,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   P.k_scale_dst = d->k_scale ? d->k_scale + (int64_t)l0 * m.kv_heads : nullptr;
   P.num_blocks = d->num_blocks; P.block_size = d->block_size; P.num_seqs = d->num_seqs;
   P.max_blocks = d->max_blocks_per_seq;
-  P.segs = slot.dev; P.n_segs = n; P.status = c->d_status;
+  P.segs = inline_descs ? nullptr : slot_p->dev; P.n_segs = n; P.status = c->d_status;
   P.sched = c->d_sched;
 
   bool any_map = false, scales_differ = false;
@@ -303,7 +316,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     int64_t chunks_total = 0;
     for (int32_t i = 0; i < n; ++i) {
       const kvr_segment& s = segs[i];
-      SegDev& o = slot.host[i];
+      SegDev& o = host_descs[i];
       const int64_t src_adv = src_group_local ? 0 : (int64_t)l0 * s.src_stride_layer * E;
       o.k_src = static_cast<const uint8_t*>(s.k_src) + src_adv;
       o.v_src = s.v_src ? static_cast<const uint8_t*>(s.v_src) + src_adv : nullptr;
@@ -347,8 +360,8 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     P.lpu = lpu; P.n_lgroups = ((m.layers + lpu - 1) / lpu) * hsplit;
     int64_t at = 0;
     for (int32_t i = 0; i < n; ++i) {
-      slot.host[i].unit_begin = at;
-      at += (int64_t)slot.host[i].n_chunks * P.n_lgroups;
+      host_descs[i].unit_begin = at;
+      at += (int64_t)host_descs[i].n_chunks * P.n_lgroups;
     }
     P.total_units = at;
   };
@@ -414,7 +427,8 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       cg_limit = cg_limit < 1 ? 1 : (cg_limit > 16 ? 16 : cg_limit);
     }
     decompose(chunk_granularity(d->block_size, cg_limit), tu.layers_per_unit, tu.hsplit, true);
-    bool ok = ring_supported(P, slot.host, &why);
+    const RingConfig rc0{tu.ctas_per_sm, tu.consumer_warps, tu.stages, tu.v_bulk_store, tu.max_ctas, tu.grab, tu.pdl, tu.warps_per_stage};
+    bool ok = ring_supported(P, host_descs, rc0, c->sm_count, &why);
     if (!ok && path == 2) { c->last_err = std::string("ring kernel unsupported: ") + (why ? why : ""); return KVR_ERR_UNSUPPORTED; }
     path = ok ? 2 : 1;
   }
@@ -425,10 +439,10 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     decompose(chunk_granularity(d->block_size, limit < 16 ? limit : 16), tu.layers_per_unit, 1, false);
   }
 
-  if (n <= kInlineSegs) {
-    for (int32_t i = 0; i < n; ++i) P.inline_segs[i] = slot.host[i];   // descriptors ride in the kernel parameters
+  if (inline_descs) {
+    for (int32_t i = 0; i < n; ++i) P.inline_segs[i] = host_descs[i];   // descriptors ride in the kernel parameters
   } else {
-    KVR_CUDA(c, cudaMemcpyAsync(slot.dev, slot.host, (size_t)n * sizeof(SegDev), cudaMemcpyHostToDevice, stream));
+    KVR_CUDA(c, cudaMemcpyAsync(slot_p->dev, slot_p->host, (size_t)n * sizeof(SegDev), cudaMemcpyHostToDevice, stream));
   }
   cudaError_t e;
   if (path == 2) {
@@ -441,9 +455,9 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   c->launches += 1;
   c->last_path = path;
   c->last_stream = stream;
-  if (!capturing) {
-    KVR_CUDA(c, cudaEventRecord(slot.ev, stream));
-    slot.pending = true;
+  if (slot_p) {
+    KVR_CUDA(c, cudaEventRecord(slot_p->ev, stream));   // the slot may be rewritten once its copy and kernel have run
+    slot_p->pending = true;
   }
   return KVR_OK;
 }
@@ -655,6 +669,7 @@ uint64_t kvr_inplace_bytes_moved(const kvr_model_desc* m, const kvr_resident_spa
 // ---- NEXT-2: span overwrite = the delta == 0 splice (R21) ----
 kvr_status kvr_write_span(kvr_ctx* c, const kvr_paged_dst* dst, const kvr_span* spans, int32_t n, void* cuda_stream) {
   if (!c) return KVR_ERR_INVALID_ARG;
+  c->last_err.clear();
   if (n < 0 || (n > 0 && !spans)) return KVR_ERR_INVALID_ARG;
   std::vector<kvr_segment> segs((size_t)n);
   for (int32_t i = 0; i < n; ++i) {

@@ -178,7 +178,7 @@ struct RingConfig {
 };
 int ring_heads_per_tile(const CallParams& P);   // heads one tile of the ring kernel covers (needs P.cg)
 bool ring_window_mode(const CallParams& P);      // rows outside the power-of-two slot layout (e.g. MLA [latent | k_pe])
-bool ring_supported(const CallParams& P, const SegDev* host_segs, const char** why);
+bool ring_supported(const CallParams& P, const SegDev* host_segs, const RingConfig& cfg, int sm_count, const char** why);
 cudaError_t launch_ring(const CallParams& P, const RingConfig& cfg, int sm_count, cudaStream_t stream,
                         int* grid, int* block, int* smem);
 

@@ -76,7 +76,16 @@ __global__ void __launch_bounds__(256) kvr_generic_kernel(const __grid_constant_
       } else {
         uint8_t qa = src[ia], qb = src[ib];
         float s_src = s.k_scale_src[l * P.heads + h], s_dst = P.k_scale_dst[l * P.heads + h];
-        if (!(is_copy[t] && s_src == s_dst)) {
+        if (s_src == s_dst) {
+          // equal scales cancel exactly ((q s c - q' s s') / s = q c - q' s'): the codes are rotated as they are,
+          // the same formulation as the ring kernel (kvr.h)
+          if (!is_copy[t]) {
+            float ra, rb;
+            rotate_plain(e4m3_to_f32(qa), e4m3_to_f32(qb), cs.x, cs.z, ra, rb);
+            qa = (uint8_t)f32_to_e4m3_sat(ra);
+            qb = (uint8_t)f32_to_e4m3_sat(rb);
+          }
+        } else {
           float c_ = is_copy[t] ? 1.0f : cs.x, s_ = is_copy[t] ? 0.0f : cs.z;
           float ra, rb, inv = __frcp_rn(s_dst);
           rotate_plain(__fmul_rn(e4m3_to_f32(qa), s_src), __fmul_rn(e4m3_to_f32(qb), s_src), c_, s_, ra, rb);

@@ -23,6 +23,7 @@
 // Persistent grid = SMs x CTAs/SM; programmatic dependent launch overlaps a launch's prologue (and its first
 // angle table) with the tail of the previous one.
 #include <cstdio>
+#include <mutex>
 
 #include "kvr_common.cuh"
 
@@ -71,6 +72,7 @@ static_assert(sizeof(TileMeta) == 32, "TileMeta layout");
 constexpr int kFlagDone = 1, kFlagRotate = 2, kFlagTokMajor = 4;   // TokMajor: the stage is laid out [token][head][dim]
 constexpr int kFlagKOnly = 8, kFlagVOnly = 16;                       // split gather tiles: the stage holds K or V alone
 constexpr int kMaxThreads = 32 * 17;
+constexpr int kMaxDevices = 64;
 
 // ------------------------------------------------------------------------------- PTX helpers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -759,7 +761,10 @@ bool ring_window_mode(const CallParams& P) {
   return P.rotary_offset != 0 || rowB > 1024 || (rowB & (rowB - 1)) != 0;
 }
 
-bool ring_supported(const CallParams& P, const SegDev* segs, const char** why) {
+static bool ring_plan(const CallParams& P_in, const RingConfig& cfg, int sm_count, CallParams& P, RingParams& RP,
+                      int& grid, int& block, int& smem);
+
+bool ring_supported(const CallParams& P, const SegDev* segs, const RingConfig& cfg, int sm_count, const char** why) {
   const int E = P.dtype == 0 ? 2 : 1;
   const int rowB = P.head_dim * E;
   const char* w = nullptr;
@@ -775,17 +780,32 @@ bool ring_supported(const CallParams& P, const SegDev* segs, const char** why) {
   else if (P.dtype == 1 && (int64_t)P.layers * P.heads > 8192) w = "too many (layer, head) scales for shared memory";
   else if (P.rotary_dim / 2 > 512) w = "rotary_dim too large for the shared angle table";
   (void)segs;
+  if (!w) {
+    // the shortest ring (2 stages) with its angle tables, scales and tile descriptors must fit the CTA's shared memory:
+    // e.g. bf16 head_dim = rotary_dim = 512 with per-token shifts needs 2 x 64 KB of tables and takes the generic kernel
+    CallParams Pp; RingParams RP; int g, b, sm;
+    if (!ring_plan(P, cfg, sm_count, Pp, RP, g, b, sm)) w = "the ring's shared-memory layout (tables + scales + 2 stages) does not fit";
+  }
   if (why) *why = w;
   return w == nullptr;
 }
 
 template <int DTYPE, int PAIRING, bool MAP, int MAXT>
 static cudaError_t launch_inst(const CallParams& P, const RingParams& RP, int grid, int block, int smem, cudaStream_t st, bool pdl) {
-  static int configured = 0;   // per instantiation
-  if (configured < smem) {
-    cudaError_t e = cudaFuncSetAttribute(kvr_ring_kernel<DTYPE, PAIRING, MAP, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    configured = smem;
+  // The opt-in to > 48 KB of dynamic shared memory is a per-DEVICE attribute of the function: remember what was set per
+  // (instantiation, device), under a lock (contexts on several devices / host threads share this process-wide table).
+  static std::mutex mu;
+  static int configured[kMaxDevices] = {};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  {
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev < 0 || dev >= kMaxDevices || configured[dev] < smem) {
+      e = cudaFuncSetAttribute(kvr_ring_kernel<DTYPE, PAIRING, MAP, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+      if (e != cudaSuccess) return e;
+      if (dev >= 0 && dev < kMaxDevices) configured[dev] = smem;
+    }
   }
   cudaLaunchConfig_t lc{};
   lc.gridDim = dim3((unsigned)grid); lc.blockDim = dim3((unsigned)block); lc.dynamicSmemBytes = (size_t)smem; lc.stream = st;
@@ -796,12 +816,13 @@ static cudaError_t launch_inst(const CallParams& P, const RingParams& RP, int gr
   return cudaLaunchKernelEx(&lc, kvr_ring_kernel<DTYPE, PAIRING, MAP, MAXT>, P, RP);
 }
 
-cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_count, cudaStream_t stream,
-                        int* grid_out, int* block_out, int* smem_out) {
-  CallParams P = P_in;
+// Launch shape and shared-memory layout of one call; false when even the shortest ring does not fit.
+static bool ring_plan(const CallParams& P_in, const RingConfig& cfg, int sm_count, CallParams& P, RingParams& RP,
+                      int& grid_out, int& block_out, int& smem_out) {
+  P = P_in;
   P.grab = cfg.grab > 0 ? (cfg.grab > 32 ? 32 : cfg.grab) : 1;
   const int E = P.dtype == 0 ? 2 : 1;
-  RingParams RP{};
+  RP = RingParams{};
   RP.cg = P.cg;
   RP.rowB = P.head_dim * E;
   RP.nr = P.rotary_dim * E / 16;
@@ -846,7 +867,7 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   };
   int S = cfg.stages > 0 ? cfg.stages : 64;
   while (S > 2 && layout(S) > budget) --S;
-  if (layout(S) > budget) return cudaErrorInvalidConfiguration;
+  if (layout(S) > budget) return false;
   // Stage ownership: consumer warp w serves stages (w / wpg) + k * (NW / wpg); S is a multiple of NW / wpg, so the
   // successive phases of one mbarrier are ordered by one warp's program order (a warp two phases ahead would pass a
   // parity wait early).  wpg > 1 only in gather mode, when the ring holds fewer (large) stages than consumer warps.
@@ -886,8 +907,16 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   if (cfg.max_ctas > 0 && g > cfg.max_ctas) g = cfg.max_ctas;
   if (g > P.total_units) g = P.total_units;
   if (g < 1) g = 1;
-  const int block = (RP.NW + 1) * 32;
-  *grid_out = (int)g; *block_out = block; *smem_out = smem;
+  grid_out = (int)g; block_out = (RP.NW + 1) * 32; smem_out = smem;
+  return true;
+}
+
+cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_count, cudaStream_t stream,
+                        int* grid_out, int* block_out, int* smem_out) {
+  CallParams P; RingParams RP; int g = 0, block = 0, smem = 0;
+  if (!ring_plan(P_in, cfg, sm_count, P, RP, g, block, smem)) return cudaErrorInvalidConfiguration;
+  *grid_out = g; *block_out = block; *smem_out = smem;
+  const int ctas = cfg.ctas_per_sm > 0 ? cfg.ctas_per_sm : 2;
   const bool map = P.any_pos_map != 0;
   const bool small = block <= 256 && ctas <= 2, mid = block <= 448 && ctas == 1;
 #define KVR_LAUNCH(D, PR, M)                                                                             \

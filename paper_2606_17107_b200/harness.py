@@ -17,36 +17,71 @@ def model_of(w):
                           _DTYPE[w.dtype], w.inv_freq, rotary_offset=getattr(w, "rotary_offset", 0))
 
 
+GUARD_BYTE = 0xA5
+
+
 class DeviceWorkload:
     """Sources, sentinel-filled pool, block table, position maps and scales of `w` resident on `device`,
-    plus the ctypes structs of one kvr_reposition_splice call over all segments."""
+    plus the ctypes structs of one kvr_reposition_splice call over all segments.
 
-    def __init__(self, w, device="cuda:0", sources=None, make_pool=True):
+    guard_bytes > 0 (the GPU tests): every device buffer a call may touch -- pools, sources, block table, position
+    maps, scales -- is a window inside a larger allocation whose first and last `guard_bytes` bytes hold a canary
+    pattern; check_guards() asserts that no kernel wrote outside a window (compute-sanitizer is closed on the GPU
+    pool, and the pool's own sentinel only guards bytes INSIDE it)."""
+
+    def __init__(self, w, device="cuda:0", sources=None, make_pool=True, guard_bytes=0):
         from workloads import make_pool as _make_pool, make_sources
         self.w = w
         self.device = torch.device(device)
+        self.guard_bytes = int(guard_bytes)
+        self._guarded = []                         # (name, whole uint8 allocation, payload bytes)
         self.model, self._inv_keep = model_of(w)
         if sources is None:
             sources = make_sources(w, self.device)
-        self.sources = [(k.to(self.device).contiguous(), None if v is None else v.to(self.device).contiguous())
-                        for k, v in sources]      # v is None for a K-only [latent | k_pe] cache (kvr.h, NEXT-3)
-        self.block_table = torch.from_numpy(np.ascontiguousarray(w.block_table)).to(self.device)
+        self.sources = [(self._dev(k, f"k_src[{i}]"), None if v is None else self._dev(v, f"v_src[{i}]"))
+                        for i, (k, v) in enumerate(sources)]   # v is None for a K-only [latent | k_pe] cache (kvr.h, NEXT-3)
+        self.block_table = self._dev(torch.from_numpy(np.ascontiguousarray(w.block_table)), "block_table")
         self.k_scale = self.k_scale_src = None
         if w.k_scale is not None:
-            self.k_scale = torch.from_numpy(w.k_scale).to(self.device)
+            self.k_scale = self._dev(torch.from_numpy(w.k_scale), "k_scale")
         if w.k_scale_src is not None:
-            self.k_scale_src = torch.from_numpy(w.k_scale_src).to(self.device)
-        self.pos_maps = [None if s.pos_map is None else torch.from_numpy(s.pos_map).to(self.device)
-                         for s in w.segments]
+            self.k_scale_src = self._dev(torch.from_numpy(w.k_scale_src), "k_scale_src")
+        self.pos_maps = [None if s.pos_map is None else self._dev(torch.from_numpy(s.pos_map), f"pos_map[{i}]")
+                         for i, s in enumerate(w.segments)]
         self.k_cache = self.v_cache = None
         if make_pool:
-            self.k_cache, self.v_cache = _make_pool(w, self.device)
+            kc, vc = _make_pool(w, "cpu" if self.guard_bytes else self.device)
+            self.k_cache = self._dev(kc, "k_cache")
+            self.v_cache = None if vc is None else self._dev(vc, "v_cache")
         self.segs = kvr.segment_array([
             kvr.segment(k, v, w.src_strides(s), s.len, s.old_start, s.new_start, s.dst_seq, s.dst_token_start,
                         pos_map=pm, k_scale_src=self.k_scale_src,
                         flags=kvr.KVR_SEG_PRE_ROPE if getattr(s, "pre_rope", False) else 0)
             for s, (k, v), pm in zip(w.segments, self.sources, self.pos_maps)])
         self.dst = self.dst_for(self.k_cache, self.v_cache) if make_pool else None
+
+    def _dev(self, t, name):
+        """`t` on the device; with guards, as a window between two canary regions of one larger allocation."""
+        if not self.guard_bytes:
+            return t.to(self.device).contiguous()
+        t = t.contiguous()
+        g, n = self.guard_bytes, t.numel() * t.element_size()
+        whole = torch.full((2 * g + n,), GUARD_BYTE, dtype=torch.uint8, device=self.device)
+        win = whole[g:g + n].view(t.dtype).view(t.shape)
+        win.copy_(t)
+        self._guarded.append((name, whole, n))
+        return win
+
+    def check_guards(self):
+        """Every canary byte before and after every guarded window still holds GUARD_BYTE."""
+        assert self.guard_bytes and self._guarded, "built without guard_bytes"
+        g = self.guard_bytes
+        for name, whole, n in self._guarded:
+            for side, region in (("before", whole[:g]), ("after", whole[g + n:])):
+                bad = torch.nonzero(region != GUARD_BYTE)
+                assert bad.numel() == 0, (f"{name}: {bad.numel()} byte(s) written {side} the buffer, "
+                                          f"first at offset {int(bad[0])} of the guard region")
+        return len(self._guarded)
 
     def dst_for(self, k_cache, v_cache):
         w = self.w
