@@ -147,7 +147,10 @@ typedef struct {
   int32_t gather;          /* ring kernel, dense token-major pools: tiles of all heads x few tokens, several consumer
                               warps per tile (see kvr_ring.cu): 0 auto, 1 on, 2 off, 3 on with K and V in tiles of their own                            */
   int32_t warps_per_stage; /* gather mode: consumer warps that share one stage (default: all of them)                  */
-  int32_t reserved[2];
+  int32_t lanes_over_heads; /* gather mode: a warp pass covers several HEADS of one token (adjacent rows of a dense
+                              token-major pool) instead of several tokens of one head: 0 auto, 1 on, 2 off */
+  int32_t transpose_load;  /* dense token-major pools: tiles of all heads x few tokens loaded by TMA tensor maps whose
+                              dimension order transposes them into the pool's order on the way in: 0 auto, 1 on, 2 off */
 } kvr_tuning;
 
 /* Creates a context on CUDA device `cuda_device` (must be compute capability 10.x).  Allocates a few

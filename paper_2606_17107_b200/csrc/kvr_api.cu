@@ -2,6 +2,7 @@
 // descriptor staging and kernel dispatch.  No arithmetic of the method happens on the host.
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -16,14 +17,60 @@ namespace {
 constexpr int kSlots = 16;          // descriptor staging ring (launches in flight per context)
 constexpr int kStageBufs = 2;       // host-source path: device staging buffers (copy of group g+1 overlaps kernel g)
 constexpr int kInitialSegCap = 256;
+constexpr bool kTransposeAuto = true;    // tuning.transpose_load == 0: on (B200: every BASELINE config gains)
 
 struct Slot {
   SegDev* host = nullptr;           // pinned
   SegDev* dev = nullptr;
   size_t cap = 0;
+  TmapPair* tm_host = nullptr;      // pinned: tensor maps of the segments' sources (transposing loads), allocated on demand
+  TmapPair* tm_dev = nullptr;
+  size_t tm_cap = 0;
   cudaEvent_t ev = nullptr;
   bool pending = false;
 };
+
+// cuTensorMapEncodeTiled, fetched from the driver the runtime has already loaded (no link against libcuda)
+typedef CUresult (*TmapEncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+TmapEncodeFn tmap_encoder() {
+  static TmapEncodeFn fn = nullptr;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess &&
+        qr == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<TmapEncodeFn>(p);
+    (void)cudaGetLastError();
+  });
+  return fn;
+}
+
+// Tensor map of one source tensor [layers][heads][len][head_dim] (element strides sl, sh, st) with its dimensions ordered
+// (dim, head, token, layer): a box {head_dim, heads, ct, 1} then lands in shared memory as [token][head][dim].
+bool encode_source_map(CUtensorMap* out, const void* base, int dtype, int head_dim, int heads, int len, int layers,
+                       int64_t sl, int64_t sh, int64_t st, int ct) {
+  TmapEncodeFn enc = tmap_encoder();
+  if (!enc || !base) return false;
+  const uint64_t E = dtype == KVR_BF16 ? 2 : 1, rowB = (uint64_t)head_dim * E;
+  // a dimension of extent 1 never uses its stride: give it a legal one
+  uint64_t s_h = (uint64_t)sh * E, s_t = (uint64_t)st * E, s_l = (uint64_t)sl * E;
+  if (heads == 1 && s_h == 0) s_h = rowB;
+  if (len == 1 && s_t == 0) s_t = rowB;
+  if (layers == 1 && s_l == 0) s_l = rowB;
+  if (s_h == 0 || s_t == 0 || s_l == 0) return false;
+  const cuuint64_t dims[4] = {(cuuint64_t)head_dim, (cuuint64_t)heads, (cuuint64_t)len, (cuuint64_t)layers};
+  const cuuint64_t strides[3] = {s_h, s_t, s_l};
+  const cuuint32_t box[4] = {(cuuint32_t)head_dim, (cuuint32_t)heads, (cuuint32_t)ct, 1u};
+  const cuuint32_t es[4] = {1u, 1u, 1u, 1u};
+  const CUtensorMapL2promotion promo = rowB >= 256 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
+                                     : rowB >= 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : CU_TENSOR_MAP_L2_PROMOTION_NONE;
+  return enc(out, dtype == KVR_BF16 ? CU_TENSOR_MAP_DATA_TYPE_UINT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8, 4,
+             const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+             promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 
 inline int elt_bytes(int dtype) { return dtype == KVR_BF16 ? 2 : 1; }
 
@@ -130,6 +177,7 @@ struct kvr_ctx {
     if (e_ != cudaSuccess) return (ctx)->cuda_fail(e_, #call); \
   } while (0)
 
+static kvr_status slot_reserve_tmaps(kvr_ctx* c, Slot& s, size_t n);
 static kvr_status slot_reserve(kvr_ctx* c, Slot& s, size_t n) {
   if (n <= s.cap) return KVR_OK;
   size_t cap = s.cap ? s.cap : kInitialSegCap;
@@ -140,6 +188,19 @@ static kvr_status slot_reserve(kvr_ctx* c, Slot& s, size_t n) {
   KVR_CUDA(c, cudaMallocHost(&s.host, cap * sizeof(SegDev)));
   KVR_CUDA(c, cudaMalloc(&s.dev, cap * sizeof(SegDev)));
   s.cap = cap;
+  return KVR_OK;
+}
+
+static kvr_status slot_reserve_tmaps(kvr_ctx* c, Slot& s, size_t n) {
+  if (n <= s.tm_cap) return KVR_OK;
+  size_t cap = s.tm_cap ? s.tm_cap : kInitialSegCap;
+  while (cap < n) cap *= 2;
+  if (s.tm_host) cudaFreeHost(s.tm_host);
+  if (s.tm_dev) cudaFree(s.tm_dev);
+  s.tm_host = nullptr; s.tm_dev = nullptr; s.tm_cap = 0;
+  KVR_CUDA(c, cudaMallocHost(&s.tm_host, cap * sizeof(TmapPair)));
+  KVR_CUDA(c, cudaMalloc(&s.tm_dev, cap * sizeof(TmapPair)));
+  s.tm_cap = cap;
   return KVR_OK;
 }
 
@@ -200,6 +261,8 @@ kvr_status kvr_destroy(kvr_ctx* c) {
   for (Slot& s : c->slots) {
     if (s.host) cudaFreeHost(s.host);
     if (s.dev) cudaFree(s.dev);
+    if (s.tm_host) cudaFreeHost(s.tm_host);
+    if (s.tm_dev) cudaFree(s.tm_dev);
     if (s.ev) cudaEventDestroy(s.ev);
   }
   for (int b = 0; b < kStageBufs; ++b) {
@@ -307,7 +370,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     P.cg = cg;
     // head split (ring kernel only): must divide the number of head groups of a unit
     int hsplit = 1;
-    if (hsplit_request > 1 && !any_map) {
+    if (hsplit_request > 1 && !any_map && !P.tmajor) {
       const int hgroups = m.kv_heads / ring_heads_per_tile(P);
       hsplit = hsplit_request > hgroups ? hgroups : hsplit_request;
       while (hsplit > 1 && hgroups % hsplit) --hsplit;
@@ -338,7 +401,8 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       // concurrently read neighbouring source rows of one layer (DRAM page locality: +3 % on configs[2] against
       // 11 layers per unit) and the tail is short.  With a position map the per-chunk angle table is rebuilt per
       // unit, so a unit holds ~24 tiles there.
-      const int tiles_per_layer = ((m.kv_heads / ring_heads_per_tile(P)) / hsplit) * (P.gather == 2 ? 2 : 1);
+      const int tiles_per_layer = P.tmajor ? (cg + P.ct - 1) / P.ct
+                                           : ((m.kv_heads / ring_heads_per_tile(P)) / hsplit) * (P.gather == 2 ? 2 : 1);
       // (with pre-RoPE keys every token has its own shift, nothing deduplicates: ~96 tiles per unit.  One value per
       //  call: giving the constant-shift segments of such a call their own, smaller units measured slower.)
       bool any_pre = false;
@@ -369,14 +433,35 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
   const kvr_tuning& tu = c->tuning;
   int path = tu.path;
   const char* why = nullptr;
-  if (path == 0 || path == 2) {
+  TmapInline tmaps_inline;             // tensor maps of a call with inline descriptors (transposing loads)
+  bool use_tmaps = false;
+  for (int attempt = 0; attempt < 2 && (path == 0 || path == 2); ++attempt) {
     int cg_limit = (tu.chunk_tokens > 0 && tu.chunk_tokens < 16) ? tu.chunk_tokens : 16;
     P.tile_min_bytes = tu.tile_bytes;
+    // TRANSPOSING loads (kvr_ring.cu, TmapPair): dense token-major (NHD) pool, several heads, power-of-two rows, not in
+    // place: a tile = ALL heads x ct tokens, loaded by one TMA tensor operation per tensor so that it lands in shared
+    // memory in the pool's own order; V then leaves as one contiguous bulk store and K as contiguous warp stores.
+    // tuning.transpose_load: 0 auto, 1 on, 2 off.  Second attempt (the encoder refused a source): off.
+    P.tmajor = 0; P.ct = 0; P.tmaps = nullptr;
+    {
+      const int64_t rowB = (int64_t)m.head_dim * E;
+      const bool pow2_row = rowB >= 32 && rowB <= 1024 && (rowB & (rowB - 1)) == 0 && m.rotary_offset == 0;
+      const bool dense_nhd = d->stride_head == m.head_dim && d->stride_token == (int64_t)m.kv_heads * m.head_dim;
+      const bool want = tu.transpose_load == 1 || (tu.transpose_load == 0 && kTransposeAuto);
+      if (attempt == 0 && want && !inplace && pow2_row && dense_nhd && m.kv_heads >= 2 && m.kv_heads <= 256 &&
+          m.head_dim <= 256 && tu.hsplit <= 1 && tu.chunk_tokens <= 0 && (tu.gather == 0 || tu.gather == 2) && tmap_encoder()) {
+        const int cg_full = chunk_granularity(d->block_size, 16);
+        const int64_t tokB = (int64_t)m.kv_heads * rowB;                         // one token, all heads, one tensor
+        const int64_t target = tu.tile_bytes > 0 ? tu.tile_bytes : 4096;
+        const int ct = chunk_granularity(cg_full, (int)(target / tokB > 1 ? target / tokB : 1));
+        if (tokB * ct <= 32768) { P.tmajor = 1; P.ct = ct; }
+      }
+    }
     // GATHER mode (kvr_ring.cu): dense token-major (NHD) pool, several heads, power-of-two rows, not in place:
     // a tile = all heads x cg tokens with K (and V) <= 16 KB each, so that a token's H*D destination row is written
     // by one warp in one burst.  tuning.gather: 0 auto (on), 1 on, 2 off.
     P.gather = 0;
-    {
+    if (!P.tmajor) {
       const int64_t rowB = (int64_t)m.head_dim * E;
       const bool pow2_row = rowB >= 32 && rowB <= 1024 && (rowB & (rowB - 1)) == 0 && m.rotary_offset == 0;
       const bool dense_nhd = d->stride_head == m.head_dim && d->stride_token == (int64_t)m.kv_heads * m.head_dim;
@@ -427,12 +512,37 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       cg_limit = cg_limit < 1 ? 1 : (cg_limit > 16 ? 16 : cg_limit);
     }
     decompose(chunk_granularity(d->block_size, cg_limit), tu.layers_per_unit, tu.hsplit, true);
-    const RingConfig rc0{tu.ctas_per_sm, tu.consumer_warps, tu.stages, tu.v_bulk_store, tu.max_ctas, tu.grab, tu.pdl, tu.warps_per_stage};
+    const RingConfig rc0{tu.ctas_per_sm, tu.consumer_warps, tu.stages, tu.v_bulk_store, tu.max_ctas, tu.grab, tu.pdl, tu.warps_per_stage,
+                         tu.lanes_over_heads, nullptr};
     bool ok = ring_supported(P, host_descs, rc0, c->sm_count, &why);
+    if (ok && P.tmajor) {
+      // one tensor map per source tensor; the token extent is the segment's length, so a box that runs past the last
+      // row is zero-filled instead of reading past the source allocation
+      TmapPair* maps = tmaps_inline.m;
+      if (!inline_descs) {
+        st = slot_reserve_tmaps(c, *slot_p, (size_t)n);
+        if (st != KVR_OK) return st;
+        maps = slot_p->tm_host;
+      }
+      bool enc_ok = true;
+      for (int32_t i = 0; i < n && enc_ok; ++i) {
+        const SegDev& o = host_descs[i];
+        enc_ok = encode_source_map(&maps[i].k, o.k_src, m.dtype, m.head_dim, m.kv_heads, o.len, m.layers, o.sl, o.sh, o.st, P.ct);
+        if (enc_ok && o.v_src && !P.no_v)
+          enc_ok = encode_source_map(&maps[i].v, o.v_src, m.dtype, m.head_dim, m.kv_heads, o.len, m.layers, o.sl, o.sh, o.st, P.ct);
+      }
+      if (!enc_ok) continue;                 // plan again without transposing loads
+      use_tmaps = true;
+      if (!inline_descs) P.tmaps = slot_p->tm_dev;
+    } else if (!ok && P.tmajor) {
+      continue;                              // e.g. the layout does not fit: plan again without transposing loads
+    }
     if (!ok && path == 2) { c->last_err = std::string("ring kernel unsupported: ") + (why ? why : ""); return KVR_ERR_UNSUPPORTED; }
     path = ok ? 2 : 1;
+    break;
   }
   if (path == 1) {
+    P.tmajor = 0; P.ct = 0; P.tmaps = nullptr; P.gather = 0;
     // generic kernel: chunk table [cg][R/2] float4 must fit 48 KB of static-limit shared memory
     int limit = (int)(47 * 1024 / ((m.rotary_dim / 2) * 16 + 4));
     if (limit < 1) return KVR_ERR_UNSUPPORTED;
@@ -443,10 +553,13 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     for (int32_t i = 0; i < n; ++i) P.inline_segs[i] = host_descs[i];   // descriptors ride in the kernel parameters
   } else {
     KVR_CUDA(c, cudaMemcpyAsync(slot_p->dev, slot_p->host, (size_t)n * sizeof(SegDev), cudaMemcpyHostToDevice, stream));
+    if (use_tmaps && path == 2)
+      KVR_CUDA(c, cudaMemcpyAsync(slot_p->tm_dev, slot_p->tm_host, (size_t)n * sizeof(TmapPair), cudaMemcpyHostToDevice, stream));
   }
   cudaError_t e;
   if (path == 2) {
-    RingConfig rc{tu.ctas_per_sm, tu.consumer_warps, tu.stages, tu.v_bulk_store, tu.max_ctas, tu.grab, tu.pdl, tu.warps_per_stage};
+    RingConfig rc{tu.ctas_per_sm, tu.consumer_warps, tu.stages, tu.v_bulk_store, tu.max_ctas, tu.grab, tu.pdl, tu.warps_per_stage,
+                  tu.lanes_over_heads, (use_tmaps && inline_descs) ? &tmaps_inline : nullptr};
     e = launch_ring(P, rc, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
   } else {
     e = launch_generic(P, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);

@@ -14,6 +14,7 @@
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <cuda_fp8.h>
+#include <cuda.h>            // CUtensorMap (type only; the encoder is fetched through cudaGetDriverEntryPoint)
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -35,6 +36,12 @@ struct SegDev {
 };
 
 constexpr int kInlineSegs = 8;    // calls with <= this many segments carry their descriptors in the kernel parameters
+
+// TRANSPOSING loads (ring kernel, dense token-major pools): one TMA tensor map per source tensor, dims ordered
+// (dim, head, token, layer) -- the head stride is larger than the token stride, which the encoder accepts -- so that a box
+// of {head_dim, heads, ct tokens, 1} lands in shared memory as [token][head][dim], i.e. in the pool's own order.
+struct TmapPair { CUtensorMap k, v; };
+struct TmapInline { TmapPair m[kInlineSegs]; };
 
 struct CallParams {
   // model
@@ -68,6 +75,9 @@ struct CallParams {
   int32_t gather;              // ring kernel: gather mode (dense token-major pool; a tile = all heads of a few tokens)
   int32_t no_v;                // V is neither read nor written (in-place calls; K-only [latent | k_pe] caches)
   int32_t inplace;             // kvr_reposition_inplace: K rows are read from the pool slot they are written back to; no V
+  int32_t tmajor;              // ring kernel: transposing tensor loads, tiles of ALL heads x ct tokens (see TmapPair)
+  int32_t ct;                  // tmajor: tokens per tile (divides cg)
+  const TmapPair* tmaps;       // tmajor, > kInlineSegs segments: DEVICE array [n_segs]
   SegDev inline_segs[kInlineSegs];
 };
 
@@ -174,7 +184,8 @@ __device__ __forceinline__ uint32_t f32x2_to_e4m3x2_sat(float lo, float hi) {
 cudaError_t launch_generic(const CallParams& P, int sm_count, cudaStream_t stream, int* grid, int* block, int* smem);
 
 struct RingConfig {
-  int ctas_per_sm, consumer_warps, stages, v_bulk_store, max_ctas, grab, pdl, warps_per_stage;
+  int ctas_per_sm, consumer_warps, stages, v_bulk_store, max_ctas, grab, pdl, warps_per_stage, lanes_over_heads;
+  const TmapInline* tmaps_inline;   // HOST pointer: tensor maps of a call with <= kInlineSegs segments (tmajor mode)
 };
 int ring_heads_per_tile(const CallParams& P);   // heads one tile of the ring kernel covers (needs P.cg)
 bool ring_window_mode(const CallParams& P);      // rows outside the power-of-two slot layout (e.g. MLA [latent | k_pe])

@@ -54,6 +54,12 @@ struct RingParams {
                                           // wpg consumer warps share it, each taking whole token rows, tokens outer / heads
                                           // inner, so that a token's H*D row reaches L2 (and DRAM) as one contiguous burst
                                           // instead of H pieces written by H different warps at different times; 1 otherwise
+  int hmaj;                               // gather tiles, "lanes over heads": a warp pass covers rpi HEADS of one token (their
+                                          // rows are adjacent in a dense token-major pool) instead of rpi tokens of one head,
+                                          // so every warp store instruction writes one contiguous run, as on a head-major pool
+  int log_pt;                             // hmaj: log2(hpt * nv), the 16-byte vectors of one token in a tile
+  int log_hp;                             // hmaj: a pass covers 2^log_hp heads (min(hpt, rpi)) x (rpi >> log_hp) tokens
+  int ct;                                 // tmajor: tokens per tile
   int ip_mode;                            // in-place source runs: 0 one run per head (d_st == head_dim), 1 one run for the
                                           // whole tile (token-major pool, all heads in the tile), 2 one copy per row
 };
@@ -120,6 +126,14 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
   asm volatile(
       "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
       ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+}
+// global -> shared TILED tensor copy (TMA, 4-D box), completion signalled on an mbarrier
+__device__ __forceinline__ void tensor_g2s_4d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, int c3,
+                                              uint32_t bar, uint64_t pol) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+      " [%0], [%1, {%2, %3, %4, %5}], [%6], %7;"
+      ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar), "l"(pol) : "memory");
 }
 // shared -> global bulk copy (TMA, 1-D), tracked by the issuing thread's bulk async-group
 __device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src, uint32_t bytes) {
@@ -243,7 +257,8 @@ __device__ __forceinline__ void requant_fp8(uint4& A, float s_src, float inv_dst
 // MAXT = kMaxThreads: the wide shapes the tuning knobs allow (up to 16 consumer warps, or 3+ CTAs per SM).
 template <int DTYPE, int PAIRING, bool MAP, int MAXT>
 __global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1))   // 256 x 2, 448 x 1: 128 registers; 544 x 1: 96
-kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ RingParams RP) {
+kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ RingParams RP,
+                const __grid_constant__ TmapInline TI) {
   using G = Geo<DTYPE, PAIRING>;
   constexpr int E = (DTYPE == 0) ? 2 : 1;
   extern __shared__ __align__(128) unsigned char smem[];
@@ -428,9 +443,12 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
           const int l0 = lgi * P.lpu, l1 = min(P.layers, l0 + P.lpu);
           const int hg_per = hgroups / P.hsplit;
           const int kinds = RP.split ? 2 : 1;                            // split: a K tile, then a V tile
-          const int n_tiles = (l1 - l0) * hg_per * kinds;
+          const bool tmajor = P.tmajor != 0;                             // tiles = (layer, sub-chunk of ct tokens), all heads
+          const int n_sub = tmajor ? (n_tok + RP.ct - 1) / RP.ct : 1;
+          const int n_tiles = tmajor ? (l1 - l0) * n_sub : (l1 - l0) * hg_per * kinds;
           const bool inplace = P.inplace != 0;
-          const int flags = ((MAP || sg.delta != 0) ? kFlagRotate : 0) | ((inplace && RP.ip_mode == 1) ? kFlagTokMajor : 0);
+          const int flags = ((MAP || sg.delta != 0) ? kFlagRotate : 0) |
+                            (((inplace && RP.ip_mode == 1) || tmajor) ? kFlagTokMajor : 0);
           const uint32_t run_bytes = (uint32_t)(n_tok * RP.rowB);
           const bool packed_rows = (sg.st == P.head_dim);
           const int64_t dst_chunk = (int64_t)blk * P.d_sb + (int64_t)off * P.d_st;
@@ -438,7 +456,28 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
           const int pass = S < 32 ? S : 32;
           for (int tb0 = 0; tb0 < n_tiles; tb0 += pass) {
             const int n = min(pass, n_tiles - tb0);
-            if (lane < n) {
+            if (lane < n && tmajor) {
+              // transposing tensor loads: the box {head_dim, heads, ct tokens, 1 layer} of the source lands as
+              // [token][head][dim], the order of a dense token-major pool; one TMA operation per tensor and tile
+              const int t = tb0 + lane;
+              const int l = l0 + t / n_sub, tok0 = (t % n_sub) * RP.ct;
+              int my_stage = stage + lane;
+              uint32_t my_phase = phase;
+              if (my_stage >= S) { my_stage -= S; my_phase ^= 1u; }
+              const uint32_t bar = s_full + 8u * my_stage;
+              mbar_wait(s_empty + 8u * my_stage, my_phase ^ 1u, 2);
+              TileMeta m;
+              m.dst_off = (int64_t)l * P.d_sl + dst_chunk + (int64_t)tok0 * P.d_st;
+              m.n_tok = min(RP.ct, n_tok - tok0); m.tab = tb; m.gen = gen;
+              m.flags = flags | (tok0 << 8);                                   // bits 8+: first token of the tile in its chunk
+              m.scale_idx = l * P.heads; m.seg = si;
+              meta[my_stage] = m;
+              mbar_arrive_expect_tx(bar, (RP.no_v ? 1u : 2u) * (uint32_t)RP.tile_bytes);   // the whole box, zero-filled past the end
+              const uint32_t sk = s_base + RP.off_stage + (uint32_t)my_stage * RP.stage_bytes;
+              const TmapPair* tp = (P.n_segs <= kInlineSegs) ? &TI.m[si] : &P.tmaps[si];
+              tensor_g2s_4d(sk, &tp->k, 0, 0, t0 + tok0, l, bar, pol);
+              if (!RP.no_v) tensor_g2s_4d(sk + RP.tile_bytes, &tp->v, 0, 0, t0 + tok0, l, bar, pol);
+            } else if (lane < n) {
               const int t = (tb0 + lane) / kinds;
               const int kind = RP.split ? (tb0 + lane) - t * kinds : -1;      // 0: K tile, 1: V tile, -1: both
               const int l = l0 + t / hg_per, h0 = (hpart * hg_per + t % hg_per) * RP.hpt;
@@ -560,7 +599,7 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     uint4 B = lds128(ks + t * sm_st + vb * 16);
     bool rot_row = rotate;
     if (MAP) {
-      const int run = reinterpret_cast<const int32_t*>(smem + RP.off_tab + m.tab * RP.tab_stride + RP.cg * RP.half_R * 16)[t];
+      const int run = reinterpret_cast<const int32_t*>(smem + RP.off_tab + m.tab * RP.tab_stride + RP.cg * RP.half_R * 16)[t + (m.flags >> 8)];
       rot_row = run >= 0;
       if (rot_row && (rot_a || rot_b) && (run != my_run || m.gen != my_gen)) {   // cos/sin registers follow the run
         my_run = run; my_gen = m.gen;
@@ -620,6 +659,20 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     // ---- V (step a6): bytes unchanged ----
     if (RP.no_v || (m.flags & kFlagKOnly)) {
       // in-place: V is position-free and already where it belongs
+    } else if (RP.hmaj && RP.v_bulk == 0) {
+      // lanes over heads (dense token-major pool): this warp's tokens, each as ONE contiguous run of hpt * rowB
+      // destination bytes; consecutive lanes write consecutive 16-byte vectors (a warp instruction = 512 contiguous
+      // bytes), reading the head-major stage in 128-byte row pieces (conflict-free per quarter warp)
+      const int tpw = (n_tok + wpg - 1) / wpg, tk0 = wsub * tpw, tk1 = min(n_tok, tk0 + tpw);
+      const int total = (tk1 - tk0) << RP.log_pt;
+      uint8_t* const vd = P.v_cache + (m.dst_off + (int64_t)tk0 * P.d_st) * E;
+      const int64_t tok_step = P.d_st * E - ((int64_t)RP.hpt * RP.rowB);     // gap between token runs (0: all heads in the tile)
+#pragma unroll 4
+      for (int idx = lane; idx < total; idx += 32) {
+        const int tt = idx >> RP.log_pt, rem = idx & ((1 << RP.log_pt) - 1);
+        const int hh = rem >> RP.log_nv, v = rem & (nv - 1);
+        stg128(vd + (int64_t)idx * 16 + tt * tok_step, lds128(sv + (hh * RP.cg + tk0 + tt) * RP.rowB + v * 16));
+      }
     } else if (RP.gather) {
       // gather mode: this warp's tokens leave by one bulk (TMA) store per (token, head) row, heads innermost, so the
       // rows of a token arrive back to back and form one contiguous H*D run of the dense token-major pool
@@ -656,8 +709,11 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       bulk_commit();
     } else if (RP.v_bulk) {
       if (lane == 0) {
-        for (int hh = 0; hh < RP.hpt; ++hh)
-          bulk_s2g(P.v_cache + (m.dst_off + (int64_t)hh * P.d_sh) * E, sv + hh * RP.cg * RP.rowB, (uint32_t)(n_tok * RP.rowB));
+        if (m.flags & kFlagTokMajor)       // the stage is in the pool's order: the tile's V is ONE contiguous run
+          bulk_s2g(P.v_cache + m.dst_off * E, sv, (uint32_t)(n_tok * RP.hpt * RP.rowB));
+        else
+          for (int hh = 0; hh < RP.hpt; ++hh)
+            bulk_s2g(P.v_cache + (m.dst_off + (int64_t)hh * P.d_sh) * E, sv + hh * RP.cg * RP.rowB, (uint32_t)(n_tok * RP.rowB));
         bulk_commit();
       }
     } else {
@@ -691,6 +747,31 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     const int sm_st = (m.flags & kFlagTokMajor) ? RP.hpt * RP.rowB : RP.rowB;
     if (m.flags & kFlagVOnly) {
       // split gather tile holding V alone: nothing to rotate
+    } else if (RP.hmaj) {
+      // lanes over heads: a pass of the warp covers 2^log_hp adjacent HEADS of (rpi >> log_hp) tokens, so its rows are
+      // adjacent in a dense token-major pool and a pair of warp store instructions writes contiguous runs, as on a
+      // head-major pool.  Items = (token group, head group), token group major; warp wsub of the wpg warps that share
+      // the stage takes a contiguous range of them.
+      const int log_hp = RP.log_hp, log_tp = RP.log_rpi - log_hp;
+      const int hgs = RP.hpt >> log_hp, tgs = (n_tok + (1 << log_tp) - 1) >> log_tp;
+      const int items = tgs * hgs, ipw = (items + wpg - 1) / wpg;
+      const int it0 = wsub * ipw, it1 = min(items, it0 + ipw);
+      const int hsub = rsub & ((1 << log_hp) - 1), tsub = rsub >> log_hp;
+      int tg = it0 / hgs, g = it0 - tg * hgs;
+      uint8_t* const kd0 = P.k_cache + m.dst_off * E;
+      const int64_t kd_step = P.d_sh * E;
+      float s_src = 1.0f, inv_dst = 1.0f; bool requant = false;
+      int hh = (g << log_hp) + hsub;
+      if (DTYPE == 1) head_scales(m, hh, s_src, inv_dst, requant);
+      for (int it = it0; it < it1; ++it) {
+        const int t = (tg << log_tp) + tsub;
+        if (t < n_tok) k_row(m, tab, rotate, sk + hh * sm_sh, kd0 + hh * kd_step, t, sm_st, s_src, inv_dst, requant);
+        if (++g == hgs) { g = 0; ++tg; }
+        if (hgs > 1) {
+          hh = (g << log_hp) + hsub;
+          if (DTYPE == 1) head_scales(m, hh, s_src, inv_dst, requant);
+        }
+      }
     } else if (RP.gather) {
       // gather mode: tokens outer, heads inner -- a pass of this warp completes rpi whole token rows
       // (token group, head) items of this warp, token group major; the walk keeps running pointers (no divisions)
@@ -749,6 +830,7 @@ static int ilog2(int x) { int l = 0; while ((1 << l) < x) ++l; return l; }
 // takes all heads (its tile is then one contiguous run of the pool)
 int ring_heads_per_tile(const CallParams& P) {
   const int rowB = P.head_dim * (P.dtype == 0 ? 2 : 1);
+  if (P.tmajor) return P.heads;        // transposing loads: a tile is all heads x ct tokens
   if (P.inplace && P.d_st != P.head_dim && P.d_sh == P.head_dim && P.d_st == (int64_t)P.heads * P.head_dim) return P.heads;
   for (int h = 1; h <= P.heads; ++h)
     if (P.heads % h == 0 && h * P.cg * rowB >= (P.tile_min_bytes > 0 ? P.tile_min_bytes : 4096)) return h;
@@ -791,7 +873,8 @@ bool ring_supported(const CallParams& P, const SegDev* segs, const RingConfig& c
 }
 
 template <int DTYPE, int PAIRING, bool MAP, int MAXT>
-static cudaError_t launch_inst(const CallParams& P, const RingParams& RP, int grid, int block, int smem, cudaStream_t st, bool pdl) {
+static cudaError_t launch_inst(const CallParams& P, const RingParams& RP, const TmapInline& TI, int grid, int block, int smem,
+                               cudaStream_t st, bool pdl) {
   // The opt-in to > 48 KB of dynamic shared memory is a per-DEVICE attribute of the function: remember what was set per
   // (instantiation, device), under a lock (contexts on several devices / host threads share this process-wide table).
   static std::mutex mu;
@@ -813,7 +896,7 @@ static cudaError_t launch_inst(const CallParams& P, const RingParams& RP, int gr
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = at; lc.numAttrs = pdl ? 1 : 0;
-  return cudaLaunchKernelEx(&lc, kvr_ring_kernel<DTYPE, PAIRING, MAP, MAXT>, P, RP);
+  return cudaLaunchKernelEx(&lc, kvr_ring_kernel<DTYPE, PAIRING, MAP, MAXT>, P, RP, TI);
 }
 
 // Launch shape and shared-memory layout of one call; false when even the shortest ring does not fit.
@@ -843,8 +926,9 @@ static bool ring_plan(const CallParams& P_in, const RingConfig& cfg, int sm_coun
   }
   const int hpt = ring_heads_per_tile(P);
   RP.hpt = hpt;
-  RP.tile_bytes = hpt * RP.cg * RP.rowB;
-  RP.split = (P.gather == 2 && !RP.no_v) ? 1 : 0;
+  RP.ct = P.tmajor ? P.ct : RP.cg;
+  RP.tile_bytes = hpt * RP.ct * RP.rowB;
+  RP.split = (P.gather == 2 && !RP.no_v && !P.tmajor) ? 1 : 0;
   RP.stage_bytes = ((RP.no_v || RP.split) ? 1 : 2) * RP.tile_bytes;
   const int ctas = cfg.ctas_per_sm > 0 ? cfg.ctas_per_sm : 2;
   RP.NW = cfg.consumer_warps > 0 ? cfg.consumer_warps : 6;
@@ -871,7 +955,7 @@ static bool ring_plan(const CallParams& P_in, const RingConfig& cfg, int sm_coun
   // Stage ownership: consumer warp w serves stages (w / wpg) + k * (NW / wpg); S is a multiple of NW / wpg, so the
   // successive phases of one mbarrier are ordered by one warp's program order (a warp two phases ahead would pass a
   // parity wait early).  wpg > 1 only in gather mode, when the ring holds fewer (large) stages than consumer warps.
-  RP.gather = P.gather ? 1 : 0;
+  RP.gather = (P.gather && !P.tmajor) ? 1 : 0;
   RP.wpg = 1;
   if (RP.gather && (cfg.warps_per_stage > 0 || S < RP.NW)) {
     // Few large stages: groups of wpg warps walk the ring in NW / wpg strides.  A group should own TWO stages (one
@@ -902,7 +986,23 @@ static bool ring_plan(const CallParams& P_in, const RingConfig& cfg, int sm_coun
   else RP.v_bulk = runs ? 1 : 0;
   if (RP.gather)   // gather mode: 2 = one bulk store per (token, head) row (default: measured faster), 0 = warp copies
     RP.v_bulk = (cfg.v_bulk_store == 2) ? 0 : (cfg.v_bulk_store == 3 || cfg.v_bulk_store == 1) ? 2 : 2;
+  if (P.tmajor) RP.v_bulk = 1;      // the stage is in the pool's order: V leaves as one bulk store per tile
   if (RP.no_v) RP.v_bulk = 0;
+  // lanes over heads (dense token-major pools): needs whole groups of min(hpt, rpi) heads per tile and a power of two
+  // of vectors per token.  tuning.lanes_over_heads: 0 auto (on in gather mode), 1 on wherever possible, 2 off.
+  RP.hmaj = 0; RP.log_pt = 0; RP.log_hp = 0;
+  {
+    const int pt = RP.hpt * RP.nv, hp = RP.hpt < RP.rpi ? RP.hpt : RP.rpi;
+    const bool can = !RP.win && !P.inplace && RP.log_nv >= 0 && hp >= 1 && (hp & (hp - 1)) == 0 && RP.hpt % hp == 0 &&
+                     (pt & (pt - 1)) == 0 && RP.hpt > 1 && P.d_sh == P.head_dim && P.d_st >= (int64_t)RP.hpt * P.head_dim;
+    if (can && (cfg.lanes_over_heads == 1 || (cfg.lanes_over_heads == 0 && (RP.gather || P.tmajor)))) {
+      RP.hmaj = 1; RP.log_pt = ilog2(pt); RP.log_hp = ilog2(hp);
+      if (P.tmajor) { /* V: one bulk store per tile (set above) */ }
+      else if (RP.no_v) RP.v_bulk = 0;
+      else if (cfg.v_bulk_store == 3 || cfg.v_bulk_store == 1) RP.v_bulk = 2;   // forced: one bulk store per row
+      else RP.v_bulk = 0;                                                        // V leaves by contiguous warp copies
+    }
+  }
   int64_t g = (int64_t)sm_count * ctas;
   if (cfg.max_ctas > 0 && g > cfg.max_ctas) g = cfg.max_ctas;
   if (g > P.total_units) g = P.total_units;
@@ -919,10 +1019,12 @@ cudaError_t launch_ring(const CallParams& P_in, const RingConfig& cfg, int sm_co
   const int ctas = cfg.ctas_per_sm > 0 ? cfg.ctas_per_sm : 2;
   const bool map = P.any_pos_map != 0;
   const bool small = block <= 256 && ctas <= 2, mid = block <= 448 && ctas == 1;
+  static const TmapInline no_maps{};
+  const TmapInline& TI = (P.tmajor && cfg.tmaps_inline) ? *cfg.tmaps_inline : no_maps;
 #define KVR_LAUNCH(D, PR, M)                                                                             \
-  return small ? launch_inst<D, PR, M, 256>(P, RP, (int)g, block, smem, stream, cfg.pdl != 2)            \
-         : mid ? launch_inst<D, PR, M, 448>(P, RP, (int)g, block, smem, stream, cfg.pdl != 2)            \
-               : launch_inst<D, PR, M, kMaxThreads>(P, RP, (int)g, block, smem, stream, cfg.pdl != 2)
+  return small ? launch_inst<D, PR, M, 256>(P, RP, TI, (int)g, block, smem, stream, cfg.pdl != 2)            \
+         : mid ? launch_inst<D, PR, M, 448>(P, RP, TI, (int)g, block, smem, stream, cfg.pdl != 2)            \
+               : launch_inst<D, PR, M, kMaxThreads>(P, RP, TI, (int)g, block, smem, stream, cfg.pdl != 2)
   if (P.dtype == 0) {
     if (P.pairing == 0) { if (map) KVR_LAUNCH(0, 0, true); else KVR_LAUNCH(0, 0, false); }
     else { if (map) KVR_LAUNCH(0, 1, true); else KVR_LAUNCH(0, 1, false); }

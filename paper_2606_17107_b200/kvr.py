@@ -50,7 +50,7 @@ class kvr_tuning(C.Structure):
                 ("stages", C.c_int32), ("layers_per_unit", C.c_int32), ("v_bulk_store", C.c_int32),
                 ("max_ctas", C.c_int32), ("grab", C.c_int32), ("pdl", C.c_int32), ("hsplit", C.c_int32),
                 ("chunk_tokens", C.c_int32), ("tile_bytes", C.c_int32), ("gather", C.c_int32),
-                ("warps_per_stage", C.c_int32), ("reserved", C.c_int32 * 2)]
+                ("warps_per_stage", C.c_int32), ("lanes_over_heads", C.c_int32), ("transpose_load", C.c_int32)]
 
 
 class kvr_resident_span(C.Structure):

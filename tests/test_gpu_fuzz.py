@@ -63,6 +63,11 @@ def _random_case(seed):
             tuning["gather"] = int(rng.choice([1, 3]))
         if rng.random() < 0.3:
             tuning["grab"] = int(rng.integers(1, 5))
+    rng2 = np.random.default_rng(5000 + seed)          # drawn from a stream of its own: the cases above stay as they were
+    if rng2.random() < 0.4 and "gather" not in tuning:
+        tuning["transpose_load"] = 1                   # ignored by the library where the pool is not dense token-major
+        if rng2.random() < 0.5:
+            tuning["tile_bytes"] = int(rng2.choice([512, 2048, 8192]))
     return w, tuning
 
 

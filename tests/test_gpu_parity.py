@@ -362,6 +362,15 @@ def test_time_is_linear_in_tokens():
                                     dict(gather=1, warps_per_stage=6), dict(gather=3, warps_per_stage=4, consumer_warps=4),
                                     dict(gather=1, warps_per_stage=3, consumer_warps=12, ctas_per_sm=1, max_ctas=2),
                                     dict(gather=3), dict(gather=3, max_ctas=2, stages=2, consumer_warps=4),
+                                    dict(gather=1, lanes_over_heads=2), dict(gather=3, lanes_over_heads=2),
+                                    dict(gather=2, lanes_over_heads=1), dict(gather=2, lanes_over_heads=1, tile_bytes=8192),
+                                    dict(gather=2, lanes_over_heads=1, tile_bytes=16384, max_ctas=3),
+                                    dict(gather=2, lanes_over_heads=1, tile_bytes=32768, ctas_per_sm=1),
+                                    dict(gather=1, lanes_over_heads=1, v_bulk_store=3),
+                                    dict(transpose_load=1), dict(transpose_load=1, tile_bytes=8192),
+                                    dict(transpose_load=1, tile_bytes=1024, max_ctas=2, stages=2, consumer_warps=3),
+                                    dict(transpose_load=1, lanes_over_heads=2, max_ctas=3, stages=5),
+                                    dict(transpose_load=1, tile_bytes=16384, ctas_per_sm=1, consumer_warps=12),
                                     dict(gather=3, max_ctas=3, stages=5, consumer_warps=10, ctas_per_sm=1)])
 @pytest.mark.parametrize("c", [0, 1, 2, 3, 4])
 def test_gather_mode(c, tuning):
@@ -378,6 +387,10 @@ def test_gather_mode_ragged_blocks(bs, heads, D, dtype):
                                     [dict(len=77, dst_token_start=1, new_start=9)]])
     check_parity(w, "ring", gather=1)
     check_parity(w, "ring", gather=3)
+    check_parity(w, "ring", gather=2, lanes_over_heads=1, tile_bytes=8192)     # lanes over heads on ordinary tiles
+    check_parity(w, "ring", gather=1, lanes_over_heads=2)
+    check_parity(w, "ring", transpose_load=1)                                     # transposing tensor loads
+    check_parity(w, "ring", transpose_load=1, tile_bytes=2048, max_ctas=2, stages=3)
 
 
 @pytest.mark.parametrize("path", ["generic", "ring"])
@@ -534,6 +547,8 @@ def test_last_block_of_the_pool_and_last_row_of_the_source(dtype, layout):
     for path in ("ring", "generic"):
         check_parity(w, path)          # _gpu() asserts the canaries around pools, sources and tables
     check_parity(w, "ring", gather=2)
+    if layout == "NHD":
+        check_parity(w, "ring", transpose_load=1)      # boxes that run past the last source row are zero-filled
 
 
 def test_pre_rope_chunk_at_a_shift_near_2_to_the_30():
@@ -569,3 +584,35 @@ def test_contexts_on_two_devices_in_one_process():
             torch.cuda.synchronize(dev)
             assert np.array_equal(np_bits(dw.v_cache), vc)
             assert k_distance(w, np_bits(dw.k_cache), kc).max() <= K_TOL[w.dtype]
+
+
+@pytest.mark.parametrize("dtype", ["bf16", "fp8"])
+def test_transposing_loads_many_segments_maps_and_fresh_suffix(dtype):
+    """Transposing tensor loads (tuning.transpose_load = 1) with more than 8 segments (tensor maps staged in device
+    memory), a position map with Delta = 0 tokens, a pre-RoPE suffix, padded source rows and two sequences."""
+    pm = pos_map_with_gaps(90, 700, 0.25, 32, 9)
+    pm[:3] = np.arange(3) + 11
+    pad = 8 if dtype == "bf16" else 16
+    lst, at = [], 2
+    for i in range(10):
+        lst.append(dict(len=9 + 5 * i, dst_token_start=at, new_start=300 + 91 * i, old_start=7 * i,
+                        src_row_pad=pad if i % 3 == 0 else 0))
+        at += 9 + 5 * i + (i % 2)
+    w = make_workload(name="tl-many", layers=3, kv_heads=4, head_dim=128, theta=1e6, block_size=16, seed=77, dtype=dtype,
+                      scales_differ=(dtype == "fp8"),
+                      seq_segments=[lst, [dict(len=90, dst_token_start=13, new_start=700, old_start=11, pos_map=pm),
+                                          dict(len=40, dst_token_start=103, new_start=900, pre_rope=True)]])
+    check_parity(w, "ring", transpose_load=1)
+    check_parity(w, "ring", transpose_load=1, tile_bytes=1024, max_ctas=2, stages=4, consumer_warps=2)
+
+
+@pytest.mark.parametrize("heads,D,dtype,pairing,R", [(2, 64, "bf16", "gptj", 32), (6, 128, "bf16", "neox", 128),
+                                                      (16, 64, "fp8", "neox", 64), (3, 256, "fp8", "gptj", 128),
+                                                      (8, 32, "bf16", "neox", 32)])
+def test_transposing_loads_shapes(heads, D, dtype, pairing, R):
+    """Head counts that are not a power of two take the transposed stage without lanes-over-heads; small rows."""
+    w = make_workload(name="tl-shapes", layers=2, kv_heads=heads, head_dim=D, rotary_dim=R, pairing=pairing, dtype=dtype,
+                      theta=1e4, block_size=8, seed=78,
+                      seq_segments=[[dict(len=61, dst_token_start=3, new_start=1234), dict(len=1, dst_token_start=70)],
+                                    [dict(len=24, dst_token_start=8, new_start=0)]])
+    check_parity(w, "ring", transpose_load=1)
