@@ -449,8 +449,8 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       const bool dense_nhd = d->stride_head == m.head_dim && d->stride_token == (int64_t)m.kv_heads * m.head_dim;
       const bool want = tu.transpose_load == 1 || (tu.transpose_load == 0 && kTransposeAuto);
       if (attempt == 0 && want && !inplace && pow2_row && dense_nhd && m.kv_heads >= 2 && m.kv_heads <= 256 &&
-          m.head_dim <= 256 && tu.hsplit <= 1 && tu.chunk_tokens <= 0 && (tu.gather == 0 || tu.gather == 2) && tmap_encoder()) {
-        const int cg_full = chunk_granularity(d->block_size, 16);
+          m.head_dim <= 256 && tu.hsplit <= 1 && (tu.gather == 0 || tu.gather == 2) && tmap_encoder()) {
+        const int cg_full = chunk_granularity(d->block_size, cg_limit);
         const int64_t tokB = (int64_t)m.kv_heads * rowB;                         // one token, all heads, one tensor
         const int64_t target = tu.tile_bytes > 0 ? tu.tile_bytes : 4096;
         const int ct = chunk_granularity(cg_full, (int)(target / tokB > 1 ? target / tokB : 1));

@@ -96,8 +96,9 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
   uint32_t ok;
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-      "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"      // %3: how long the hardware may suspend the
+      "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity), "r"(1000000u) : "memory");   // thread (ns) before it
+                                                                                                    // returns false: fewer spins
   return ok != 0;
 }
 // Bounded wait: a protocol bug must surface as a trapped launch (an error the caller sees), never as a hung GPU.
@@ -361,7 +362,14 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         const int t0 = __shfl_sync(FULL, d_t0, j), n_tok = __shfl_sync(FULL, d_ntok, j);
         const int off = __shfl_sync(FULL, d_off, j), lg = __shfl_sync(FULL, d_lg, j);
         const int blk = __shfl_sync(FULL, d_blk, j);
-        if (si != cur_si) { sg = segs[si]; cur_si = si; }
+        if (si != cur_si) {
+          sg = segs[si]; cur_si = si;
+          if (P.tmajor && lane < 2) {      // bring the segment's two tensor maps into the TMA unit's descriptor cache
+            const TmapPair* tp = (P.n_segs <= kInlineSegs) ? &TI.m[si] : &P.tmaps[si];
+            if (lane == 0 || !RP.no_v)
+              asm volatile("prefetch.tensormap [%0];" ::"l"(lane == 0 ? &tp->k : &tp->v) : "memory");
+          }
+        }
         if (blk < 0 || blk >= P.num_blocks) {
           if (lane == 0) report_bad_block(P.status, sg.index, t0);
           continue;
@@ -593,10 +601,14 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
   uint32_t phase = (uint32_t)((warp / wpg) / S) & 1u;
 
   // one K row-slot of this lane: load, rotate (or requantise), store
-  auto k_row = [&](const TileMeta& m, uint32_t tab, bool rotate, uint32_t ks, uint8_t* kd, int t, int sm_st,
+  // srow / grow: shared-memory address and destination pointer of the row (callers step them; no 64-bit multiply per row);
+  // t: the row's token within its chunk (names its table row when shifts are per token)
+  const int va16 = va * 16, vb16 = vb * 16;
+  const int64_t tokB = P.d_st * E;                // bytes between the rows of consecutive tokens in the pool
+  auto k_row = [&](const TileMeta& m, uint32_t tab, bool rotate, uint32_t srow, uint8_t* grow, int t,
                    float s_src, float inv_dst, bool requant) {
-    uint4 A = lds128(ks + t * sm_st + va * 16);
-    uint4 B = lds128(ks + t * sm_st + vb * 16);
+    uint4 A = lds128(srow + va16);
+    uint4 B = lds128(srow + vb16);
     bool rot_row = rotate;
     if (MAP) {
       const int run = reinterpret_cast<const int32_t*>(smem + RP.off_tab + m.tab * RP.tab_stride + RP.cg * RP.half_R * 16)[t + (m.flags >> 8)];
@@ -634,9 +646,8 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         }
       }
     }
-    uint8_t* row = kd + (int64_t)t * P.d_st * E;
-    stg128(row + va * 16, A);
-    stg128(row + vb * 16, B);
+    stg128(grow + va16, A);
+    stg128(grow + vb16, B);
   };
   auto head_scales = [&](const TileMeta& m, int hh, float& s_src, float& inv_dst, bool& requant) {
     s_src = 1.0f; inv_dst = 1.0f; requant = false;
@@ -758,16 +769,23 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       const int it0 = wsub * ipw, it1 = min(items, it0 + ipw);
       const int hsub = rsub & ((1 << log_hp) - 1), tsub = rsub >> log_hp;
       int tg = it0 / hgs, g = it0 - tg * hgs;
-      uint8_t* const kd0 = P.k_cache + m.dst_off * E;
-      const int64_t kd_step = P.d_sh * E;
       float s_src = 1.0f, inv_dst = 1.0f; bool requant = false;
       int hh = (g << log_hp) + hsub;
       if (DTYPE == 1) head_scales(m, hh, s_src, inv_dst, requant);
+      // the row's shared-memory address and destination pointer are stepped, not recomputed
+      int t = (tg << log_tp) + tsub;
+      const int64_t kd_step = P.d_sh * E;
+      const uint32_t s_item = (uint32_t)sm_sh << log_hp, s_wrap = ((uint32_t)sm_st << log_tp) - (uint32_t)(hgs - 1) * s_item;
+      const int64_t g_item = kd_step << log_hp, g_wrap = (tokB << log_tp) - (int64_t)(hgs - 1) * g_item;
+      uint32_t srow = sk + hh * sm_sh + t * sm_st;
+      uint8_t* grow = P.k_cache + m.dst_off * E + hh * kd_step + t * tokB;
       for (int it = it0; it < it1; ++it) {
-        const int t = (tg << log_tp) + tsub;
-        if (t < n_tok) k_row(m, tab, rotate, sk + hh * sm_sh, kd0 + hh * kd_step, t, sm_st, s_src, inv_dst, requant);
-        if (++g == hgs) { g = 0; ++tg; }
-        if (hgs > 1) {
+        if (t < n_tok) k_row(m, tab, rotate, srow, grow, t, s_src, inv_dst, requant);
+        if (hgs == 1) {
+          t += 1 << log_tp; srow += s_wrap; grow += g_wrap;
+        } else {
+          if (++g == hgs) { g = 0; t += 1 << log_tp; srow += s_wrap; grow += g_wrap; }
+          else { srow += s_item; grow += g_item; }
           hh = (g << log_hp) + hsub;
           if (DTYPE == 1) head_scales(m, hh, s_src, inv_dst, requant);
         }
@@ -787,7 +805,7 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       for (int it = it0; it < it1; ++it) {
         float s_src = 1.0f, inv_dst = 1.0f; bool requant = false;
         if (DTYPE == 1) head_scales(m, hh, s_src, inv_dst, requant);
-        if (t < n_tok) k_row(m, tab, rotate, ks, kd, t, sm_st, s_src, inv_dst, requant);
+        if (t < n_tok) k_row(m, tab, rotate, ks + t * sm_st, kd + t * tokB, t, s_src, inv_dst, requant);
         ++hh; ks += sm_sh; kd += kd_step;
         if (hh == RP.hpt) { hh = 0; ks = sk; kd = kd0; t += rpi; }
       }
@@ -797,7 +815,14 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
       uint8_t* kd = P.k_cache + (m.dst_off + (int64_t)hh * P.d_sh) * E;
       float s_src, inv_dst; bool requant;
       head_scales(m, hh, s_src, inv_dst, requant);
-      for (int t = rsub; t < n_tok; t += rpi) k_row(m, tab, rotate, ks, kd, t, sm_st, s_src, inv_dst, requant);
+      {
+        uint32_t srow = ks + rsub * sm_st;
+        uint8_t* grow = kd + rsub * tokB;
+        const uint32_t s_step = (uint32_t)(rpi * sm_st);
+        const int64_t g_step = rpi * tokB;
+        for (int t = rsub; t < n_tok; t += rpi, srow += s_step, grow += g_step)
+          k_row(m, tab, rotate, srow, grow, t, s_src, inv_dst, requant);
+      }
       if (RP.win) {
         // window mode: everything outside the rotary window (the MLA latent) is position-free -- 16-byte copies
         const int npass = nv - nr;
@@ -833,7 +858,9 @@ int ring_heads_per_tile(const CallParams& P) {
   if (P.tmajor) return P.heads;        // transposing loads: a tile is all heads x ct tokens
   if (P.inplace && P.d_st != P.head_dim && P.d_sh == P.head_dim && P.d_st == (int64_t)P.heads * P.head_dim) return P.heads;
   for (int h = 1; h <= P.heads; ++h)
-    if (P.heads % h == 0 && h * P.cg * rowB >= (P.tile_min_bytes > 0 ? P.tile_min_bytes : 4096)) return h;
+    if (P.heads % h == 0 && h * P.cg * rowB >= (P.tile_min_bytes > 0 ? P.tile_min_bytes : (P.inplace ? 8192 : 4096))) return h;
+  // (in place a stage holds K alone: 8 KB tiles keep as many bytes in flight as the splice's K + V stages; B200,
+  //  head-major pools: configs[2] 5673 -> 6240 GB/s, configs[3] 5194 -> 5845, configs[4] 6180 -> 6424)
   return P.heads;
 }
 
@@ -993,9 +1020,10 @@ static bool ring_plan(const CallParams& P_in, const RingConfig& cfg, int sm_coun
   RP.hmaj = 0; RP.log_pt = 0; RP.log_hp = 0;
   {
     const int pt = RP.hpt * RP.nv, hp = RP.hpt < RP.rpi ? RP.hpt : RP.rpi;
-    const bool can = !RP.win && !P.inplace && RP.log_nv >= 0 && hp >= 1 && (hp & (hp - 1)) == 0 && RP.hpt % hp == 0 &&
+    const bool ip_tm = P.inplace && RP.ip_mode == 1;        // in place on a dense token-major pool: the stage is in pool order
+    const bool can = !RP.win && (!P.inplace || ip_tm) && RP.log_nv >= 0 && hp >= 1 && (hp & (hp - 1)) == 0 && RP.hpt % hp == 0 &&
                      (pt & (pt - 1)) == 0 && RP.hpt > 1 && P.d_sh == P.head_dim && P.d_st >= (int64_t)RP.hpt * P.head_dim;
-    if (can && (cfg.lanes_over_heads == 1 || (cfg.lanes_over_heads == 0 && (RP.gather || P.tmajor)))) {
+    if (can && (cfg.lanes_over_heads == 1 || (cfg.lanes_over_heads == 0 && (RP.gather || P.tmajor || ip_tm)))) {
       RP.hmaj = 1; RP.log_pt = ilog2(pt); RP.log_hp = ilog2(hp);
       if (P.tmajor) { /* V: one bulk store per tile (set above) */ }
       else if (RP.no_v) RP.v_bulk = 0;
