@@ -70,6 +70,13 @@ def lib():
             [C.c_int] * 3)                                        # control
         _lib.kvr_oracle_bytes_moved.restype = C.c_uint64
         _lib.kvr_oracle_bytes_moved.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int64]
+        _lib.kvr_oracle_rotate_on_read_attention.restype = C.c_int
+        _lib.kvr_oracle_rotate_on_read_attention.argtypes = (
+            [C.c_void_p] + [C.c_int] * 6 + [C.c_void_p, C.c_double] +     # q, shapes, inv_freq, scale
+            [C.c_int] + [C.c_void_p] * 6 +                                  # segments
+            [C.c_void_p, C.c_void_p, C.c_int])                              # o, lse, n_threads
+        _lib.kvr_oracle_attention_bytes_read.restype = C.c_uint64
+        _lib.kvr_oracle_attention_bytes_read.argtypes = [C.c_int, C.c_int, C.c_int64]
     return _lib
 
 
@@ -198,6 +205,41 @@ def reposition_inplace(*, layers, kv_heads, head_dim, rotary_dim, pairing, dtype
 
 def bytes_moved(layers, kv_heads, head_dim, dtype, tokens):
     return int(lib().kvr_oracle_bytes_moved(layers, kv_heads, head_dim, dtype, tokens))
+
+
+def rotate_on_read_attention(*, q, kv_heads, rotary_dim, pairing, inv_freq, scale, segments, rotary_offset=0,
+                             n_threads=1):
+    """kvr_oracle_rotate_on_read_attention (kvr_attention_oracle.c; reading R25) for ONE request at ONE layer.
+    q: uint16 [q_heads, head_dim] bf16 bits (post-RoPE at the query's position).  segments: list of
+    (k_bits, v_bits, delta) with k_bits / v_bits uint16 arrays [kv_heads, len, head_dim] AT THAT LAYER (any strides
+    numpy can express with head_dim contiguous).  Returns (o float64 [q_heads, head_dim], lse float64 [q_heads])."""
+    q = np.ascontiguousarray(q, dtype=np.uint16)
+    q_heads, head_dim = q.shape
+    inv_freq = np.ascontiguousarray(inv_freq, dtype=np.float64)
+    assert inv_freq.shape == (rotary_dim // 2,)
+    n = len(segments)
+    keep, kp, vp = [], (C.c_void_p * n)(), (C.c_void_p * n)()
+    sh, st = np.empty(n, np.int64), np.empty(n, np.int64)
+    ln, dl = np.empty(n, np.int32), np.empty(n, np.int32)
+    for i, (k, v, delta) in enumerate(segments):
+        assert k.dtype == np.uint16 and v.dtype == np.uint16 and k.shape == v.shape and k.shape[0] == kv_heads
+        assert k.shape[2] == head_dim and k.strides[2] == 2 and v.strides == k.strides, (k.shape, k.strides, v.strides)
+        keep.append((k, v))
+        kp[i], vp[i] = k.ctypes.data, v.ctypes.data
+        sh[i], st[i], ln[i], dl[i] = k.strides[0] // 2, k.strides[1] // 2, k.shape[1], delta
+    o = np.empty((q_heads, head_dim), np.float64)
+    lse = np.empty(q_heads, np.float64)
+    status = lib().kvr_oracle_rotate_on_read_attention(
+        _ptr(q), q_heads, kv_heads, head_dim, rotary_dim, rotary_offset, pairing, _ptr(inv_freq), float(scale),
+        n, C.cast(kp, C.c_void_p), C.cast(vp, C.c_void_p), _ptr(sh), _ptr(st), _ptr(ln), _ptr(dl),
+        _ptr(o, writable=True), _ptr(lse, writable=True), n_threads)
+    if status != OK:
+        raise ValueError(f"kvr_oracle_rotate_on_read_attention -> {status}")
+    return o, lse
+
+
+def attention_bytes_read(kv_heads, head_dim, tokens):
+    return int(lib().kvr_oracle_attention_bytes_read(kv_heads, head_dim, tokens))
 
 
 def host_threads():

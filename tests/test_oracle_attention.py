@@ -1,0 +1,216 @@
+"""Pins of oracle/kvr_attention_oracle.c (rotate-on-read attention, reading R25)
+against what the paper and the mathematics fix.  None of them re-types the oracle's loop nest: the re-rotated keys
+come from a complex-exponential RoPE in numpy, the softmax-attention from torch's scaled_dot_product_attention in
+fp64 (a library routine), closed forms are worked by hand from integers.
+
+PAPER.md:131 "we re-rotate the chunk's keys from their source positions to the target positions (values are
+position-free)"; "FlashAttention, paged attention/vLLM, and GQA/MQA".
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import kvr_oracle as orc
+from tests.helpers import PAIRING, rope_direct_np
+from workloads import inv_freq_llama3, inv_freq_standard
+
+
+def bf16_bits(x):
+    """fp64/fp32 array -> bf16 bit patterns (torch's RNE cast; the codec itself is pinned in test_oracle_codecs.py)."""
+    t = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).to(torch.bfloat16)
+    return t.view(torch.int16).numpy().view(np.uint16)
+
+
+def bf16_val(bits):
+    return torch.from_numpy(bits.view(np.int16)).view(torch.bfloat16).to(torch.float64).numpy()
+
+
+def rope_complex(k, delta, inv_freq, R, pairing, offset=0):
+    """Independent re-rotation: pair (a, b) as the complex number a + ib, multiplied by exp(i * delta * inv_freq)."""
+    k = np.array(k, dtype=np.float64)
+    h = R // 2
+    if pairing == "neox":
+        ia, ib = offset + np.arange(h), offset + h + np.arange(h)
+    else:
+        ia, ib = offset + 2 * np.arange(h), offset + 2 * np.arange(h) + 1
+    z = (k[..., ia] + 1j * k[..., ib]) * np.exp(1j * float(delta) * np.asarray(inv_freq, dtype=np.float64))
+    out = k.copy()
+    out[..., ia], out[..., ib] = z.real, z.imag
+    return out
+
+
+def sdpa_reference(q, segs_kprime_v, kv_heads, scale):
+    """torch fp64 scaled_dot_product_attention per query head over the concatenated (already re-rotated) keys, and
+    logsumexp of the scaled scores.  q [Hq, D] float64; segs: list of (K' [Hkv, L, D], V [Hkv, L, D]) float64."""
+    Hq, D = q.shape
+    G = Hq // kv_heads
+    K = torch.from_numpy(np.concatenate([k for k, _ in segs_kprime_v], axis=1))
+    V = torch.from_numpy(np.concatenate([v for _, v in segs_kprime_v], axis=1))
+    o, lse = np.empty((Hq, D)), np.empty(Hq)
+    for g in range(Hq):
+        h = g // G
+        qg = torch.from_numpy(q[g])[None, None, :]
+        out = torch.nn.functional.scaled_dot_product_attention(qg[None], K[h][None, None], V[h][None, None], scale=scale)
+        o[g] = out[0, 0, 0].numpy()
+        lse[g] = torch.logsumexp((K[h] @ qg[0, 0]) * scale, dim=0).item()
+    return o, lse
+
+
+def random_case(rng, Hq, Hkv, D, lens):
+    q = bf16_bits(rng.standard_normal((Hq, D)))
+    segs = []
+    for L in lens:
+        segs.append((bf16_bits(rng.standard_normal((Hkv, L, D))), bf16_bits(rng.standard_normal((Hkv, L, D)))))
+    return q, segs
+
+
+@pytest.mark.parametrize("pairing", ["neox", "gptj"])
+@pytest.mark.parametrize("Hq,Hkv,D,R,off", [(8, 2, 64, 64, 0), (4, 4, 32, 16, 0), (6, 1, 48, 16, 32), (32, 8, 128, 128, 0)])
+def test_against_sdpa_over_independently_rotated_keys(pairing, Hq, Hkv, D, R, off):
+    rng = np.random.default_rng(25)
+    inv = inv_freq_standard(1e6, R) if R != 16 else inv_freq_llama3(5e5, R, 8.0, 1.0, 4.0, 8192)
+    lens, deltas = [37, 130, 5], [2000, -17, 161]
+    q, segs = random_case(rng, Hq, Hkv, D, lens)
+    scale = 1.0 / np.sqrt(D)
+    o, lse = orc.rotate_on_read_attention(q=q, kv_heads=Hkv, rotary_dim=R, pairing=PAIRING[pairing], inv_freq=inv,
+                                          scale=scale, rotary_offset=off,
+                                          segments=[(k, v, d) for (k, v), d in zip(segs, deltas)])
+    ref_o, ref_lse = sdpa_reference(bf16_val(q), [(rope_complex(bf16_val(k), d, inv, R, pairing, off), bf16_val(v))
+                                                  for (k, v), d in zip(segs, deltas)], Hkv, scale)
+    assert np.max(np.abs(o - ref_o)) < 1e-12
+    assert np.max(np.abs(lse - ref_lse)) < 1e-12
+
+
+@pytest.mark.parametrize("pairing", ["neox", "gptj"])
+def test_quarter_turn_closed_form(pairing):
+    """inv_freq = pi/2, Delta = 1: every pair (a, b) becomes (-b, a) -- direction, sign and pairing by hand.  Small
+    integers are exact in bf16, so the scores are integers: with one key per segment the result is a two-way softmax
+    whose weights are worked out here from the permuted integers."""
+    D = R = 8
+    h = R // 2
+    inv = np.full(h, np.pi / 2)
+    k = np.arange(1, D + 1, dtype=np.float64)                     # 1..8
+    if pairing == "neox":
+        kq = np.concatenate([-k[h:], k[:h]])                       # (a_i, b_i) = (k[i], k[i+h]) -> (-b_i, a_i)
+    else:
+        kq = np.empty(D); kq[0::2], kq[1::2] = -k[1::2], k[0::2]
+    q = np.array([1, 0, -1, 2, 0, 1, 1, -2], dtype=np.float64)
+    v0, v1 = np.arange(D, dtype=np.float64), -np.ones(D)
+    x0, x1 = float(q @ kq), float(q @ k)                           # segment 0 turned by a quarter, segment 1 at rest
+    scale = 0.125
+    w0 = 1.0 / (1.0 + np.exp(scale * (x1 - x0)))
+    o, lse = orc.rotate_on_read_attention(
+        q=bf16_bits(q[None]), kv_heads=1, rotary_dim=R, pairing=PAIRING[pairing], inv_freq=inv, scale=scale,
+        segments=[(bf16_bits(k[None, None]), bf16_bits(v0[None, None]), 1), (bf16_bits(k[None, None]), bf16_bits(v1[None, None]), 0)])
+    assert np.allclose(o[0], w0 * v0 + (1 - w0) * v1, rtol=0, atol=1e-13)
+    assert abs(lse[0] - (scale * x0 + np.log1p(np.exp(scale * (x1 - x0))))) < 1e-13
+    # Delta = 2 is a half turn (k -> -k), Delta = 4 the identity
+    for delta, kk in ((2, -k), (4, k)):
+        _, l2 = orc.rotate_on_read_attention(q=bf16_bits(q[None]), kv_heads=1, rotary_dim=R, pairing=PAIRING[pairing],
+                                             inv_freq=inv, scale=scale, segments=[(bf16_bits(k[None, None]), bf16_bits(v0[None, None]), delta)])
+        assert abs(l2[0] - scale * float(q @ kk)) < 1e-12
+
+
+@pytest.mark.parametrize("pairing", ["neox", "gptj"])
+def test_textbook_rope_attention_at_true_positions(pairing):
+    """The paper's statement: a skill compiled at positions 0..L-1 and read at offset new_start behaves like keys
+    RoPE'd at new_start + t.  q0, k0 are pre-RoPE; the cache holds bf16(RoPE(k0, t)); the expected attention is plain
+    RoPE attention at the true positions (numpy direct RoPE + torch SDPA).  The only difference is the bf16 rounding
+    of the CACHED keys (relative 2^-9 per element), so the tolerance is loose -- a wrong sign of Delta, a transposed
+    pairing or a missing rotation misses it by orders of magnitude (checked below)."""
+    rng = np.random.default_rng(7)
+    Hq, Hkv, D, L, new_start, p_q = 4, 2, 64, 96, 3000, 3200
+    inv = inv_freq_standard(1e4, D)
+    q0, k0, v = rng.standard_normal((Hq, D)), rng.standard_normal((Hkv, L, D)), rng.standard_normal((Hkv, L, D))
+    q = bf16_bits(rope_direct_np(q0, np.full(Hq, p_q), inv, D, pairing))
+    cached = bf16_bits(np.stack([rope_direct_np(k0[h], np.arange(L), inv, D, pairing) for h in range(Hkv)]))
+    vb = bf16_bits(v)
+    scale = 1 / np.sqrt(D)
+    true_k = np.stack([rope_direct_np(k0[h], new_start + np.arange(L), inv, D, pairing) for h in range(Hkv)])
+    ref_o, ref_lse = sdpa_reference(bf16_val(q), [(true_k, bf16_val(vb))], Hkv, scale)
+    o, lse = orc.rotate_on_read_attention(q=q, kv_heads=Hkv, rotary_dim=D, pairing=PAIRING[pairing], inv_freq=inv,
+                                          scale=scale, segments=[(cached, vb, new_start)])
+    assert np.max(np.abs(o - ref_o)) < 0.02 and np.max(np.abs(lse - ref_lse)) < 0.02
+    for wrong in (-new_start, 0):
+        o_w, _ = orc.rotate_on_read_attention(q=q, kv_heads=Hkv, rotary_dim=D, pairing=PAIRING[pairing], inv_freq=inv,
+                                              scale=scale, segments=[(cached, vb, wrong)])
+        assert np.max(np.abs(o_w - ref_o)) > 0.2
+
+
+def test_zero_query_gives_the_mean_of_the_values():
+    rng = np.random.default_rng(1)
+    Hq, Hkv, D = 4, 2, 32
+    q = np.zeros((Hq, D), np.uint16)
+    _, segs = random_case(rng, Hq, Hkv, D, [9, 40])
+    o, lse = orc.rotate_on_read_attention(q=q, kv_heads=Hkv, rotary_dim=D, pairing=orc.NEOX_HALF,
+                                          inv_freq=inv_freq_standard(1e4, D), scale=0.3,
+                                          segments=[(k, v, 5 + i) for i, (k, v) in enumerate(segs)])
+    allv = np.concatenate([bf16_val(v) for _, v in segs], axis=1)            # [Hkv, 49, D]
+    for g in range(Hq):
+        assert np.allclose(o[g], allv[g // 2].mean(axis=0), rtol=0, atol=1e-14)
+    assert np.allclose(lse, np.log(49.0), rtol=0, atol=1e-14)
+
+
+def test_merge_of_single_segment_results():
+    """(o, lse) are partial-attention pairs: the result over {A, B} is the lse-weighted merge of A alone and B alone."""
+    rng = np.random.default_rng(2)
+    Hq, Hkv, D = 8, 2, 64
+    inv = inv_freq_standard(5e5, D)
+    q, segs = random_case(rng, Hq, Hkv, D, [70, 33])
+    kw = dict(q=q, kv_heads=Hkv, rotary_dim=D, pairing=orc.GPTJ_INTERLEAVED, inv_freq=inv, scale=0.2)
+    (ka, va), (kb, vb) = segs
+    o, lse = orc.rotate_on_read_attention(segments=[(ka, va, 100), (kb, vb, -7)], **kw)
+    oa, la = orc.rotate_on_read_attention(segments=[(ka, va, 100)], **kw)
+    ob, lb = orc.rotate_on_read_attention(segments=[(kb, vb, -7)], **kw)
+    l = np.logaddexp(la, lb)
+    assert np.max(np.abs(l - lse)) < 1e-13
+    assert np.max(np.abs(np.exp(la - l)[:, None] * oa + np.exp(lb - l)[:, None] * ob - o)) < 1e-13
+
+
+def test_gqa_head_mapping_and_strides_by_brute_force():
+    """Query head g reads kv head g // (Hq / Hkv); sources may be strided views (padded token rows, a layer slice of a
+    [layers][heads][len][dim] tensor).  Brute force in plain Python loops on a tiny case."""
+    rng = np.random.default_rng(3)
+    Hq, Hkv, D, L = 6, 3, 8, 5
+    big_k = bf16_bits(rng.standard_normal((2, Hkv, L, D + 8)))               # 2 layers, rows padded to D + 8
+    big_v = bf16_bits(rng.standard_normal((2, Hkv, L, D + 8)))
+    k, v = big_k[1, :, :, :D], big_v[1, :, :, :D]                               # layer 1, strided view
+    q = bf16_bits(rng.standard_normal((Hq, D)))
+    inv, scale, delta = inv_freq_standard(1e4, D), 0.35, 11
+    o, lse = orc.rotate_on_read_attention(q=q, kv_heads=Hkv, rotary_dim=D, pairing=orc.NEOX_HALF, inv_freq=inv,
+                                          scale=scale, segments=[(k, v, delta)])
+    qv, kv_, vv = bf16_val(q), bf16_val(np.ascontiguousarray(k)), bf16_val(np.ascontiguousarray(v))
+    for g in range(Hq):
+        h = g // 2
+        xs = []
+        for t in range(L):
+            kr = rope_complex(kv_[h, t], delta, inv, D, "neox")
+            xs.append(scale * sum(qv[g, d] * kr[d] for d in range(D)))
+        m = max(xs)
+        z = sum(np.exp(x - m) for x in xs)
+        assert abs(lse[g] - (m + np.log(z))) < 1e-13
+        for d in range(D):
+            assert abs(o[g, d] - sum(np.exp(x - m) / z * vv[h, t, d] for t, x in enumerate(xs))) < 1e-13
+
+
+def test_counter_rotated_query_gives_the_same_scores():
+    """q . R(Delta) k == (R(-Delta) q) . k -- the identity the CUDA path uses (the oracle rotates the keys)."""
+    rng = np.random.default_rng(4)
+    D, L = 128, 64
+    inv = inv_freq_standard(1e6, D)
+    q, segs = random_case(rng, 4, 1, D, [L])
+    k, v = segs[0]
+    for pairing in ("neox", "gptj"):
+        _, lse = orc.rotate_on_read_attention(q=q, kv_heads=1, rotary_dim=D, pairing=PAIRING[pairing], inv_freq=inv,
+                                              scale=1.0, segments=[(k, v, 4096)])
+        q_back = rope_complex(bf16_val(q), -4096, inv, D, pairing)
+        x = q_back @ bf16_val(k)[0].T                                          # [4, L]
+        assert np.max(np.abs(torch.logsumexp(torch.from_numpy(x), dim=1).numpy() - lse)) < 1e-11
+
+
+def test_bytes_read_and_argument_checks():
+    assert orc.attention_bytes_read(8, 128, 1000) == 2 * 8 * 128 * 2 * 1000
+    q = np.zeros((4, 8), np.uint16)
+    k = np.zeros((3, 2, 8), np.uint16)
+    with pytest.raises(ValueError):                                            # 4 query heads over 3 kv heads
+        orc.rotate_on_read_attention(q=q, kv_heads=3, rotary_dim=8, pairing=0, inv_freq=np.ones(4), scale=1.0, segments=[(k, k, 0)])
