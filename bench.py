@@ -76,11 +76,13 @@ def parse_args(argv=None):
     ap.add_argument("--latency", action="store_true",
                     help="also report launch-to-launch latency and CUDA-graph replay time per call, rotating over 8 "
                          "buffer sets (SURVEY.md 8(d); always on for --config 0)")
-    ap.add_argument("--op", default="splice", choices=["splice", "inplace", "span"],
+    ap.add_argument("--op", default="splice", choices=["splice", "inplace", "span", "attend"],
                     help="splice = kvr_reposition_splice (the BASELINE.json metric); inplace = kvr_reposition_inplace "
                          "(SURVEY.md 8(f) NEXT-1: re-float resident chunks, 2*B1 bytes per token; device-timed only); "
                          "span = kvr_write_span over the same rows (Delta = 0: byte copies with the same access pattern "
-                         "= this library's own copy ceiling, SURVEY.md H1)")
+                         "= this library's own copy ceiling, SURVEY.md H1); attend = kvr_rotate_on_read_attention over a "
+                         "rotate-on-read workload (--workload attend-serving | attend-32k-x8 | attend-compose4; SURVEY.md "
+                         "8(f) rank 4, first alternative; device-timed only)")
     ap.add_argument("--sweep", dest="sweep", action="store_true", default=None, help="force the per_config sweep")
     ap.add_argument("--no-sweep", dest="sweep", action="store_false")
     ap.add_argument("--min-device-s", type=float, default=0.25, help="device time per (config, layout) of the sweep")
@@ -583,10 +585,84 @@ def run_kvr(args):
     return 0
 
 
+def run_attend(args):
+    """--op attend: one step = one kvr_rotate_on_read_attention call (one layer) over a rotate-on-read workload.
+    HBM roofline: K and V of the layer are read once (2 * kv_heads * head_dim * 2 bytes per token); the contraction
+    flops (2 * 2 * q_heads * head_dim per token, on the tensor cores) are reported beside it."""
+    import torch
+    from paper_2606_17107_b200 import build as _kbuild
+    _kbuild.build()
+    from paper_2606_17107_b200 import kvr
+    from paper_2606_17107_b200.harness import DeviceReadWorkload
+    from paper_2606_17107_b200.replicas import Replicas
+    from workloads import attention_config
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the kvr path has no CPU fallback")
+    device = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(device)
+    rep = Replicas(backend="nccl", device=device)
+    steps = args.steps if args.steps is not None else 200
+    warmup = max(3, args.warmup if args.warmup is not None else 20)
+    peak, peak_src = measured_peak()
+    stream = torch.cuda.Stream(device=device)
+    timer = Timer(device, stream, rep, ClockSampler(device))
+    w = attention_config(args.workload or "attend-serving")
+    # sets of sources rotated step by step so that no call finds its keys in the 126 MB L2 from the call before
+    sets = max(1, min(8, int(-(-3 * L2_BYTES // max(1, w.bytes_read())))))
+    dws = [DeviceReadWorkload(w, device) for _ in range(sets)]
+    ctx = kvr.Context(dws[0].model, device=device.index)
+    if args.tune:
+        ctx.set_tuning(**{k: int(v) for k, v in (kv.split("=") for kv in args.tune.split(","))})
+    state = {"i": 0}
+
+    def run_step():
+        dws[state["i"] % sets].run(ctx, stream=stream)
+        state["i"] += 1
+    ramp, est = timer.warm(run_step, warmup)
+    timer.sampler.reset()
+    l0 = ctx.launch_count()
+    with timer.sampler:
+        exact_s = timer.exact_block(run_step, steps)
+        launches = ctx.launch_count() - l0
+        blk = timer.blocks(run_step, steps, est, args.min_device_s)
+    per = [b / steps for b in blk]
+    med, best, worst = _median(per), min(per), max(per)
+    info = ctx.last_launch_info()
+    b = dws[0].bytes_read()
+    flops = 4.0 * w.q_heads * w.head_dim * w.tokens
+    achieved = b / (exact_s / steps) / 1e9
+    ctx.close()
+    if rep.rank == 0:
+        line = {
+            "metric": "KV tokens attended by rotate-on-read/sec (one layer)", "value": w.tokens * rep.world / (exact_s / steps),
+            "unit": UNIT, "n_gpus": rep.world, "steps": steps, "warmup": warmup, "warmup_ramp_steps": ramp,
+            "ms_per_step": exact_s / steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16", "arithmetic": "bf16 tensor-core contractions (tcgen05, fp32 accumulation in TMEM), fp32 softmax, "
+                     "fp64 counter-rotation of the query",
+            "data": "synthetic",
+            "config": {"workload": w.name, "op": "attend", "requests": w.n_req, "segments": len(w.segments), "tokens": w.tokens,
+                       "q_heads": w.q_heads, "kv_heads": w.kv_heads, "head_dim": w.head_dim, "bytes_per_step": int(b),
+                       "parallelism": f"replicas x{rep.world}",
+                       "l2": f"{sets} independent source sets rotated step by step ({sets * b} B > 126 MB L2)"},
+            "launch": {"kernel": "kvr_attend_kernel", "grid": info["grid"], "block": info["block"], "smem": info["smem"]},
+            "gpu_launches": launches, "clocks": timer.sampler.summary(),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": traffic_of(w.name, "src", "attend"), "peak_source": peak_src,
+                         "median_achieved": b / med / 1e9, "best_achieved": b / best / 1e9, "spread": (worst - best) / med,
+                         "blocks": len(blk), "tensor_tflops": flops / (exact_s / steps) / 1e12},
+            "e2e": None, "cpu_baseline": None,
+        }
+        print(json.dumps(line), flush=True)
+    rep.close()
+    return 0
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.op == "attend":
+        return run_attend(args)
     return run_kvr(args)
 
 

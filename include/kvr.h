@@ -234,6 +234,42 @@ typedef struct {
 KVR_API kvr_status kvr_write_span(kvr_ctx* ctx, const kvr_paged_dst* dst, const kvr_span* spans, int32_t n_spans,
                                   void* cuda_stream);
 
+/* ---- NEXT-4, first alternative: ROTATE-ON-READ decode attention ---------------------------------------------
+ * "fusing the rotate into a consumer (rotate-on-read in the attention K load ...) so K is never
+ * materialised twice"; "we re-rotate the chunk's keys from their source positions to the target positions
+ * (values are position-free)"; PAPER.md:143 (the pass is O(L)); PAPER.md:209 (works under FlashAttention / paged
+ * attention, GQA/MQA).  DESIGN.md reading R25.
+ * A decode-step query attends the cached keys and values of precompiled skills WHERE THEY LIE -- nothing is spliced,
+ * nothing is written back.  For request r, query head g (kv head h = g / (q_heads / kv_heads)), over every token t of
+ * every segment s with segs[s].request == r, at model layer `layer`:
+ *     x_{s,t} = softmax_scale * sum_d q[r][g][d] * (R(delta_s) k_{s,t})[d]      R = the re-rotation of kvr_reposition_splice
+ *     lse[r][g] = ln sum exp(x)            o[r][g][:] = sum exp(x_{s,t} - lse[r][g]) * v_{s,t}[:]
+ * (o, lse) is the partial-attention pair the caller merges with its attention over the rest of the context.
+ * q: DEVICE bf16 [n_req][q_heads][head_dim], the query as the model produced it (RoPE'd at its own position).
+ * o: DEVICE fp32 [n_req][q_heads][head_dim]; lse: DEVICE fp32 [n_req][q_heads] (natural logarithm).
+ * Arithmetic: the kernel uses q . R(delta) k = (R(-delta) q) . k: the counter-rotated query is evaluated in fp64 and
+ * rounded once to bf16; both contractions run on the tensor cores (bf16 operands, fp32 accumulation), the softmax
+ * weights are rounded to bf16 before they multiply V and their row sum adds the rounded weights.
+ * Limits (else KVR_ERR_UNSUPPORTED): KVR_BF16 caches, head_dim == 128, q_heads / kv_heads <= 16.  Every request must
+ * own at least one segment; k_src / v_src as in kvr_segment (DEVICE, [layers][kv_heads][len][head_dim], element strides,
+ * 16-byte aligned).  Asynchronous on `cuda_stream`; descriptors are staged through context-owned pinned memory, so the
+ * call cannot be captured in a CUDA graph (KVR_ERR_UNSUPPORTED under capture).  Reads 2 * kv_heads * head_dim * 2 bytes
+ * per token (kvr_attention_bytes_read): K and V of one layer, once. */
+typedef struct {
+  const void* k_src;
+  const void* v_src;
+  int64_t src_stride_layer, src_stride_head, src_stride_token; /* elements */
+  int32_t len;
+  int32_t delta;   /* new_start - old_start: where the skill sits in this request's context minus where it was compiled */
+  int32_t request; /* row of q / o / lse that attends this segment */
+  int32_t reserved_; /* must be 0 */
+} kvr_read_segment;
+
+KVR_API kvr_status kvr_rotate_on_read_attention(kvr_ctx* ctx, const void* q, int32_t n_req, int32_t q_heads, int32_t layer,
+                                                float softmax_scale, const kvr_read_segment* segs, int32_t n_segs,
+                                                float* o, float* lse, void* cuda_stream);
+KVR_API uint64_t kvr_attention_bytes_read(const kvr_model_desc* model, const kvr_read_segment* segs, int32_t n_segs);
+
 /* Algorithmic bytes of a call: read K, read V, write K, write V = 4 * layers*kv_heads*head_dim*esz * sum(len)
  * (2 * ... for a K-only call, i.e. when segs[0].v_src == NULL).
  * This is the O(L) of PAPER.md:143 and the numerator of every GB/s this repository reports. */
@@ -244,7 +280,7 @@ KVR_API uint64_t kvr_bytes_moved(const kvr_model_desc* model, const kvr_segment*
 KVR_API kvr_status kvr_last_device_status(kvr_ctx* ctx, int32_t* bad_segment, int32_t* bad_token);
 
 /* Introspection for benchmarks: kernels launched by this context so far; the kernel path the last call took
- * (1 generic, 2 TMA ring); grid size, CTA size and dynamic shared memory of its main kernel. */
+ * (1 generic, 2 TMA ring, 3 rotate-on-read attention); grid size, CTA size and dynamic shared memory of its main kernel. */
 KVR_API uint64_t kvr_launch_count(const kvr_ctx* ctx);
 KVR_API kvr_status kvr_last_launch_info(const kvr_ctx* ctx, int32_t* path, int32_t* grid, int32_t* block,
                                         int32_t* smem_bytes);

@@ -1,5 +1,7 @@
 // kvr_api.cu -- the C ABI of include/kvr.h: context, host-side validation, work decomposition,
 // descriptor staging and kernel dispatch.  No arithmetic of the method happens on the host.
+#include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <mutex>
@@ -8,6 +10,7 @@
 #include <vector>
 
 #include "../../include/kvr.h"
+#include "kvr_attend.cuh"
 #include "kvr_common.cuh"
 
 using namespace kvr;
@@ -163,6 +166,14 @@ struct kvr_ctx {
   void* aux_dev = nullptr;            // pos_map / k_scale_src copies
   size_t aux_cap = 0;
   uint64_t h2d_bytes = 0;             // bytes the last host-source call copied host -> device
+  // rotate-on-read attention (kvr_rotate_on_read_attention): descriptor staging ring, partial results, group tickets
+  struct AttnSlot { unsigned char* host = nullptr; unsigned char* dev = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; bool pending = false; };
+  AttnSlot attn_slots[4];
+  int attn_next = 0;
+  float* attn_part = nullptr;         // [items][group][128 + 2]
+  size_t attn_part_cap = 0;           // bytes
+  unsigned int* attn_tickets = nullptr;
+  size_t attn_ticket_cap = 0;         // entries
 
   kvr_status cuda_fail(cudaError_t e, const char* what) {
     last_err = std::string(what) + ": " + cudaGetErrorString(e);
@@ -271,6 +282,13 @@ kvr_status kvr_destroy(kvr_ctx* c) {
     if (c->stage_drained[b]) cudaEventDestroy(c->stage_drained[b]);
   }
   if (c->fork_ev) cudaEventDestroy(c->fork_ev);
+  for (auto& a : c->attn_slots) {
+    if (a.host) cudaFreeHost(a.host);
+    if (a.dev) cudaFree(a.dev);
+    if (a.ev) cudaEventDestroy(a.ev);
+  }
+  if (c->attn_part) cudaFree(c->attn_part);
+  if (c->attn_tickets) cudaFree(c->attn_tickets);
   if (c->aux_dev) cudaFree(c->aux_dev);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->d_inv_freq) cudaFree(c->d_inv_freq);
@@ -588,6 +606,187 @@ struct DeviceGuard {
   explicit DeviceGuard(int dev) : cur(dev) { cudaGetDevice(&prev); if (prev != cur) cudaSetDevice(cur); }
   ~DeviceGuard() { if (prev != cur) cudaSetDevice(prev); }
 };
+
+// ---- NEXT-4, first alternative: rotate-on-read decode attention (kvr.h; R25) ----
+namespace {
+
+// Tensor map of one source tensor [layers][heads][len][128] bf16 with dims ordered (dim, token, head, layer): a box of
+// {64 dims, 128 tokens} lands as 128 rows of 128 bytes, 128-byte swizzled -- the tcgen05 shared-memory operand layout.
+bool encode_attn_map(CUtensorMap* out, const void* base, int heads, int len, int layers, int64_t sl, int64_t sh, int64_t st) {
+  TmapEncodeFn enc = tmap_encoder();
+  if (!enc || !base) return false;
+  uint64_t s_t = (uint64_t)st * 2, s_h = (uint64_t)sh * 2, s_l = (uint64_t)sl * 2;
+  if (len == 1 && s_t == 0) s_t = 256;          // a dimension of extent 1 never uses its stride: give it a legal one
+  if (heads == 1 && s_h == 0) s_h = 256;
+  if (layers == 1 && s_l == 0) s_l = 256;
+  if (s_t == 0 || s_h == 0 || s_l == 0) return false;
+  const cuuint64_t dims[4] = {128u, (cuuint64_t)len, (cuuint64_t)heads, (cuuint64_t)layers};
+  const cuuint64_t strides[3] = {s_t, s_h, s_l};
+  const cuuint32_t box[4] = {64u, 128u, 1u, 1u};
+  const cuuint32_t es[4] = {1u, 1u, 1u, 1u};
+  return enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(base), dims, strides, box, es,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+extern "C" {
+
+uint64_t kvr_attention_bytes_read(const kvr_model_desc* m, const kvr_read_segment* segs, int32_t n) {
+  if (!m || (n > 0 && !segs)) return 0;
+  uint64_t tokens = 0;
+  for (int32_t i = 0; i < n; ++i) tokens += segs[i].len > 0 ? (uint64_t)segs[i].len : 0u;
+  return 2ull * (uint64_t)m->kv_heads * (uint64_t)m->head_dim * (uint64_t)elt_bytes(m->dtype) * tokens;
+}
+
+kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req, int32_t q_heads, int32_t layer,
+                                        float softmax_scale, const kvr_read_segment* segs, int32_t n, float* o, float* lse,
+                                        void* cuda_stream) {
+  if (!c) return KVR_ERR_INVALID_ARG;
+  c->last_err.clear();
+  const kvr_model_desc& m = c->model;
+  if (!q || !o || !lse || !segs || n <= 0 || n_req <= 0 || q_heads <= 0 || layer < 0 || layer >= m.layers) return KVR_ERR_INVALID_ARG;
+  if (q_heads % m.kv_heads != 0 || !(softmax_scale > 0.0f) || !std::isfinite(softmax_scale)) return KVR_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(o) || (reinterpret_cast<uintptr_t>(lse) & 3u)) return KVR_ERR_ALIGNMENT;
+  const int group = q_heads / m.kv_heads;
+  if (m.dtype != KVR_BF16 || m.head_dim != 128 || group > 16) {
+    c->last_err = "rotate-on-read attention: bf16 caches, head_dim 128 and q_heads / kv_heads <= 16 only";
+    return KVR_ERR_UNSUPPORTED;
+  }
+  std::vector<int32_t> per_req((size_t)n_req, 0);
+  for (int32_t i = 0; i < n; ++i) {
+    const kvr_read_segment& s = segs[i];
+    if (!s.k_src || !s.v_src || s.len <= 0 || s.request < 0 || s.request >= n_req || s.reserved_ != 0) return KVR_ERR_INVALID_ARG;
+    if ((s.src_stride_token < m.head_dim && s.len > 1) || s.src_stride_layer < 0 || s.src_stride_head < 0) return KVR_ERR_INVALID_ARG;
+    if ((s.src_stride_head < m.head_dim && m.kv_heads > 1)) return KVR_ERR_INVALID_ARG;
+    if (!aligned16(s.k_src) || !aligned16(s.v_src)) return KVR_ERR_ALIGNMENT;
+    if ((s.src_stride_layer * 2) % 16 || (s.src_stride_head * 2) % 16 || (s.src_stride_token * 2) % 16) return KVR_ERR_ALIGNMENT;
+    per_req[(size_t)s.request] += 1;
+  }
+  for (int32_t r = 0; r < n_req; ++r)
+    if (per_req[(size_t)r] == 0) { c->last_err = "rotate-on-read attention: a request without segments"; return KVR_ERR_INVALID_ARG; }
+  if (!tmap_encoder()) { c->last_err = "cuTensorMapEncodeTiled is not available"; return KVR_ERR_UNSUPPORTED; }
+  DeviceGuard guard(c->device);
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  KVR_CUDA(c, cudaStreamIsCapturing(stream, &cap));
+  if (cap != cudaStreamCaptureStatusNone) {
+    c->last_err = "rotate-on-read attention stages its descriptors through pinned memory and cannot be captured";
+    return KVR_ERR_UNSUPPORTED;
+  }
+
+  // ---- work decomposition: items = (segment, kv head, run of key tiles); groups = (request, kv head) ----
+  std::vector<int32_t> order((size_t)n);
+  for (int32_t i = 0; i < n; ++i) order[(size_t)i] = i;
+  std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return segs[a].request < segs[b].request; });
+  int64_t total_tiles = 0;
+  for (int32_t i = 0; i < n; ++i) total_tiles += ((int64_t)segs[i].len + 127) / 128;
+  total_tiles *= m.kv_heads;
+  // ~4 items per SM when the call is large enough; 2..32 tiles (256..4096 keys) per item; tuning.layers_per_unit
+  // doubles as "tiles per item" for experiments (this call has no layers to group)
+  int64_t tpi = (total_tiles + 4ll * c->sm_count - 1) / (4ll * c->sm_count);
+  tpi = tpi < 2 ? 2 : (tpi > 32 ? 32 : tpi);
+  if (c->tuning.layers_per_unit > 0) tpi = c->tuning.layers_per_unit;
+  std::vector<AttnItem> items;
+  items.reserve((size_t)(total_tiles / tpi + (int64_t)n * m.kv_heads));
+  int32_t n_groups = 0;
+  for (size_t a = 0; a < order.size();) {
+    size_t b = a;
+    while (b < order.size() && segs[order[b]].request == segs[order[a]].request) ++b;
+    const int32_t r = segs[order[a]].request;
+    for (int32_t h = 0; h < m.kv_heads; ++h) {
+      const int32_t first = (int32_t)items.size();
+      for (size_t j = a; j < b; ++j) {
+        const int32_t si = order[j], len = segs[si].len;
+        for (int32_t k0 = 0; k0 < len; k0 += (int32_t)tpi * 128) {
+          AttnItem it{};
+          it.seg = si; it.head = h; it.key0 = k0; it.n_keys = std::min<int32_t>((int32_t)tpi * 128, len - k0);
+          it.group = n_groups; it.group_first = first; it.out_q0 = r * q_heads + h * group;
+          items.push_back(it);
+        }
+      }
+      const int32_t cnt = (int32_t)items.size() - first;
+      for (int32_t j = first; j < first + cnt; ++j) items[(size_t)j].group_count = cnt;
+      ++n_groups;
+    }
+    a = b;
+  }
+  const size_t n_items = items.size();
+
+  // ---- staging: [AttnSeg x n][AttnItem x n_items] through one pinned slot and one H2D copy ----
+  const size_t seg_bytes = (size_t)n * sizeof(AttnSeg), bytes = seg_bytes + n_items * sizeof(AttnItem);
+  kvr_ctx::AttnSlot& slot = c->attn_slots[c->attn_next];
+  c->attn_next = (c->attn_next + 1) % 4;
+  if (slot.pending) { KVR_CUDA(c, cudaEventSynchronize(slot.ev)); slot.pending = false; }
+  if (!slot.ev) KVR_CUDA(c, cudaEventCreateWithFlags(&slot.ev, cudaEventDisableTiming));
+  if (bytes > slot.cap) {
+    size_t cap = slot.cap ? slot.cap : (size_t)1 << 16;
+    while (cap < bytes) cap *= 2;
+    if (slot.host) cudaFreeHost(slot.host);
+    if (slot.dev) cudaFree(slot.dev);
+    slot.host = nullptr; slot.dev = nullptr; slot.cap = 0;
+    KVR_CUDA(c, cudaMallocHost(&slot.host, cap));
+    KVR_CUDA(c, cudaMalloc(&slot.dev, cap));
+    slot.cap = cap;
+  }
+  AttnSeg* hs = reinterpret_cast<AttnSeg*>(slot.host);
+  for (int32_t i = 0; i < n; ++i) {
+    const kvr_read_segment& s = segs[i];
+    if (!encode_attn_map(&hs[i].k, s.k_src, m.kv_heads, s.len, m.layers, s.src_stride_layer, s.src_stride_head, s.src_stride_token) ||
+        !encode_attn_map(&hs[i].v, s.v_src, m.kv_heads, s.len, m.layers, s.src_stride_layer, s.src_stride_head, s.src_stride_token)) {
+      c->last_err = "rotate-on-read attention: a source tensor cannot be described by a TMA tensor map";
+      return KVR_ERR_UNSUPPORTED;
+    }
+    hs[i].delta = s.delta; hs[i].len = s.len; hs[i].request = s.request; hs[i].pad_ = 0;
+  }
+  std::memcpy(slot.host + seg_bytes, items.data(), n_items * sizeof(AttnItem));
+  // partial results and tickets (grown on demand; a regrowth waits for the launches that may still use the old buffers)
+  const size_t part_bytes = n_items * (size_t)group * (128 + 2) * sizeof(float);
+  if (part_bytes > c->attn_part_cap || (size_t)n_groups > c->attn_ticket_cap) {
+    KVR_CUDA(c, cudaDeviceSynchronize());
+    if (part_bytes > c->attn_part_cap) {
+      if (c->attn_part) cudaFree(c->attn_part);
+      c->attn_part = nullptr; c->attn_part_cap = 0;
+      size_t cap = std::max<size_t>(part_bytes * 2, (size_t)1 << 20);
+      KVR_CUDA(c, cudaMalloc(&c->attn_part, cap));
+      c->attn_part_cap = cap;
+    }
+    if ((size_t)n_groups > c->attn_ticket_cap) {
+      if (c->attn_tickets) cudaFree(c->attn_tickets);
+      c->attn_tickets = nullptr; c->attn_ticket_cap = 0;
+      size_t cap = std::max<size_t>((size_t)n_groups * 2, 1024);
+      KVR_CUDA(c, cudaMalloc(&c->attn_tickets, cap * sizeof(unsigned int)));
+      KVR_CUDA(c, cudaMemset(c->attn_tickets, 0, cap * sizeof(unsigned int)));
+      c->attn_ticket_cap = cap;
+    }
+  }
+  KVR_CUDA(c, cudaMemcpyAsync(slot.dev, slot.host, bytes, cudaMemcpyHostToDevice, stream));
+
+  AttnParams P{};
+  P.q = static_cast<const uint16_t*>(q); P.o = o; P.lse = lse;
+  P.segs = reinterpret_cast<const AttnSeg*>(slot.dev);
+  P.items = reinterpret_cast<const AttnItem*>(slot.dev + seg_bytes);
+  P.n_items = (int32_t)n_items;
+  P.q_heads = q_heads; P.group = group; P.layer = layer;
+  P.rotary_dim = m.rotary_dim; P.rotary_offset = m.rotary_offset; P.pairing = m.pairing;
+  P.scale_log2 = (float)((double)softmax_scale * 1.4426950408889634);
+  P.inv_freq = c->d_inv_freq;
+  P.part_o = c->attn_part;
+  P.part_ml = c->attn_part + n_items * (size_t)group * 128;
+  P.tickets = c->attn_tickets;
+  cudaError_t e = launch_attend(P, c->tuning.max_ctas > 0 ? std::min(c->tuning.max_ctas, c->sm_count) : c->sm_count, stream,
+                                &c->last_grid, &c->last_block, &c->last_smem);
+  if (e != cudaSuccess) return c->cuda_fail(e, "launch_attend");
+  c->launches += 1;
+  c->last_path = 3;
+  c->last_stream = stream;
+  KVR_CUDA(c, cudaEventRecord(slot.ev, stream));
+  slot.pending = true;
+  return KVR_OK;
+}
+
+}  // extern "C"
 
 extern "C" {
 

@@ -143,3 +143,38 @@ def bits_to_numpy(t):
     """Bit-pattern tensor (int16 for bf16, uint8 for fp8) -> contiguous numpy array (uint16 / uint8) on the host."""
     a = t.detach().cpu().contiguous().numpy()
     return a.view(np.uint16) if a.dtype == np.int16 else a
+
+
+class DeviceReadWorkload:
+    """Sources, queries and outputs of a workloads.ReadWorkload resident on `device`, plus the ctypes structs of one
+    kvr_rotate_on_read_attention call (one layer) over all segments.  guard_bytes as in DeviceWorkload."""
+
+    def __init__(self, w, device="cuda:0", sources=None, queries=None, guard_bytes=0):
+        from workloads import make_queries, make_read_sources
+        self.w = w
+        self.device = torch.device(device)
+        self.guard_bytes = int(guard_bytes)
+        self._guarded = []
+        self.model, self._inv_keep = kvr.model_desc(w.layers, w.kv_heads, w.head_dim, w.rotary_dim, _PAIRING[w.pairing],
+                                                    kvr.KVR_BF16, w.inv_freq, rotary_offset=w.rotary_offset)
+        if sources is None:
+            sources = make_read_sources(w, self.device)
+        if queries is None:
+            queries = make_queries(w, self.device)
+        self.sources = [(self._dev(k, f"k_src[{i}]"), self._dev(v, f"v_src[{i}]")) for i, (k, v) in enumerate(sources)]
+        self.q = self._dev(queries, "q")
+        self.o = self._dev(torch.full((w.n_req, w.q_heads, w.head_dim), float("nan"), dtype=torch.float32), "o")
+        self.lse = self._dev(torch.full((w.n_req, w.q_heads), float("nan"), dtype=torch.float32), "lse")
+        self.segs = kvr.read_segment_array([kvr.read_segment(k, v, w.src_strides(s), s.len, s.delta, s.request)
+                                            for s, (k, v) in zip(w.segments, self.sources)])
+
+    _dev = DeviceWorkload._dev
+    check_guards = DeviceWorkload.check_guards
+
+    def bytes_read(self):
+        return kvr.kvr_attention_bytes_read(self.model, self.segs)
+
+    def run(self, ctx, stream=None, layer=None):
+        w = self.w
+        return ctx.rotate_on_read_attention(self.q, w.n_req, w.q_heads, w.layer if layer is None else layer, w.scale,
+                                            self.segs, self.o, self.lse, stream=stream)

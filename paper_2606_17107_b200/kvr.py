@@ -16,7 +16,7 @@ KVR_ERR_OUT_OF_RANGE, KVR_ERR_CUDA, KVR_ERR_NOMEM = -4, -5, -6
 KVR_BF16, KVR_FP8_E4M3 = 0, 1
 KVR_PAIR_NEOX_HALF, KVR_PAIR_GPTJ_INTERLEAVED = 0, 1
 KVR_SEG_PRE_ROPE = 1
-PATH_AUTO, PATH_GENERIC, PATH_RING = 0, 1, 2
+PATH_AUTO, PATH_GENERIC, PATH_RING, PATH_ATTEND = 0, 1, 2, 3
 
 
 class kvr_model_desc(C.Structure):
@@ -64,7 +64,13 @@ class kvr_span(C.Structure):
                 ("len", C.c_int32), ("dst_seq", C.c_int32), ("dst_token_start", C.c_int32)]
 
 
-EXPORTS = ["kvr_reposition_inplace", "kvr_inplace_bytes_moved", "kvr_write_span",
+class kvr_read_segment(C.Structure):
+    _fields_ = [("k_src", C.c_void_p), ("v_src", C.c_void_p),
+                ("src_stride_layer", C.c_int64), ("src_stride_head", C.c_int64), ("src_stride_token", C.c_int64),
+                ("len", C.c_int32), ("delta", C.c_int32), ("request", C.c_int32), ("reserved_", C.c_int32)]
+
+
+EXPORTS = ["kvr_rotate_on_read_attention", "kvr_attention_bytes_read", "kvr_reposition_inplace", "kvr_inplace_bytes_moved", "kvr_write_span",
            "kvr_create", "kvr_destroy", "kvr_set_tuning", "kvr_validate", "kvr_reposition_splice",
            "kvr_reposition_splice_host", "kvr_last_h2d_bytes",
            "kvr_bytes_moved", "kvr_last_device_status", "kvr_launch_count", "kvr_last_launch_info",
@@ -95,6 +101,11 @@ def _load():
     lib.kvr_inplace_bytes_moved.argtypes = [P(kvr_model_desc), P(kvr_resident_span), C.c_int32]
     lib.kvr_write_span.restype = C.c_int
     lib.kvr_write_span.argtypes = [C.c_void_p, P(kvr_paged_dst), P(kvr_span), C.c_int32, C.c_void_p]
+    lib.kvr_rotate_on_read_attention.restype = C.c_int
+    lib.kvr_rotate_on_read_attention.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_float,
+                                                 P(kvr_read_segment), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.kvr_attention_bytes_read.restype = C.c_uint64
+    lib.kvr_attention_bytes_read.argtypes = [P(kvr_model_desc), P(kvr_read_segment), C.c_int32]
     lib.kvr_last_h2d_bytes.restype = C.c_uint64
     lib.kvr_last_h2d_bytes.argtypes = [C.c_void_p]
     lib.kvr_bytes_moved.restype = C.c_uint64
@@ -171,6 +182,20 @@ def span(k_src, v_src, src_strides, len, dst_seq, dst_token_start):
 
 def span_array(spans):
     return (kvr_span * len(spans))(*spans)
+
+
+def read_segment(k_src, v_src, src_strides, len, delta, request):
+    sl, sh, st = src_strides
+    return kvr_read_segment(_ptr(k_src), _ptr(v_src), sl, sh, st, len, delta, request, 0)
+
+
+def read_segment_array(segs):
+    return (kvr_read_segment * len(segs))(*segs)
+
+
+def kvr_attention_bytes_read(model, segs):
+    arr = segs if not isinstance(segs, (list, tuple)) else read_segment_array(segs)
+    return int(lib.kvr_attention_bytes_read(C.byref(model), arr, len(arr)))
 
 
 def kvr_inplace_bytes_moved(model, spans):
@@ -261,6 +286,17 @@ class Context:
         arr = spans if not isinstance(spans, (list, tuple)) else span_array(spans)
         s = None if stream is None else (stream if isinstance(stream, int) else stream.cuda_stream)
         st = lib.kvr_write_span(self._h, C.byref(dst), arr, len(arr), s)
+        if check and st != KVR_OK:
+            raise KvrError(st, lib.kvr_last_cuda_error(self._h).decode())
+        return st
+
+    def rotate_on_read_attention(self, q, n_req, q_heads, layer, softmax_scale, segs, o, lse, stream=None, check=True):
+        """kvr_rotate_on_read_attention: q bf16 [n_req, q_heads, head_dim], o fp32 [n_req, q_heads, head_dim],
+        lse fp32 [n_req, q_heads] (device tensors or addresses); segs = read_segment_array() or a list."""
+        arr = segs if not isinstance(segs, (list, tuple)) else read_segment_array(segs)
+        s = None if stream is None else (stream if isinstance(stream, int) else stream.cuda_stream)
+        st = lib.kvr_rotate_on_read_attention(self._h, _ptr(q), n_req, q_heads, layer, softmax_scale, arr, len(arr),
+                                              _ptr(o), _ptr(lse), s)
         if check and st != KVR_OK:
             raise KvrError(st, lib.kvr_last_cuda_error(self._h).decode())
         return st

@@ -1,0 +1,249 @@
+"""GPU parity of kvr_rotate_on_read_attention (include/kvr.h; R25) against the fp64 oracle
+(oracle/kvr_attention_oracle.c), through the C ABI.
+
+Two comparisons per case, both element by element:
+ (1) against the ORACLE (the definition: every key re-rotated in fp64, exact softmax), within the tolerance DESIGN.md
+     derives from the kernel's arithmetic contract: the counter-rotated query is rounded once to bf16, so score j is off
+     by at most E_j = scale * sum_d |q'_d - bf16(q'_d)| * |k_jd| (computed here exactly, per query head), the softmax
+     weights are rounded to bf16 (relative 2^-9 each, numerator and denominator alike), everything else is fp32:
+         |o - o_ref|   <= (expm1(2 max_j E_j) + 2^-8 + 2^-12) * max_j |v_jd|
+         |lse - lse_ref| <= max_j E_j + 2^-8
+ (2) against the same definition evaluated with the bf16-rounded counter-rotated query (numpy fp64; "both sides take
+     the rounding decision in the same precision"): what is left is the bf16 rounding of the weights and fp32
+     accumulation, so the bound is tight enough to see a single wrong key, dim or head:
+         |o - o_model| <= 2^-7 * sum_j w_j |v_jd| + 2^-12 * max_j |v_jd| ;  |lse - lse_model| <= 2^-8
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import kvr_oracle as orc
+from tests.helpers import PAIRING, np_bits
+from workloads import READ_WORKLOADS, attention_config, inv_freq_llama3, make_queries, make_read_sources, read_workload
+
+pytestmark = pytest.mark.gpu
+
+GUARD = 64 * 1024
+
+
+def bf16_val(bits):
+    return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16).to(torch.float64).numpy()
+
+
+def bf16_round(x):
+    """fp64 -> fp32 -> bf16 (RNE), back as fp64: the rounding kvr.h states for the counter-rotated query."""
+    t = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float64)).to(torch.float32).to(torch.bfloat16)
+    return t.to(torch.float64).numpy()
+
+
+def counter_rotate(q, delta, inv_freq, R, pairing, offset):
+    """R(-delta) q in fp64 (complex form; independent of oracle and kernel)."""
+    q = np.array(q, dtype=np.float64)
+    h = R // 2
+    if pairing == "neox":
+        ia, ib = offset + np.arange(h), offset + h + np.arange(h)
+    else:
+        ia, ib = offset + 2 * np.arange(h), offset + 2 * np.arange(h) + 1
+    z = (q[..., ia] + 1j * q[..., ib]) * np.exp(-1j * float(delta) * np.asarray(inv_freq, dtype=np.float64))
+    out = q.copy()
+    out[..., ia], out[..., ib] = z.real, z.imag
+    return out
+
+
+def reference(w, srcs, q_bits, n_threads):
+    """Per request: oracle (o, lse), the bf16-query model (o, lse, sum_j w_j |v_j|), E = max_j E_j and max_j |v_jd|."""
+    D, G = w.head_dim, w.q_heads // w.kv_heads
+    out = []
+    for r in range(w.n_req):
+        segs = [(i, s) for i, s in enumerate(w.segments) if s.request == r]
+        o_ref, lse_ref = orc.rotate_on_read_attention(
+            q=q_bits[r], kv_heads=w.kv_heads, rotary_dim=w.rotary_dim, pairing=PAIRING[w.pairing], inv_freq=w.inv_freq,
+            scale=w.scale, rotary_offset=w.rotary_offset, n_threads=n_threads,
+            segments=[(srcs[i][0][w.layer][:, :, :D], srcs[i][1][w.layer][:, :, :D], s.delta) for i, s in segs])
+        qv = bf16_val(q_bits[r])                                       # [Hq, D]
+        xs, vs, E = [], [], np.zeros(w.q_heads)
+        for i, s in segs:
+            k = bf16_val(srcs[i][0][w.layer][:, :, :D])                 # [Hkv, L, D]
+            v = bf16_val(srcs[i][1][w.layer][:, :, :D])
+            qp = counter_rotate(qv, s.delta, w.inv_freq, w.rotary_dim, w.pairing, w.rotary_offset)
+            qb = bf16_round(qp)
+            kk = np.repeat(k, G, axis=0)                                # [Hq, L, D]
+            xs.append(w.scale * np.einsum("gd,gld->gl", qb, kk))
+            E = np.maximum(E, w.scale * np.einsum("gd,gld->gl", np.abs(qp - qb), np.abs(kk)).max(axis=1))
+            vs.append(np.repeat(v, G, axis=0))
+        x, v = np.concatenate(xs, axis=1), np.concatenate(vs, axis=1)   # [Hq, T], [Hq, T, D]
+        m = x.max(axis=1, keepdims=True)
+        p = np.exp(x - m)
+        z = p.sum(axis=1, keepdims=True)
+        wgt = p / z
+        out.append(dict(o_ref=o_ref, lse_ref=lse_ref, o_model=np.einsum("gt,gtd->gd", wgt, v),
+                        lse_model=(m + np.log(z))[:, 0], wabsv=np.einsum("gt,gtd->gd", wgt, np.abs(v)),
+                        vmax=np.abs(v).max(axis=1), E=E))
+    return out
+
+
+def run_and_check(w, tuning=None, n_threads=None, layer=None):
+    from paper_2606_17107_b200 import kvr
+    from paper_2606_17107_b200.harness import DeviceReadWorkload
+    if layer is not None:
+        w.layer = layer
+    srcs_t = make_read_sources(w, "cpu")
+    q_t = make_queries(w, "cpu")
+    dw = DeviceReadWorkload(w, "cuda:0", sources=srcs_t, queries=q_t, guard_bytes=GUARD)
+    with kvr.Context(dw.model) as ctx:
+        if tuning:
+            ctx.set_tuning(**tuning)
+        dw.run(ctx)
+        dw.run(ctx)                                        # twice: tickets and staging slots re-arm themselves
+        torch.cuda.synchronize()
+        info = ctx.last_launch_info()
+        assert ctx.last_device_status()[0] == kvr.KVR_OK
+    assert info["path"] == kvr.PATH_ATTEND
+    dw.check_guards()
+    o, lse = dw.o.cpu().numpy().astype(np.float64), dw.lse.cpu().numpy().astype(np.float64)
+    assert np.isfinite(o).all() and np.isfinite(lse).all()
+    srcs = [(np_bits(k), np_bits(v)) for k, v in srcs_t]
+    ref = reference(w, srcs, np_bits(q_t), n_threads or orc.host_threads())
+    worst = 0.0
+    for r, R in enumerate(ref):
+        E = R["E"][:, None]
+        tol_o = (np.expm1(2 * E) + 2.0 ** -8 + 2.0 ** -12) * R["vmax"]
+        assert (np.abs(o[r] - R["o_ref"]) <= tol_o).all(), (r, float(np.abs(o[r] - R["o_ref"]).max()), float(tol_o.min()))
+        assert (np.abs(lse[r] - R["lse_ref"]) <= R["E"] + 2.0 ** -8).all(), (r, float(np.abs(lse[r] - R["lse_ref"]).max()))
+        tol_m = 2.0 ** -7 * R["wabsv"] + 2.0 ** -12 * R["vmax"]
+        d = np.abs(o[r] - R["o_model"])
+        assert (d <= tol_m).all(), (r, float((d / tol_m).max()), np.unravel_index(np.argmax(d / tol_m), d.shape))
+        assert (np.abs(lse[r] - R["lse_model"]) <= 2.0 ** -8).all(), (r, float(np.abs(lse[r] - R["lse_model"]).max()))
+        worst = max(worst, float((d / tol_m).max()))
+    return info, worst
+
+
+@pytest.mark.parametrize("name", READ_WORKLOADS)
+def test_attention_workloads_reduced(name):
+    """The four rotate-on-read workloads with every length divided (several tiles, ragged tails, several items per group)."""
+    shrink = {"attend-tiny": 1, "attend-compose4": 8, "attend-32k-x8": 32, "attend-serving": 16}[name]
+    run_and_check(attention_config(name, shrink=shrink))
+
+
+@pytest.mark.parametrize("q_heads,kv_heads", [(2, 2), (6, 2), (8, 2), (10, 2), (16, 2), (16, 1), (32, 8)])
+def test_gqa_group_sizes(q_heads, kv_heads):
+    """q_heads / kv_heads = 1, 3, 4, 5, 8, 16: the three instantiations (4, 8, 16 columns) with and without padding rows."""
+    w = read_workload("gqa", q_heads=q_heads, kv_heads=kv_heads, requests=[[(300, 1234), (129, -77)], [(515, 40000)]],
+                      seed=4242 + q_heads)
+    run_and_check(w)
+
+
+@pytest.mark.parametrize("pairing", ["neox", "gptj"])
+@pytest.mark.parametrize("R,off", [(128, 0), (64, 0), (64, 64), (32, 16)])
+def test_pairings_partial_rotary_and_window(pairing, R, off):
+    inv = inv_freq_llama3(5e5, R, 8.0, 1.0, 4.0, 8192)
+    w = read_workload("rot", q_heads=8, kv_heads=2, rotary_dim=R, rotary_offset=off, pairing=pairing, inv_freq=inv,
+                      requests=[[(257, 161), (64, 100000)]], seed=99 + R + off)
+    run_and_check(w)
+
+
+@pytest.mark.parametrize("lens", [[1], [127], [128], [129], [1, 1, 1], [255, 1, 384], [4096 + 17]])
+def test_ragged_lengths(lens):
+    w = read_workload("ragged", q_heads=8, kv_heads=2, requests=[[(L, 37 + 1000 * i) for i, L in enumerate(lens)]], seed=7 + sum(lens))
+    run_and_check(w)
+
+
+@pytest.mark.parametrize("tiles_per_item,max_ctas", [(1, 0), (1, 1), (3, 2), (2, 5), (32, 0)])
+def test_item_shapes_and_cta_counts(tiles_per_item, max_ctas):
+    """One tile per item (every tile a partial to merge), everything on one CTA (item transitions, every double buffer
+    wraps), a handful of CTAs: the decomposition never changes the result beyond the tolerance."""
+    w = read_workload("items", q_heads=16, kv_heads=4, requests=[[(1500, 2000), (700, 5)], [(129, -3)], [(2048, 77)]], seed=31337)
+    info, _ = run_and_check(w, tuning=dict(layers_per_unit=tiles_per_item, max_ctas=max_ctas))
+    if max_ctas:
+        assert info["grid"] <= max_ctas
+
+
+def test_padded_source_rows_every_layer_and_unsorted_requests():
+    w = read_workload("strides", q_heads=8, kv_heads=2, layers=3, pad=8,
+                      requests=[[(200, 10)], [(333, 20), (100, 30)], [(64, 40)]], seed=555)
+    w.segments = [w.segments[i] for i in (2, 0, 3, 1)]          # segments need not be grouped by request
+    for layer in range(3):
+        run_and_check(w, layer=layer)
+
+
+def test_large_scores_move_the_reference_maximum():
+    """Scaled-up queries: scores span hundreds of log2 units between tiles, so the lazily moved reference maximum and
+    the rescale of O^T in TMEM are exercised (a tile whose maximum exceeds the reference by more than 2^8)."""
+    from paper_2606_17107_b200 import kvr
+    from paper_2606_17107_b200.harness import DeviceReadWorkload
+    w = read_workload("hot", q_heads=8, kv_heads=2, requests=[[(1024, 9)]], seed=2024)
+    q = make_queries(w, "cpu")
+    q = (q.view(torch.bfloat16).to(torch.float32) * 16).to(torch.bfloat16).view(torch.int16)     # exact in bf16
+    srcs = make_read_sources(w, "cpu")
+    dw = DeviceReadWorkload(w, "cuda:0", sources=srcs, queries=q, guard_bytes=GUARD)
+    with kvr.Context(dw.model) as ctx:
+        ctx.set_tuning(max_ctas=1, layers_per_unit=8)
+        dw.run(ctx)
+        torch.cuda.synchronize()
+    o, lse = dw.o.cpu().numpy().astype(np.float64), dw.lse.cpu().numpy().astype(np.float64)
+    R = reference(w, [(np_bits(k), np_bits(v)) for k, v in srcs], np_bits(q), orc.host_threads())[0]
+    assert (np.abs(lse[0] - R["lse_model"]) <= 2.0 ** -8 + 1e-6 * np.abs(R["lse_model"])).all()
+    assert (np.abs(o[0] - R["o_model"]) <= 2.0 ** -7 * R["wabsv"] + 2.0 ** -12 * R["vmax"]).all()
+    assert (np.abs(lse[0] - R["lse_ref"]) <= R["E"] + 2.0 ** -8).all()
+
+
+def test_argument_errors_and_limits():
+    from paper_2606_17107_b200 import kvr
+    from paper_2606_17107_b200.harness import DeviceReadWorkload
+    w = read_workload("err", q_heads=8, kv_heads=2, requests=[[(130, 5)], [(64, 6)]], seed=1)
+    dw = DeviceReadWorkload(w, "cuda:0")
+    with kvr.Context(dw.model) as ctx:
+        call = lambda **kw: ctx.rotate_on_read_attention(
+            kw.get("q", dw.q), kw.get("n_req", 2), kw.get("q_heads", 8), kw.get("layer", 1), kw.get("scale", w.scale),
+            kw.get("segs", dw.segs), dw.o, dw.lse, check=False)
+        assert call() == kvr.KVR_OK
+        assert call(layer=2) == kvr.KVR_ERR_INVALID_ARG
+        assert call(q_heads=7) == kvr.KVR_ERR_INVALID_ARG
+        assert call(scale=0.0) == kvr.KVR_ERR_INVALID_ARG
+        assert call(n_req=3) == kvr.KVR_ERR_INVALID_ARG                 # request 2 owns no segment
+        assert call(q_heads=64) == kvr.KVR_ERR_UNSUPPORTED              # 32 query heads per kv head
+        assert call(q=dw.q.data_ptr() + 2) == kvr.KVR_ERR_ALIGNMENT
+        k, v = dw.sources[0]
+        bad = [kvr.read_segment(k, v, w.src_strides(w.segments[0]), 130, 5, 5)]
+        assert call(segs=bad) == kvr.KVR_ERR_INVALID_ARG                # request out of range
+        g = torch.cuda.CUDAGraph()
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            g.capture_begin()
+            st = ctx.rotate_on_read_attention(dw.q, 2, 8, 1, w.scale, dw.segs, dw.o, dw.lse, stream=s, check=False)
+            g.capture_end()
+        assert st == kvr.KVR_ERR_UNSUPPORTED
+        torch.cuda.synchronize()
+    w64 = read_workload("d64", q_heads=4, kv_heads=2, head_dim=64, requests=[[(64, 1)]], seed=2)
+    d64 = DeviceReadWorkload(w64, "cuda:0")
+    with kvr.Context(d64.model) as ctx:
+        assert d64.run.__func__ is not None
+        st = ctx.rotate_on_read_attention(d64.q, 1, 4, 1, w64.scale, d64.segs, d64.o, d64.lse, check=False)
+        assert st == kvr.KVR_ERR_UNSUPPORTED
+
+
+@pytest.mark.parametrize("name", ["attend-compose4", "attend-32k-x8", "attend-serving"])
+def test_full_size_sampled_requests(name):
+    """BASELINE-sized calls in the launch configuration bench.py times: the whole call runs on the GPU; the oracle
+    checks a sample of requests completely (every query head and dim of them)."""
+    from paper_2606_17107_b200 import kvr
+    from paper_2606_17107_b200.harness import DeviceReadWorkload
+    w = attention_config(name)
+    dw = DeviceReadWorkload(w, "cuda:0")
+    with kvr.Context(dw.model) as ctx:
+        dw.run(ctx)
+        torch.cuda.synchronize()
+        assert ctx.last_launch_info()["grid"] == torch.cuda.get_device_properties(0).multi_processor_count
+    o, lse = dw.o.cpu().numpy().astype(np.float64), dw.lse.cpu().numpy().astype(np.float64)
+    assert np.isfinite(o).all() and np.isfinite(lse).all()
+    sample = sorted({0, w.n_req // 2, w.n_req - 1})[: (1 if name == "attend-32k-x8" else 3)]
+    for r in sample:
+        idx = [i for i, s in enumerate(w.segments) if s.request == r]
+        sub = read_workload("sub", q_heads=w.q_heads, kv_heads=w.kv_heads, layers=w.layers, layer=w.layer,
+                            requests=[[(w.segments[i].len, w.segments[i].delta) for i in idx]], seed=0, inv_freq=w.inv_freq)
+        srcs = [(np_bits(dw.sources[i][0]), np_bits(dw.sources[i][1])) for i in idx]
+        R = reference(sub, srcs, np_bits(dw.q[r:r + 1]), orc.host_threads())[0]
+        assert (np.abs(o[r] - R["o_model"]) <= 2.0 ** -7 * R["wabsv"] + 2.0 ** -12 * R["vmax"]).all(), r
+        assert (np.abs(lse[r] - R["lse_model"]) <= 2.0 ** -8).all(), r
+        assert (np.abs(o[r] - R["o_ref"]) <= (np.expm1(2 * R["E"][:, None]) + 2.0 ** -8 + 2.0 ** -12) * R["vmax"]).all(), r
+        assert (np.abs(lse[r] - R["lse_ref"]) <= R["E"] + 2.0 ** -8).all(), r
