@@ -167,9 +167,17 @@ struct kvr_ctx {
   size_t aux_cap = 0;
   uint64_t h2d_bytes = 0;             // bytes the last host-source call copied host -> device
   // rotate-on-read attention (kvr_rotate_on_read_attention): descriptor staging ring, partial results, group tickets
-  struct AttnSlot { unsigned char* host = nullptr; unsigned char* dev = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; bool pending = false; };
-  AttnSlot attn_slots[4];
-  int attn_next = 0;
+  // A slot keeps the device-resident descriptors (tensor maps, work items) of one call, keyed by the call's segment
+  // array: a decode loop reads the same skills at every step and every layer, so the same call comes back and then
+  // enqueues nothing but its kernel.
+  struct AttnSlot {
+    unsigned char* host = nullptr; unsigned char* dev = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; bool pending = false;
+    std::vector<unsigned char> key; int32_t n_req = 0, q_heads = 0, tpi_tuning = 0, n_groups = 0;
+    size_t n_items = 0, seg_bytes = 0, n_merges = 0; uint64_t last_use = 0;
+  };
+  static constexpr int kAttnSlots = 8;
+  AttnSlot attn_slots[kAttnSlots];
+  uint64_t attn_clock = 0;
   float* attn_part = nullptr;         // [items][group][128 + 2]
   size_t attn_part_cap = 0;           // bytes
   unsigned int* attn_tickets = nullptr;
@@ -246,8 +254,8 @@ kvr_status kvr_create(kvr_ctx** out, const kvr_model_desc* model, int cuda_devic
   if (e == cudaSuccess) e = cudaMalloc(&c->d_status, 4 * sizeof(int32_t));
   if (e == cudaSuccess) e = cudaMemset(c->d_status, 0, 4 * sizeof(int32_t));
   if (e == cudaSuccess) e = cudaMallocHost(&c->h_status, 4 * sizeof(int32_t));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_sched, 2 * sizeof(unsigned long long));
-  if (e == cudaSuccess) e = cudaMemset(c->d_sched, 0, 2 * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_sched, 4 * sizeof(unsigned long long));   // [0..1] ring kernel, [2..3] attention kernel
+  if (e == cudaSuccess) e = cudaMemset(c->d_sched, 0, 4 * sizeof(unsigned long long));
   for (int i = 0; i < kSlots && e == cudaSuccess; ++i)
     e = cudaEventCreateWithFlags(&c->slots[i].ev, cudaEventDisableTiming);
   // every staging slot is usable from the first call on (a call under stream capture cannot allocate)
@@ -676,71 +684,94 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
     return KVR_ERR_UNSUPPORTED;
   }
 
-  // ---- work decomposition: items = (segment, kv head, run of key tiles); groups = (request, kv head) ----
-  std::vector<int32_t> order((size_t)n);
-  for (int32_t i = 0; i < n; ++i) order[(size_t)i] = i;
-  std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return segs[a].request < segs[b].request; });
-  int64_t total_tiles = 0;
-  for (int32_t i = 0; i < n; ++i) total_tiles += ((int64_t)segs[i].len + 127) / 128;
-  total_tiles *= m.kv_heads;
-  // ~4 items per SM when the call is large enough; 2..32 tiles (256..4096 keys) per item; tuning.layers_per_unit
-  // doubles as "tiles per item" for experiments (this call has no layers to group)
-  int64_t tpi = (total_tiles + 4ll * c->sm_count - 1) / (4ll * c->sm_count);
-  tpi = tpi < 2 ? 2 : (tpi > 32 ? 32 : tpi);
-  if (c->tuning.layers_per_unit > 0) tpi = c->tuning.layers_per_unit;
-  std::vector<AttnItem> items;
-  items.reserve((size_t)(total_tiles / tpi + (int64_t)n * m.kv_heads));
-  int32_t n_groups = 0;
-  for (size_t a = 0; a < order.size();) {
-    size_t b = a;
-    while (b < order.size() && segs[order[b]].request == segs[order[a]].request) ++b;
-    const int32_t r = segs[order[a]].request;
-    for (int32_t h = 0; h < m.kv_heads; ++h) {
-      const int32_t first = (int32_t)items.size();
-      for (size_t j = a; j < b; ++j) {
-        const int32_t si = order[j], len = segs[si].len;
-        for (int32_t k0 = 0; k0 < len; k0 += (int32_t)tpi * 128) {
-          AttnItem it{};
-          it.seg = si; it.head = h; it.key0 = k0; it.n_keys = std::min<int32_t>((int32_t)tpi * 128, len - k0);
-          it.group = n_groups; it.group_first = first; it.out_q0 = r * q_heads + h * group;
-          items.push_back(it);
-        }
-      }
-      const int32_t cnt = (int32_t)items.size() - first;
-      for (int32_t j = first; j < first + cnt; ++j) items[(size_t)j].group_count = cnt;
-      ++n_groups;
-    }
-    a = b;
+  // ---- descriptors: cached per distinct segment array ----
+  const size_t key_bytes = (size_t)n * sizeof(kvr_read_segment);
+  kvr_ctx::AttnSlot* slot_p = nullptr;
+  for (auto& a : c->attn_slots)
+    if (a.key.size() == key_bytes && a.n_req == n_req && a.q_heads == q_heads && a.tpi_tuning == c->tuning.layers_per_unit &&
+        std::memcmp(a.key.data(), segs, key_bytes) == 0) { slot_p = &a; break; }
+  const bool hit = slot_p != nullptr;
+  if (!hit) {
+    slot_p = &c->attn_slots[0];
+    for (auto& a : c->attn_slots) if (a.last_use < slot_p->last_use) slot_p = &a;     // least recently used
   }
-  const size_t n_items = items.size();
-
-  // ---- staging: [AttnSeg x n][AttnItem x n_items] through one pinned slot and one H2D copy ----
-  const size_t seg_bytes = (size_t)n * sizeof(AttnSeg), bytes = seg_bytes + n_items * sizeof(AttnItem);
-  kvr_ctx::AttnSlot& slot = c->attn_slots[c->attn_next];
-  c->attn_next = (c->attn_next + 1) % 4;
-  if (slot.pending) { KVR_CUDA(c, cudaEventSynchronize(slot.ev)); slot.pending = false; }
+  kvr_ctx::AttnSlot& slot = *slot_p;
+  slot.last_use = ++c->attn_clock;
   if (!slot.ev) KVR_CUDA(c, cudaEventCreateWithFlags(&slot.ev, cudaEventDisableTiming));
-  if (bytes > slot.cap) {
-    size_t cap = slot.cap ? slot.cap : (size_t)1 << 16;
-    while (cap < bytes) cap *= 2;
-    if (slot.host) cudaFreeHost(slot.host);
-    if (slot.dev) cudaFree(slot.dev);
-    slot.host = nullptr; slot.dev = nullptr; slot.cap = 0;
-    KVR_CUDA(c, cudaMallocHost(&slot.host, cap));
-    KVR_CUDA(c, cudaMalloc(&slot.dev, cap));
-    slot.cap = cap;
-  }
-  AttnSeg* hs = reinterpret_cast<AttnSeg*>(slot.host);
-  for (int32_t i = 0; i < n; ++i) {
-    const kvr_read_segment& s = segs[i];
-    if (!encode_attn_map(&hs[i].k, s.k_src, m.kv_heads, s.len, m.layers, s.src_stride_layer, s.src_stride_head, s.src_stride_token) ||
-        !encode_attn_map(&hs[i].v, s.v_src, m.kv_heads, s.len, m.layers, s.src_stride_layer, s.src_stride_head, s.src_stride_token)) {
-      c->last_err = "rotate-on-read attention: a source tensor cannot be described by a TMA tensor map";
-      return KVR_ERR_UNSUPPORTED;
+  if (!hit) {
+    if (slot.pending) { KVR_CUDA(c, cudaEventSynchronize(slot.ev)); slot.pending = false; }
+    slot.key.clear();
+    // ---- work decomposition: items = (segment, kv head, run of key tiles); groups = (request, kv head) ----
+    std::vector<int32_t> order((size_t)n);
+    for (int32_t i = 0; i < n; ++i) order[(size_t)i] = i;
+    std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return segs[a].request < segs[b].request; });
+    int64_t total_tiles = 0;
+    for (int32_t i = 0; i < n; ++i) total_tiles += ((int64_t)segs[i].len + 127) / 128;
+    total_tiles *= m.kv_heads;
+    // ~8 items per SM when the call is large enough (items are handed out dynamically: the tail is at most one item);
+    // 4..16 tiles (512..2048 keys) per item; tuning.layers_per_unit doubles as "tiles per item" for experiments (this
+    // call has no layers to group)
+    int64_t tpi = (total_tiles + 8ll * c->sm_count - 1) / (8ll * c->sm_count);
+    tpi = tpi < 4 ? 4 : (tpi > 16 ? 16 : tpi);
+    if (c->tuning.layers_per_unit > 0) tpi = c->tuning.layers_per_unit;
+    std::vector<AttnItem> items;
+    std::vector<AttnMerge> merges;
+    items.reserve((size_t)(total_tiles / tpi + (int64_t)n * m.kv_heads));
+    int32_t n_groups = 0;
+    for (size_t a = 0; a < order.size();) {
+      size_t b = a;
+      while (b < order.size() && segs[order[b]].request == segs[order[a]].request) ++b;
+      for (int32_t h = 0; h < m.kv_heads; ++h) {
+        const int32_t first = (int32_t)items.size();
+        for (size_t j = a; j < b; ++j) {
+          const int32_t si = order[j], len = segs[si].len;
+          for (int32_t k0 = 0; k0 < len; k0 += (int32_t)tpi * 128) {
+            AttnItem it{};
+            it.seg = si; it.head = h; it.key0 = k0; it.n_keys = std::min<int32_t>((int32_t)tpi * 128, len - k0);
+            it.group = n_groups; it.group_first = first; it.index = (int32_t)items.size();
+            items.push_back(it);
+          }
+        }
+        const int32_t cnt = (int32_t)items.size() - first;
+        const bool defer = cnt > attend_inline_merge_limit(group);      // merged by the merge kernel after the grid
+        for (int32_t j = first; j < first + cnt; ++j) items[(size_t)j].group_count = defer ? -cnt : cnt;
+        if (defer) merges.push_back(AttnMerge{first, cnt, segs[order[a]].request * q_heads + h * group, 0});
+        ++n_groups;
+      }
+      a = b;
     }
-    hs[i].delta = s.delta; hs[i].len = s.len; hs[i].request = s.request; hs[i].pad_ = 0;
+    // ---- staging: [AttnSeg x n][AttnItem x n_items] through the slot's pinned buffer and one H2D copy ----
+    const size_t seg_bytes = (size_t)n * sizeof(AttnSeg), item_bytes = items.size() * sizeof(AttnItem),
+                 bytes = seg_bytes + item_bytes + merges.size() * sizeof(AttnMerge);
+    if (bytes > slot.cap) {
+      size_t cap = slot.cap ? slot.cap : (size_t)1 << 16;
+      while (cap < bytes) cap *= 2;
+      if (slot.host) cudaFreeHost(slot.host);
+      if (slot.dev) cudaFree(slot.dev);
+      slot.host = nullptr; slot.dev = nullptr; slot.cap = 0;
+      KVR_CUDA(c, cudaMallocHost(&slot.host, cap));
+      KVR_CUDA(c, cudaMalloc(&slot.dev, cap));
+      slot.cap = cap;
+    }
+    AttnSeg* hs = reinterpret_cast<AttnSeg*>(slot.host);
+    for (int32_t i = 0; i < n; ++i) {
+      const kvr_read_segment& sg = segs[i];
+      if (!encode_attn_map(&hs[i].k, sg.k_src, m.kv_heads, sg.len, m.layers, sg.src_stride_layer, sg.src_stride_head, sg.src_stride_token) ||
+          !encode_attn_map(&hs[i].v, sg.v_src, m.kv_heads, sg.len, m.layers, sg.src_stride_layer, sg.src_stride_head, sg.src_stride_token)) {
+        c->last_err = "rotate-on-read attention: a source tensor cannot be described by a TMA tensor map";
+        return KVR_ERR_UNSUPPORTED;
+      }
+      hs[i].delta = sg.delta; hs[i].len = sg.len; hs[i].request = sg.request; hs[i].pad_ = 0;
+    }
+    std::memcpy(slot.host + seg_bytes, items.data(), item_bytes);
+    if (!merges.empty()) std::memcpy(slot.host + seg_bytes + item_bytes, merges.data(), merges.size() * sizeof(AttnMerge));
+    KVR_CUDA(c, cudaMemcpyAsync(slot.dev, slot.host, bytes, cudaMemcpyHostToDevice, stream));
+    slot.n_items = items.size(); slot.seg_bytes = seg_bytes; slot.n_groups = n_groups; slot.n_merges = merges.size();
+    slot.n_req = n_req; slot.q_heads = q_heads; slot.tpi_tuning = c->tuning.layers_per_unit;
+    slot.key.assign(reinterpret_cast<const unsigned char*>(segs), reinterpret_cast<const unsigned char*>(segs) + key_bytes);
   }
-  std::memcpy(slot.host + seg_bytes, items.data(), n_items * sizeof(AttnItem));
+  const size_t n_items = slot.n_items, seg_bytes = slot.seg_bytes;
+  const int32_t n_groups = slot.n_groups;
   // partial results and tickets (grown on demand; a regrowth waits for the launches that may still use the old buffers)
   const size_t part_bytes = n_items * (size_t)group * (128 + 2) * sizeof(float);
   if (part_bytes > c->attn_part_cap || (size_t)n_groups > c->attn_ticket_cap) {
@@ -761,13 +792,14 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
       c->attn_ticket_cap = cap;
     }
   }
-  KVR_CUDA(c, cudaMemcpyAsync(slot.dev, slot.host, bytes, cudaMemcpyHostToDevice, stream));
 
   AttnParams P{};
   P.q = static_cast<const uint16_t*>(q); P.o = o; P.lse = lse;
   P.segs = reinterpret_cast<const AttnSeg*>(slot.dev);
   P.items = reinterpret_cast<const AttnItem*>(slot.dev + seg_bytes);
   P.n_items = (int32_t)n_items;
+  P.merges = reinterpret_cast<const AttnMerge*>(slot.dev + seg_bytes + n_items * sizeof(AttnItem));
+  P.n_merges = (int32_t)slot.n_merges;
   P.q_heads = q_heads; P.group = group; P.layer = layer;
   P.rotary_dim = m.rotary_dim; P.rotary_offset = m.rotary_offset; P.pairing = m.pairing;
   P.scale_log2 = (float)((double)softmax_scale * 1.4426950408889634);
@@ -775,10 +807,11 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
   P.part_o = c->attn_part;
   P.part_ml = c->attn_part + n_items * (size_t)group * 128;
   P.tickets = c->attn_tickets;
+  P.sched = c->d_sched + 2;
   cudaError_t e = launch_attend(P, c->tuning.max_ctas > 0 ? std::min(c->tuning.max_ctas, c->sm_count) : c->sm_count, stream,
                                 &c->last_grid, &c->last_block, &c->last_smem);
   if (e != cudaSuccess) return c->cuda_fail(e, "launch_attend");
-  c->launches += 1;
+  c->launches += 1 + (slot.n_merges ? 1 : 0);
   c->last_path = 3;
   c->last_stream = stream;
   KVR_CUDA(c, cudaEventRecord(slot.ev, stream));

@@ -14,12 +14,16 @@ struct alignas(64) AttnSeg {
 };
 
 // One work item: keys [key0, key0 + n_keys) of kv head `head` of segment `seg`.  Items of one (request, kv head) group
-// are numbered consecutively: [group_first, group_first + group_count).
+// are numbered consecutively: [group_first, group_first + |group_count|); group_count < 0: the group is merged after
+// the grid (AttnMerge), its items only write their partials.
 struct AttnItem {
   int32_t seg, head, key0, n_keys;
   int32_t group, group_first, group_count;
-  int32_t out_q0;          // row of the group's first query head in o / lse: request * q_heads + head * (q_heads / kv_heads)
+  int32_t index;           // this item's own number (its slot in the partial buffers); items are handed out dynamically
 };
+
+// A group whose partials are merged after the attention grid (kvr_attend_merge_kernel): partials [first, first + count).
+struct AttnMerge { int32_t first, count, out_q0, pad_; };
 
 struct AttnParams {
   const uint16_t* q;       // bf16 [n_req][q_heads][128]
@@ -27,7 +31,8 @@ struct AttnParams {
   float* lse;              // [n_req][q_heads]
   const AttnSeg* segs;
   const AttnItem* items;
-  int32_t n_items;
+  const AttnMerge* merges;
+  int32_t n_items, n_merges;
   int32_t q_heads, group;  // group = q_heads / kv_heads
   int32_t layer, rotary_dim, rotary_offset, pairing;
   float scale_log2;        // softmax_scale * log2(e)
@@ -35,8 +40,11 @@ struct AttnParams {
   float* part_o;           // [n_items][group][128]: unnormalised O^T of an item, relative to its reference maximum
   float* part_ml;          // [n_items][group][2]: reference maximum (log2 units), row sum
   unsigned int* tickets;   // [groups]: items of the group that have finished; zero between launches
+  unsigned long long* sched;   // [0] next item to hand out (beyond the first, static one per CTA), [1] CTAs that have
+                               // finished; both zero between launches (the last CTA to finish resets them)
 };
 
+int attend_inline_merge_limit(int group);   // groups with more partials are merged by the merge kernel
 cudaError_t launch_attend(const AttnParams& P, int sm_count, cudaStream_t stream, int* grid, int* block, int* smem);
 
 }  // namespace kvr
