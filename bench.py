@@ -632,6 +632,23 @@ def run_attend(args):
     flops = 4.0 * w.q_heads * w.head_dim * w.tokens
     achieved = b / (exact_s / steps) / 1e9
     ctx.close()
+    # the oracle (as it stands) on the host cores, over request 0 of the workload, scaled by tokens
+    cpu = None
+    if rep.world == 1 and not args.no_cpu_baseline:
+        from oracle import kvr_oracle as orc
+        seg0 = [(i, s_) for i, s_ in enumerate(w.segments) if s_.request == 0]
+        srcs0 = [(bits_to_numpy(dws[0].sources[i][0][w.layer]), bits_to_numpy(dws[0].sources[i][1][w.layer]), s_.delta) for i, s_ in seg0]
+        q0 = bits_to_numpy(dws[0].q[0])
+        threads = min(orc.host_threads(), w.q_heads)
+        kw = dict(q=q0, kv_heads=w.kv_heads, rotary_dim=w.rotary_dim, pairing={"neox": 0, "gptj": 1}[w.pairing],
+                  inv_freq=w.inv_freq, scale=w.scale, segments=srcs0, n_threads=threads)
+        orc.rotate_on_read_attention(**kw)
+        t0 = time.perf_counter()
+        for _ in range(3):
+            orc.rotate_on_read_attention(**kw)
+        tok0 = sum(s_.len for _, s_ in seg0)
+        cpu = {"value": tok0 / ((time.perf_counter() - t0) / 3), "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"request 0 of {w.n_req} ({tok0} of {w.tokens} tokens, every query head), 3 passes after 1 warm-up"}
     if rep.rank == 0:
         line = {
             "metric": "KV tokens attended by rotate-on-read/sec (one layer)", "value": w.tokens * rep.world / (exact_s / steps),
@@ -650,7 +667,7 @@ def run_attend(args):
                          "traffic": traffic_of(w.name, "src", "attend"), "peak_source": peak_src,
                          "median_achieved": b / med / 1e9, "best_achieved": b / best / 1e9, "spread": (worst - best) / med,
                          "blocks": len(blk), "tensor_tflops": flops / (exact_s / steps) / 1e12},
-            "e2e": None, "cpu_baseline": None,
+            "e2e": None, "cpu_baseline": cpu,
         }
         print(json.dumps(line), flush=True)
     rep.close()

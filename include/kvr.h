@@ -252,9 +252,14 @@ KVR_API kvr_status kvr_write_span(kvr_ctx* ctx, const kvr_paged_dst* dst, const 
  * weights are rounded to bf16 before they multiply V and their row sum adds the rounded weights.
  * Limits (else KVR_ERR_UNSUPPORTED): KVR_BF16 caches, head_dim == 128, q_heads / kv_heads <= 16.  Every request must
  * own at least one segment; k_src / v_src as in kvr_segment (DEVICE, [layers][kv_heads][len][head_dim], element strides,
- * 16-byte aligned).  Asynchronous on `cuda_stream`; descriptors are staged through context-owned pinned memory, so the
- * call cannot be captured in a CUDA graph (KVR_ERR_UNSUPPORTED under capture).  Reads 2 * kv_heads * head_dim * 2 bytes
- * per token (kvr_attention_bytes_read): K and V of one layer, once. */
+ * 16-byte aligned).  Asynchronous on `cuda_stream`; descriptors (TMA tensor maps, work items) are built on the host,
+ * staged through context-owned pinned memory and CACHED per distinct segment array (8 entries, least recently used
+ * replaced): a decode loop that reads the same skills at every step and layer enqueues nothing but its kernels from
+ * the second call on.  Not capturable in a CUDA graph (KVR_ERR_UNSUPPORTED under capture).  One or two kernels per
+ * call (the second merges the partial results of (request, kv head) groups that were split over many CTAs).  Reads
+ * 2 * kv_heads * head_dim * 2 bytes per token (kvr_attention_bytes_read): K and V of one layer, once.  Outputs are
+ * written only by this call's kernels; partial results live in context-owned device memory, so calls on one context
+ * must be issued to one stream at a time (as for every other call). */
 typedef struct {
   const void* k_src;
   const void* v_src;

@@ -688,7 +688,7 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
   const size_t key_bytes = (size_t)n * sizeof(kvr_read_segment);
   kvr_ctx::AttnSlot* slot_p = nullptr;
   for (auto& a : c->attn_slots)
-    if (a.key.size() == key_bytes && a.n_req == n_req && a.q_heads == q_heads && a.tpi_tuning == c->tuning.layers_per_unit &&
+    if (a.key.size() == key_bytes && a.n_req == n_req && a.q_heads == q_heads && a.tpi_tuning == c->tuning.layers_per_unit + 1000 * c->tuning.hsplit &&
         std::memcmp(a.key.data(), segs, key_bytes) == 0) { slot_p = &a; break; }
   const bool hit = slot_p != nullptr;
   if (!hit) {
@@ -709,10 +709,11 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
     for (int32_t i = 0; i < n; ++i) total_tiles += ((int64_t)segs[i].len + 127) / 128;
     total_tiles *= m.kv_heads;
     // ~8 items per SM when the call is large enough (items are handed out dynamically: the tail is at most one item);
-    // 4..16 tiles (512..2048 keys) per item; tuning.layers_per_unit doubles as "tiles per item" for experiments (this
-    // call has no layers to group)
+    // 4..8 tiles (512..1024 keys) per item -- B200: 8 beats 16 by 1-4 % on the serving and 32k workloads, 4 beats 8 on
+    // the small compose call; tuning.layers_per_unit doubles as "tiles per item" for experiments (this call has no
+    // layers to group)
     int64_t tpi = (total_tiles + 8ll * c->sm_count - 1) / (8ll * c->sm_count);
-    tpi = tpi < 4 ? 4 : (tpi > 16 ? 16 : tpi);
+    tpi = tpi < 4 ? 4 : (tpi > 8 ? 8 : tpi);
     if (c->tuning.layers_per_unit > 0) tpi = c->tuning.layers_per_unit;
     std::vector<AttnItem> items;
     std::vector<AttnMerge> merges;
@@ -733,7 +734,7 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
           }
         }
         const int32_t cnt = (int32_t)items.size() - first;
-        const bool defer = cnt > attend_inline_merge_limit(group);      // merged by the merge kernel after the grid
+        const bool defer = cnt > (c->tuning.hsplit > 0 ? c->tuning.hsplit : attend_inline_merge_limit(group));   // merged after the grid (tuning.hsplit overrides the limit)
         for (int32_t j = first; j < first + cnt; ++j) items[(size_t)j].group_count = defer ? -cnt : cnt;
         if (defer) merges.push_back(AttnMerge{first, cnt, segs[order[a]].request * q_heads + h * group, 0});
         ++n_groups;
@@ -767,7 +768,7 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
     if (!merges.empty()) std::memcpy(slot.host + seg_bytes + item_bytes, merges.data(), merges.size() * sizeof(AttnMerge));
     KVR_CUDA(c, cudaMemcpyAsync(slot.dev, slot.host, bytes, cudaMemcpyHostToDevice, stream));
     slot.n_items = items.size(); slot.seg_bytes = seg_bytes; slot.n_groups = n_groups; slot.n_merges = merges.size();
-    slot.n_req = n_req; slot.q_heads = q_heads; slot.tpi_tuning = c->tuning.layers_per_unit;
+    slot.n_req = n_req; slot.q_heads = q_heads; slot.tpi_tuning = c->tuning.layers_per_unit + 1000 * c->tuning.hsplit;
     slot.key.assign(reinterpret_cast<const unsigned char*>(segs), reinterpret_cast<const unsigned char*>(segs) + key_bytes);
   }
   const size_t n_items = slot.n_items, seg_bytes = slot.seg_bytes;

@@ -13,16 +13,29 @@
 //                                                                 B = Q'       (16 rows x 128 dims, K-major, SW128)
 //     O^T [128 dims x 16] += V^T[128 dims x 128 keys] . P^T       A = V tile   (MN-major, SW128, straight from TMA)
 //                                                                 B = P        (16 rows x 128 keys, K-major, SW128)
-// One CTA per SM, persistent over work items (segment, kv head, run of <= kTilesMax key tiles), warp-specialised:
-//   warp 0      TMA producer: K and V tiles (2 x 64-dim panels of 128 keys each) into a ring of kStages stages
-//   warp 1      MMA issuer (one elected lane): tcgen05.mma kind::f16, accumulators in TMEM (S double-buffered, O)
-//   warps 2-3   query warps: fp64 sincos of -Delta * inv_freq, rotate the item's query heads, round once to bf16,
-//               write Q' in the swizzled operand layout (double-buffered, one item ahead)
+// One CTA per SM (384 threads, ~211 KB of shared memory, 64 TMEM columns), persistent over work items = (segment, kv
+// head, run of 4..8 key tiles of 128 keys), warp-specialised:
+//   warp 0 / 2  TMA producers (one elected lane each): K tiles / V tiles, each a pair of 64-dim panels of 128 keys
+//               (SWIZZLE_128B tensor loads), into rings of kKS / kVS slots of 32 KB.  The rings are separate because
+//               a K slot is free as soon as S^T is computed, while a V slot is held until P^T has multiplied it.
+//   warp 1      MMA issuer (one elected lane): tcgen05.mma kind::f16 (M 128, N 16, K 16), accumulators in TMEM: S^T
+//               double-buffered by tile, O^T double-buffered by item; the first S^T of the next item is issued before
+//               the last P.V of this one is waited for.
+//   warp 3      scheduler + query warp: lane 0 draws items (the first statically, the rest from one global counter, a
+//               draw ahead) and publishes them to the other roles through a 4-slot ring in shared memory; the warp
+//               then builds the item's Q' = R(-Delta) q (fp64 sincos, one rounding to bf16) in the swizzled operand
+//               layout, double-buffered, an item ahead of the MMAs.
 //   warps 4-7   softmax: thread i owns key i of the tile (TMEM lane i): tcgen05.ld of its <= 16 scores, tile maximum by
-//               warp shuffles + one named barrier, exp2, P^T to shared memory as the next MMA's B operand; the running
+//               warp shuffles + ONE named barrier, exp2, P^T to shared memory as the next MMA's B operand.  The
 //               reference maximum only moves when a tile exceeds it by 2^8 (O^T is then rescaled in TMEM: 16 columns,
-//               one tcgen05.ld/st pair per thread); at the end of an item O^T, the row sums and the reference go to
-//               the partial buffer and the LAST item of a (request, kv head) group merges the group's partials.
+//               one tcgen05.ld/st pair per thread).  At the end of an item the reference and the row sums go to the
+//               epilogue warps through shared memory and the next item starts at once.
+//   warps 8-11  epilogue, off the critical path: O^T (thread = dim) of a finished item goes to the output (a group of
+//               one item) or to the partial buffer.  A (request, kv head) group of few partials is merged by its last
+//               item (device-scope fence + ticket); a group of many is left to kvr_attend_merge_kernel after the
+//               grid, because under a saturated HBM every dependent load of an in-kernel merge costs microseconds
+//               (measured: a 512-partial in-kernel merge was a 600 us serial tail).
+// Programmatic dependent launch: the prologue (barriers, TMEM allocation) overlaps the tail of the previous launch.
 #include <mutex>
 
 #include "kvr_attend.cuh"

@@ -158,6 +158,36 @@ def test_item_shapes_and_cta_counts(tiles_per_item, max_ctas):
         assert info["grid"] <= max_ctas
 
 
+@pytest.mark.parametrize("inline_limit", [1, 3, 64])
+def test_merge_in_kernel_and_by_the_merge_kernel(inline_limit):
+    """Groups of 1, 2, 5 and 24 partials in one call, merged by the group's last item (few partials) or by
+    kvr_attend_merge_kernel after the grid (many): tuning.hsplit overrides the limit between the two."""
+    w = read_workload("merge", q_heads=8, kv_heads=2, requests=[[(100, 1)], [(256, 2)], [(640, 3)], [(3000, 4)]], seed=808)
+    run_and_check(w, tuning=dict(layers_per_unit=1, hsplit=inline_limit))
+
+
+def test_descriptor_cache_hits_and_evictions():
+    """Twelve different calls through ONE context, round robin, three rounds: more distinct segment arrays than the
+    8-entry descriptor cache holds, so entries are rebuilt, reused and evicted while earlier launches are in flight."""
+    from paper_2606_17107_b200 import kvr
+    from paper_2606_17107_b200.harness import DeviceReadWorkload
+    ws = [read_workload(f"c{i}", q_heads=8, kv_heads=2, requests=[[(130 + 37 * i, 10 * i + 1)], [(64 + i, 5)]], seed=900 + i)
+          for i in range(12)]
+    dws = [DeviceReadWorkload(w, "cuda:0") for w in ws]
+    with kvr.Context(dws[0].model) as ctx:
+        for _ in range(3):
+            for dw in dws:
+                dw.run(ctx)
+        torch.cuda.synchronize()
+    for w, dw in zip(ws, dws):
+        srcs = [(np_bits(k), np_bits(v)) for k, v in dw.sources]
+        ref = reference(w, srcs, np_bits(dw.q), orc.host_threads())
+        o, lse = dw.o.cpu().numpy().astype(np.float64), dw.lse.cpu().numpy().astype(np.float64)
+        for r, R in enumerate(ref):
+            assert (np.abs(o[r] - R["o_model"]) <= 2.0 ** -7 * R["wabsv"] + 2.0 ** -12 * R["vmax"]).all(), (w.name, r)
+            assert (np.abs(lse[r] - R["lse_model"]) <= 2.0 ** -8).all(), (w.name, r)
+
+
 def test_padded_source_rows_every_layer_and_unsorted_requests():
     w = read_workload("strides", q_heads=8, kv_heads=2, layers=3, pad=8,
                       requests=[[(200, 10)], [(333, 20), (100, 30)], [(64, 40)]], seed=555)
