@@ -173,7 +173,7 @@ struct kvr_ctx {
   struct AttnSlot {
     unsigned char* host = nullptr; unsigned char* dev = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; bool pending = false;
     std::vector<unsigned char> key; int32_t n_req = 0, q_heads = 0, tpi_tuning = 0, n_groups = 0;
-    size_t n_items = 0, seg_bytes = 0, n_merges = 0; uint64_t last_use = 0;
+    size_t n_items = 0, seg_bytes = 0, n_merges = 0; int32_t merge_max = 0; uint64_t last_use = 0;
   };
   static constexpr int kAttnSlots = 8;
   AttnSlot attn_slots[kAttnSlots];
@@ -768,6 +768,8 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
     if (!merges.empty()) std::memcpy(slot.host + seg_bytes + item_bytes, merges.data(), merges.size() * sizeof(AttnMerge));
     KVR_CUDA(c, cudaMemcpyAsync(slot.dev, slot.host, bytes, cudaMemcpyHostToDevice, stream));
     slot.n_items = items.size(); slot.seg_bytes = seg_bytes; slot.n_groups = n_groups; slot.n_merges = merges.size();
+    slot.merge_max = 0;
+    for (const AttnMerge& mg : merges) slot.merge_max = std::max(slot.merge_max, mg.count);
     slot.n_req = n_req; slot.q_heads = q_heads; slot.tpi_tuning = c->tuning.layers_per_unit + 1000 * c->tuning.hsplit;
     slot.key.assign(reinterpret_cast<const unsigned char*>(segs), reinterpret_cast<const unsigned char*>(segs) + key_bytes);
   }
@@ -801,6 +803,7 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
   P.n_items = (int32_t)n_items;
   P.merges = reinterpret_cast<const AttnMerge*>(slot.dev + seg_bytes + n_items * sizeof(AttnItem));
   P.n_merges = (int32_t)slot.n_merges;
+  P.merge_max_count = slot.merge_max;
   P.q_heads = q_heads; P.group = group; P.layer = layer;
   P.rotary_dim = m.rotary_dim; P.rotary_offset = m.rotary_offset; P.pairing = m.pairing;
   P.scale_log2 = (float)((double)softmax_scale * 1.4426950408889634);

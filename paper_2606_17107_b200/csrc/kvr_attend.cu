@@ -614,7 +614,7 @@ __global__ void __launch_bounds__(kThreads, 1) kvr_attend_kernel(const __grid_co
 // attention grid: one CTA per (group, query head); thread = (slice of the group's partials, dim).  Under a saturated
 // HBM a dependent load costs several microseconds, so the in-kernel merge of a long group would be a serial tail of
 // (partials / 8) such latencies; here the machine is idle, every thread has 32 loads in flight and 4 slices share a group.
-constexpr int kMergeSlices = 4;
+template <int kMergeSlices>      // 4: long groups; 1: every group has <= 32 partials (a slice per group, 4x the CTAs per SM)
 __global__ void __launch_bounds__(128 * kMergeSlices) kvr_attend_merge_kernel(const AttnMerge* __restrict__ merges, int G,
                                                                               const float* __restrict__ part_o,
                                                                               const float* __restrict__ part_ml,
@@ -702,12 +702,15 @@ cudaError_t launch_attend(const AttnParams& P, int sm_count, cudaStream_t stream
                 : P.group <= 8 ? launch_attend_inst<8>(P, grid, stream) : launch_attend_inst<16>(P, grid, stream);
   if (e != cudaSuccess || P.n_merges == 0) return e;
   cudaLaunchConfig_t lc{};
-  lc.gridDim = dim3((unsigned)(P.n_merges * P.group)); lc.blockDim = dim3(128 * kMergeSlices); lc.dynamicSmemBytes = 0; lc.stream = stream;
+  const int slices = P.merge_max_count <= 32 ? 1 : 4;
+  lc.gridDim = dim3((unsigned)(P.n_merges * P.group)); lc.blockDim = dim3(128 * slices); lc.dynamicSmemBytes = 0; lc.stream = stream;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = at; lc.numAttrs = 1;
-  return cudaLaunchKernelEx(&lc, kvr_attend_merge_kernel, P.merges, (int)P.group, (const float*)P.part_o, (const float*)P.part_ml, P.o, P.lse);
+  return slices == 1
+      ? cudaLaunchKernelEx(&lc, kvr_attend_merge_kernel<1>, P.merges, (int)P.group, (const float*)P.part_o, (const float*)P.part_ml, P.o, P.lse)
+      : cudaLaunchKernelEx(&lc, kvr_attend_merge_kernel<4>, P.merges, (int)P.group, (const float*)P.part_o, (const float*)P.part_ml, P.o, P.lse);
 }
 
 // partials the in-kernel merge takes in one step (the loads of a step are in flight together)
