@@ -277,3 +277,34 @@ def test_full_size_sampled_requests(name):
         assert (np.abs(lse[r] - R["lse_model"]) <= 2.0 ** -8).all(), r
         assert (np.abs(o[r] - R["o_ref"]) <= (np.expm1(2 * R["E"][:, None]) + 2.0 ** -8 + 2.0 ** -12) * R["vmax"]).all(), r
         assert (np.abs(lse[r] - R["lse_ref"]) <= R["E"] + 2.0 ** -8).all(), r
+
+
+@pytest.mark.parametrize("case", range(40))
+def test_fuzz_shapes_and_decompositions(case):
+    """Seeded random calls: GQA group 1..16, 1-8 kv heads, 1-5 requests of 1-4 segments of 1-3000 tokens, shifts up to
+    +-2^30 (the fp64 sincos slow path), both pairings, partial rotary windows, padded rows, random tiles per item, CTA
+    counts and in-kernel merge limits -- every one against the oracle and the bf16-query model."""
+    rng = np.random.default_rng(77000 + case)
+    kv_heads = int(rng.choice([1, 2, 4, 8]))
+    group = int(rng.choice([1, 2, 3, 4, 5, 7, 8, 12, 16]))
+    R = int(rng.choice([128, 128, 64, 32]))
+    off = int(rng.choice([0, 0, 16, 128 - R])) if R < 128 else 0
+    off = min(off, 128 - R)
+    reqs = []
+    for _ in range(int(rng.integers(1, 6))):
+        lst = []
+        for _ in range(int(rng.integers(1, 5))):
+            L = int(rng.choice([1, int(rng.integers(2, 200)), int(rng.integers(200, 3000))]))
+            big = rng.random() < 0.2
+            d = int(rng.integers(-(1 << 30), 1 << 30)) if big else int(rng.integers(-5000, 200000))
+            lst.append((L, d))
+        reqs.append(lst)
+    w = read_workload(f"fuzz{case}", q_heads=kv_heads * group, kv_heads=kv_heads, rotary_dim=R, rotary_offset=off,
+                      pairing=str(rng.choice(["neox", "gptj"])), theta=float(rng.choice([1e4, 5e5, 1e6])),
+                      layers=int(rng.integers(1, 4)), layer=0, pad=int(rng.choice([0, 0, 8, 24])), requests=reqs, seed=88000 + case)
+    w.layer = int(rng.integers(0, w.layers))
+    perm = rng.permutation(len(w.segments))
+    w.segments = [w.segments[i] for i in perm]
+    tuning = dict(layers_per_unit=int(rng.choice([0, 1, 2, 3, 5])), max_ctas=int(rng.choice([0, 0, 1, 3, 17])),
+                  hsplit=int(rng.choice([0, 1, 2, 100])))
+    run_and_check(w, tuning=tuning)
