@@ -118,13 +118,21 @@ typedef struct {
  * One kvr_reposition_splice call can thus carry the spliced skills (delta per segment), repaired seam tokens
  * (delta = 0) and the fresh suffix (RoPE applied on the way into the cache): K is never materialised twice. */
 #define KVR_SEG_PRE_ROPE 1
+/* KVR_SEG_SRC_STABLE: a promise about ordering, never about results.  The segment's k_src / v_src bytes are not written
+ * by any work enqueued on `cuda_stream` before this call -- the normal state of a PRECOMPILED skill ("we
+ * precompile a long skill", :393 "prefilled once in isolation"), unlike suffix keys a kernel has just produced.  The
+ * kernels are launched with programmatic dependent launch; with this flag a CTA may start READING the segment's
+ * sources while the previous kernel on the stream is still draining (nothing is written, and the block table, position
+ * maps and scales are only read, before that kernel has completed).  Setting it on sources that earlier work on the
+ * stream does write is a data race.  Ignored by kvr_reposition_splice_host. */
+#define KVR_SEG_SRC_STABLE 2
 typedef struct {
   const void* k_src;
   const void* v_src;
   int64_t src_stride_layer, src_stride_head, src_stride_token; /* elements */
   int32_t len, old_start, new_start;
   int32_t dst_seq, dst_token_start;
-  int32_t flags; /* 0 or KVR_SEG_PRE_ROPE (occupies what used to be padding: the struct size is unchanged) */
+  int32_t flags; /* 0 or an OR of KVR_SEG_* (occupies what used to be padding: the struct size is unchanged) */
   const int32_t* pos_map;
   const float* k_scale_src;
 } kvr_segment;

@@ -124,7 +124,7 @@ kvr_status check_call(const kvr_model_desc* m, const kvr_paged_dst* d, const kvr
     for (int64_t x : ss)
       if ((x * E) % 16 != 0) return KVR_ERR_ALIGNMENT;
     if (s.pos_map && (reinterpret_cast<uintptr_t>(s.pos_map) & 3u)) return KVR_ERR_ALIGNMENT;
-    if (s.flags & ~KVR_SEG_PRE_ROPE) return KVR_ERR_INVALID_ARG;
+    if (s.flags & ~(KVR_SEG_PRE_ROPE | KVR_SEG_SRC_STABLE)) return KVR_ERR_INVALID_ARG;
   }
   return KVR_OK;
 }
@@ -418,6 +418,7 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
       o.first_q = s.dst_token_start / cg;
       o.n_chunks = (int32_t)(((int64_t)s.dst_token_start + s.len - 1) / cg - o.first_q + 1);
       o.index = i; o.pre_rope = (s.flags & KVR_SEG_PRE_ROPE) ? 1 : 0;
+      o.src_stable = (!src_group_local && (s.flags & KVR_SEG_SRC_STABLE)) ? 1 : 0; o.pad_ = 0;
       chunks_total += o.n_chunks;
     }
     int lpu = lpu_request;

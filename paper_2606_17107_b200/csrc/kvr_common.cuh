@@ -33,6 +33,8 @@ struct SegDev {
   int32_t n_chunks;            // chunks of <= cg tokens, aligned to cg in destination token space
   int32_t index;               // position in the caller's array (for the status word)
   int32_t pre_rope;            // KVR_SEG_PRE_ROPE: every source token sits at old_start (kvr.h)
+  int32_t src_stable;          // KVR_SEG_SRC_STABLE: nothing earlier on the stream writes the sources (early loads)
+  int32_t pad_;
 };
 
 constexpr int kInlineSegs = 8;    // calls with <= this many segments carry their descriptors in the kernel parameters

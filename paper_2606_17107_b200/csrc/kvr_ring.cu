@@ -78,6 +78,7 @@ static_assert(sizeof(TileMeta) == 32, "TileMeta layout");
 
 constexpr int kFlagDone = 1, kFlagRotate = 2, kFlagTokMajor = 4;   // TokMajor: the stage is laid out [token][head][dim]
 constexpr int kFlagKOnly = 8, kFlagVOnly = 16;                       // split gather tiles: the stage holds K or V alone
+constexpr int kFlagSkip = 32;                                        // early-loaded tile whose block-table entry turned out invalid: release only
 constexpr int kMaxThreads = 32 * 17;
 constexpr int kMaxDevices = 64;
 
@@ -197,9 +198,10 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     for (int s = 0; s < S; ++s) { mbar_init(s_full + 8u * s, 1); mbar_init(s_empty + 8u * s, (uint32_t)RP.wpg); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  __syncthreads();     // the barriers are initialised before the producer warp may use them (early source loads below)
   // Programmatic dependent launch: let the next launch on this stream bring its CTAs up (they take an SM's shared
   // memory as soon as a CTA of this grid exits) and run this prologue while our tail drains; it touches no global
-  // memory until griddepcontrol.wait has seen the previous grid complete and flush.
+  // memory that earlier work on the stream may write until griddepcontrol.wait has seen the previous grid complete.
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   // Before the dependency wait the producer may only touch kernel parameters and the context's own immutable
   // inv_freq copy: with the descriptors inline it already knows the segment of its first (statically assigned)
@@ -211,6 +213,50 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     const int64_t delta = P.inline_segs[pre_si].delta;
     for (int p = lane; p < RP.half_R; p += 32) tab[tab_pos<G::PPV>(p, RP.NV)] = angle_entry(delta, P.inv_freq[p]);
     __syncwarp();
+  }
+  // EARLY SOURCE LOADS (KVR_SEG_SRC_STABLE, kvr.h): a precompiled skill is not written by anything that precedes the call
+  // on the stream, so the loads of the CTA's first (statically assigned) unit are issued NOW, while the previous grid
+  // is still draining, into stages 0.. with their byte counts posted by expect_tx WITHOUT an arrival.  The stages'
+  // destinations need the block table, which is read after the wait: the producer then writes the tile descriptors and
+  // arrives, and only then can a stage's "full" phase complete.  Inline descriptors only (they are kernel parameters).
+  int early_n = 0;
+  if (warp == NW && P.n_segs <= kInlineSegs && !P.inplace && !RP.split && (int64_t)blockIdx.x * P.grab < P.total_units) {
+    const int64_t u0 = (int64_t)blockIdx.x * P.grab;
+    const int si0 = find_segment(P.inline_segs, P.n_segs, u0);
+    const SegDev& s0 = P.inline_segs[si0];
+    if (s0.src_stable && (P.tmajor || s0.st == P.head_dim)) {
+      const int64_t local = u0 - s0.unit_begin;
+      const int lg = (int)(local / s0.n_chunks), c = (int)(local - (int64_t)lg * s0.n_chunks);
+      const Chunk ch = chunk_of(s0, c, RP.cg, P.block_size);
+      const int lgi = lg / P.hsplit, hpart = lg - lgi * P.hsplit;
+      const int l0 = lgi * P.lpu, l1 = min(P.layers, l0 + P.lpu);
+      const int hg_per = (P.heads / RP.hpt) / P.hsplit;
+      const int n_sub = P.tmajor ? (ch.n_tok + RP.ct - 1) / RP.ct : 1;
+      const int n_tiles = P.tmajor ? (l1 - l0) * n_sub : (l1 - l0) * hg_per;
+      early_n = min(S < 32 ? S : 32, n_tiles);
+      if (lane < early_n) {
+        const uint64_t pol = policy_evict_first();
+        const uint32_t bar = s_full + 8u * lane;
+        const uint32_t sk = s_base + RP.off_stage + (uint32_t)lane * RP.stage_bytes;
+        if (P.tmajor) {
+          const int l = l0 + lane / n_sub, tok0 = (lane % n_sub) * RP.ct;
+          mbar_expect_tx(bar, (RP.no_v ? 1u : 2u) * (uint32_t)RP.tile_bytes);
+          tensor_g2s_4d(sk, &TI.m[si0].k, 0, 0, ch.t0 + tok0, l, bar, pol);
+          if (!RP.no_v) tensor_g2s_4d(sk + RP.tile_bytes, &TI.m[si0].v, 0, 0, ch.t0 + tok0, l, bar, pol);
+        } else {
+          const int l = l0 + lane / hg_per, h0 = (hpart * hg_per + lane % hg_per) * RP.hpt;
+          const uint32_t run_bytes = (uint32_t)(ch.n_tok * RP.rowB);
+          mbar_expect_tx(bar, (RP.no_v ? 1u : 2u) * RP.hpt * run_bytes);
+          for (int hh = 0; hh < RP.hpt; ++hh) {
+            const int64_t src_off = ((int64_t)l * s0.sl + (int64_t)(h0 + hh) * s0.sh + (int64_t)ch.t0 * s0.st) * E;
+            const uint32_t so = (uint32_t)(hh * RP.cg * RP.rowB);
+            bulk_g2s(sk + so, s0.k_src + src_off, run_bytes, bar, pol);
+            if (!RP.no_v) bulk_g2s(sk + RP.tile_bytes + so, s0.v_src + src_off, run_bytes, bar, pol);
+          }
+        }
+      }
+      __syncwarp();
+    }
   }
   asm volatile("griddepcontrol.wait;" ::: "memory");
   if (DTYPE == 1)
@@ -295,6 +341,20 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
         }
         if (blk < 0 || blk >= P.num_blocks) {
           if (lane == 0) report_bad_block(P.status, sg.index, t0);
+          if (early_n > 0 && i == 0u && base == (int64_t)blockIdx.x * G && j == 0) {
+            // the unit's first tiles were loaded before the dependency wait: hand their stages to the consumers as
+            // SKIP tiles (released without touching the destination) so that the ring keeps turning
+            if (lane < early_n) {
+              TileMeta m{};
+              m.flags = kFlagSkip;
+              meta[lane] = m;
+              mbar_arrive(s_full + 8u * lane);
+            }
+            __syncwarp();
+            i += (uint32_t)early_n; stage += early_n;
+            if (stage >= S) { stage -= S; phase ^= 1u; }
+            early_n = 0;
+          }
           continue;
         }
         // ---- angle table (step a1) ----
@@ -385,8 +445,11 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
           const int64_t dst_chunk = (int64_t)blk * P.d_sb + (int64_t)off * P.d_st;
           const int64_t src_chunk = (int64_t)t0 * sg.st;
           const int pass = S < 32 ? S : 32;
+          // the first pass of the CTA's first unit: its loads were issued before the dependency wait (early_n tiles)
+          const bool early_unit = early_n > 0 && i == 0u && base == (int64_t)blockIdx.x * G && j == 0;
           for (int tb0 = 0; tb0 < n_tiles; tb0 += pass) {
             const int n = min(pass, n_tiles - tb0);
+            const bool early = early_unit && tb0 == 0;      // then n == early_n: descriptor + arrival only
             if (lane < n && tmajor) {
               // transposing tensor loads: the box {head_dim, heads, ct tokens, 1 layer} of the source lands as
               // [token][head][dim], the order of a dense token-major pool; one TMA operation per tensor and tile
@@ -403,11 +466,15 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
               m.flags = flags | (tok0 << 8);                                   // bits 8+: first token of the tile in its chunk
               m.scale_idx = l * P.heads; m.seg = si;
               meta[my_stage] = m;
+              if (early) {
+                mbar_arrive(bar);
+              } else {
               mbar_arrive_expect_tx(bar, (RP.no_v ? 1u : 2u) * (uint32_t)RP.tile_bytes);   // the whole box, zero-filled past the end
               const uint32_t sk = s_base + RP.off_stage + (uint32_t)my_stage * RP.stage_bytes;
               const TmapPair* tp = (P.n_segs <= kInlineSegs) ? &TI.m[si] : &P.tmaps[si];
               tensor_g2s_4d(sk, &tp->k, 0, 0, t0 + tok0, l, bar, pol);
               if (!RP.no_v) tensor_g2s_4d(sk + RP.tile_bytes, &tp->v, 0, 0, t0 + tok0, l, bar, pol);
+              }
             } else if (lane < n) {
               const int t = (tb0 + lane) / kinds;
               const int kind = RP.split ? (tb0 + lane) - t * kinds : -1;      // 0: K tile, 1: V tile, -1: both
@@ -423,6 +490,9 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
               m.flags = flags | (kind == 0 ? kFlagKOnly : 0) | (kind == 1 ? kFlagVOnly : 0);
               m.scale_idx = l * P.heads + h0; m.seg = si;
               meta[my_stage] = m;
+              if (early) {
+                mbar_arrive(bar);
+              } else {
               mbar_arrive_expect_tx(bar, ((RP.no_v || RP.split) ? 1u : 2u) * RP.hpt * run_bytes);
               const uint32_t sk = s_base + RP.off_stage + (uint32_t)my_stage * RP.stage_bytes;
               const uint32_t sv = RP.split ? sk : sk + RP.tile_bytes;
@@ -455,8 +525,10 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
                   }
                 }
               }
+              }
             }
             __syncwarp();
+            if (early) early_n = 0;
             i += (uint32_t)n;
             stage += n;
             if (stage >= S) { stage -= S; phase ^= 1u; }
@@ -586,6 +658,13 @@ kvr_ring_kernel(const __grid_constant__ CallParams P, const __grid_constant__ Ri
     mbar_wait(s_full + 8u * stage, phase, 4);
     const TileMeta m = meta[stage];
     if (m.flags & kFlagDone) break;
+    if (m.flags & kFlagSkip) {       // an early-loaded tile whose destination block is invalid: release the stage, nothing else
+      __syncwarp();
+      if (lane == 0) mbar_arrive(s_empty + 8u * stage);
+      stage += stage_step;
+      if (stage >= S) { stage -= S; phase ^= 1u; }
+      continue;
+    }
     const uint32_t sk = s_base + RP.off_stage + (uint32_t)stage * RP.stage_bytes;
     const uint32_t sv = RP.split ? sk : sk + RP.tile_bytes;
     const int n_tok = m.n_tok;

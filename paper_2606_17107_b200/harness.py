@@ -17,6 +17,11 @@ def model_of(w):
                           _DTYPE[w.dtype], w.inv_freq, rotary_offset=getattr(w, "rotary_offset", 0))
 
 
+def _seg_flags(s):
+    return ((kvr.KVR_SEG_PRE_ROPE if getattr(s, "pre_rope", False) else 0) |
+            (kvr.KVR_SEG_SRC_STABLE if getattr(s, "src_stable", False) else 0))
+
+
 GUARD_BYTE = 0xA5
 
 
@@ -56,7 +61,7 @@ class DeviceWorkload:
         self.segs = kvr.segment_array([
             kvr.segment(k, v, w.src_strides(s), s.len, s.old_start, s.new_start, s.dst_seq, s.dst_token_start,
                         pos_map=pm, k_scale_src=self.k_scale_src,
-                        flags=kvr.KVR_SEG_PRE_ROPE if getattr(s, "pre_rope", False) else 0)
+                        flags=_seg_flags(s))
             for s, (k, v), pm in zip(w.segments, self.sources, self.pos_maps)])
         self.dst = self.dst_for(self.k_cache, self.v_cache) if make_pool else None
 
@@ -131,7 +136,7 @@ class DeviceWorkload:
         self.host_segs = kvr.segment_array([
             kvr.segment(k, v, w.src_strides(s), s.len, s.old_start, s.new_start, s.dst_seq, s.dst_token_start,
                         pos_map=pm, k_scale_src=self.host_k_scale_src,
-                        flags=kvr.KVR_SEG_PRE_ROPE if getattr(s, "pre_rope", False) else 0)
+                        flags=_seg_flags(s))
             for s, (k, v), pm in zip(w.segments, self.host_sources, self.host_pos_maps)])
         return self.host_segs
 

@@ -15,7 +15,7 @@ KVR_OK, KVR_ERR_INVALID_ARG, KVR_ERR_UNSUPPORTED, KVR_ERR_ALIGNMENT = 0, -1, -2,
 KVR_ERR_OUT_OF_RANGE, KVR_ERR_CUDA, KVR_ERR_NOMEM = -4, -5, -6
 KVR_BF16, KVR_FP8_E4M3 = 0, 1
 KVR_PAIR_NEOX_HALF, KVR_PAIR_GPTJ_INTERLEAVED = 0, 1
-KVR_SEG_PRE_ROPE = 1
+KVR_SEG_PRE_ROPE, KVR_SEG_SRC_STABLE = 1, 2
 PATH_AUTO, PATH_GENERIC, PATH_RING, PATH_ATTEND = 0, 1, 2, 3
 
 

@@ -53,6 +53,6 @@ def test_traffic_table_is_keyed_by_workload_and_layout():
     assert bench.NCU_TRAFFIC_BYTES, "profiles/traffic.txt is missing or empty"
     for key in bench.NCU_TRAFFIC_BYTES:
         parts = key.split(":")
-        assert len(parts) in (2, 3) and parts[1] in ("NHD", "HND"), key
+        assert len(parts) in (2, 3) and parts[1] in ("NHD", "HND", "src"), key   # "src": rotate-on-read attention reads the sources in place (no pool layout)
     assert bench.traffic_of("cfg1-qwen3-8b", "NHD", "splice") is not None
     assert bench.traffic_of("no-such-workload", "NHD", "splice") is None

@@ -77,7 +77,8 @@ def test_validation(kvr):
     assert _call(kvr, v_src=None)[0] == kvr.KVR_ERR_INVALID_ARG
     # NEXT-4: segment flags (the field sits in former padding: the struct size asserted above is unchanged)
     assert _call(kvr, flags=kvr.KVR_SEG_PRE_ROPE)[0] == kvr.KVR_OK
-    assert _call(kvr, flags=2)[0] == kvr.KVR_ERR_INVALID_ARG
+    assert _call(kvr, flags=kvr.KVR_SEG_SRC_STABLE | kvr.KVR_SEG_PRE_ROPE)[0] == kvr.KVR_OK
+    assert _call(kvr, flags=4)[0] == kvr.KVR_ERR_INVALID_ARG
 
 
 def test_bytes_moved_is_linear(kvr):

@@ -90,6 +90,7 @@ class SegmentSpec:
     pos_map: Optional[np.ndarray] = None   # int32 [len]: new position of token t
     src_row_pad: int = 0                   # extra elements after each source token row (stride tests)
     pre_rope: bool = False                 # keys not yet position-encoded (fresh suffix keys): all tokens at old_start
+    src_stable: bool = True                # a precompiled skill: nothing earlier on the stream writes its K / V (kvr.h)
 
 
 @dataclass
@@ -231,7 +232,8 @@ def make_workload(*, name, layers, kv_heads, head_dim, rotary_dim=None, pairing=
             segs.append(SegmentSpec(len=d["len"], old_start=d.get("old_start", 0),
                                     new_start=d.get("new_start", d["dst_token_start"]), dst_seq=q,
                                     dst_token_start=d["dst_token_start"], pos_map=d.get("pos_map"),
-                                    src_row_pad=d.get("src_row_pad", 0), pre_rope=d.get("pre_rope", False)))
+                                    src_row_pad=d.get("src_row_pad", 0), pre_rope=d.get("pre_rope", False),
+                                    src_stable=d.get("src_stable", not d.get("pre_rope", False))))
     if num_blocks is None:
         num_blocks = int(np.ceil(slack * sum(rows)))
     table = _table_rows(num_blocks, rows, seed + 3000, prefix)
