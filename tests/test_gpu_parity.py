@@ -616,3 +616,57 @@ def test_transposing_loads_shapes(heads, D, dtype, pairing, R):
                       seq_segments=[[dict(len=61, dst_token_start=3, new_start=1234), dict(len=1, dst_token_start=70)],
                                     [dict(len=24, dst_token_start=8, new_start=0)]])
     check_parity(w, "ring", transpose_load=1)
+
+
+@pytest.mark.parametrize("max_ctas", [0, 1, 3])
+@pytest.mark.parametrize("layout", ["NHD", "HND"])
+def test_early_source_loads_release_skip_tiles_on_a_bad_first_block(layout, max_ctas):
+    """KVR_SEG_SRC_STABLE (kvr.h): the loads of a CTA's first unit are issued before the dependency wait, the block
+    table is read after it.  If that unit's block-table entry is invalid, the early stages must be released as SKIP
+    tiles (nothing written, ring keeps turning) and the sticky status raised -- in both the tensor-load (NHD) and the
+    bulk-copy (HND) form, with one CTA doing all the work and with many."""
+    w = make_workload(name="bad0", layers=3, kv_heads=4, head_dim=128, theta=1e4, block_size=16, layout=layout, seed=5,
+                      seq_segments=[[dict(len=100, dst_token_start=0, new_start=7)],
+                                    [dict(len=40, dst_token_start=16, new_start=900)]])
+    assert all(s.src_stable for s in w.segments)
+    good = w.block_table.copy()
+    w.block_table[0, 0] = -1                       # the first chunk of segment 0: unit 0 of CTA 0
+    srcs, kc, vc = materialize_cpu(w)
+    gk, gv, status, info = _gpu(w, srcs, dict(path=PATHS["ring"], max_ctas=max_ctas))
+    assert status[0] == -4 and status[1] == 0 and status[2] == 0
+    w.block_table[:] = good
+    run_oracle(w, srcs, kc, vc)
+    s_l, s_b, s_t, s_h = w.dst_strides()
+    skipped = np.zeros(kc.shape, dtype=bool)
+    for l in range(w.layers):
+        o = l * s_l + int(good[0, 0]) * s_b
+        skipped[o:o + s_b] = True
+    assert np.array_equal(gv[~skipped], vc[~skipped])
+    assert np.all(gk[skipped] == SENTINEL_BF16) and np.all(gv[skipped] == SENTINEL_BF16)
+    assert k_distance(w, gk[~skipped], kc[~skipped]).max() <= 2
+
+
+@pytest.mark.parametrize("c,layout", [(1, "NHD"), (1, "HND"), (3, "NHD"), (4, "NHD"), (4, "HND")])
+def test_src_stable_flag_changes_nothing_but_the_launch_order(c, layout):
+    """The same call with and without KVR_SEG_SRC_STABLE, issued back to back on one stream (programmatic dependent
+    launch: each launch's prologue and early loads overlap the tail of the one before): identical pool bytes."""
+    from paper_2606_17107_b200 import kvr
+    from paper_2606_17107_b200.harness import DeviceWorkload
+    w = config_small(c, layout)
+    srcs, _, _ = materialize_cpu(w)
+    tsrc = [(torch_bits(k), None if v is None else torch_bits(v)) for k, v in srcs]
+    pools = []
+    for stable in (True, False, True):
+        for s in w.segments:
+            s.src_stable = stable
+        dw = DeviceWorkload(w, "cuda:0", sources=tsrc)
+        pools.append(dw)
+    stream = torch.cuda.Stream()
+    with kvr.Context(pools[0].model) as ctx:
+        for _ in range(3):
+            for dw in pools:
+                dw.run(ctx, stream=stream)
+        torch.cuda.synchronize()
+        assert ctx.last_device_status()[0] == kvr.KVR_OK
+    for dw in pools[1:]:
+        assert torch.equal(dw.k_cache, pools[0].k_cache) and torch.equal(dw.v_cache, pools[0].v_cache)
