@@ -275,7 +275,7 @@ typedef struct {
   int32_t len;
   int32_t delta;   /* new_start - old_start: where the skill sits in this request's context minus where it was compiled */
   int32_t request; /* row of q / o / lse that attends this segment */
-  int32_t reserved_; /* must be 0 */
+  int32_t flags;   /* 0 or KVR_SEG_SRC_STABLE (as in kvr_segment: the K / V loads may then overlap the previous kernel's tail) */
 } kvr_read_segment;
 
 KVR_API kvr_status kvr_rotate_on_read_attention(kvr_ctx* ctx, const void* q, int32_t n_req, int32_t q_heads, int32_t layer,

@@ -666,7 +666,7 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
   std::vector<int32_t> per_req((size_t)n_req, 0);
   for (int32_t i = 0; i < n; ++i) {
     const kvr_read_segment& s = segs[i];
-    if (!s.k_src || !s.v_src || s.len <= 0 || s.request < 0 || s.request >= n_req || s.reserved_ != 0) return KVR_ERR_INVALID_ARG;
+    if (!s.k_src || !s.v_src || s.len <= 0 || s.request < 0 || s.request >= n_req || (s.flags & ~KVR_SEG_SRC_STABLE)) return KVR_ERR_INVALID_ARG;
     if ((s.src_stride_token < m.head_dim && s.len > 1) || s.src_stride_layer < 0 || s.src_stride_head < 0) return KVR_ERR_INVALID_ARG;
     if ((s.src_stride_head < m.head_dim && m.kv_heads > 1)) return KVR_ERR_INVALID_ARG;
     if (!aligned16(s.k_src) || !aligned16(s.v_src)) return KVR_ERR_ALIGNMENT;
@@ -805,6 +805,8 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
   P.merges = reinterpret_cast<const AttnMerge*>(slot.dev + seg_bytes + n_items * sizeof(AttnItem));
   P.n_merges = (int32_t)slot.n_merges;
   P.merge_max_count = slot.merge_max;
+  P.early = 1;
+  for (int32_t i = 0; i < n; ++i) if (!(segs[i].flags & KVR_SEG_SRC_STABLE)) P.early = 0;
   P.q_heads = q_heads; P.group = group; P.layer = layer;
   P.rotary_dim = m.rotary_dim; P.rotary_offset = m.rotary_offset; P.pairing = m.pairing;
   P.scale_log2 = (float)((double)softmax_scale * 1.4426950408889634);

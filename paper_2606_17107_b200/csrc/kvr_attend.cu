@@ -35,7 +35,8 @@
 //               item (device-scope fence + ticket); a group of many is left to kvr_attend_merge_kernel after the
 //               grid, because under a saturated HBM every dependent load of an in-kernel merge costs microseconds
 //               (measured: a 512-partial in-kernel merge was a 600 us serial tail).
-// Programmatic dependent launch: the prologue (barriers, TMEM allocation) overlaps the tail of the previous launch.
+// Programmatic dependent launch: the prologue (barriers, TMEM allocation) and -- for precompiled skills
+// (KVR_SEG_SRC_STABLE) -- the K / V loads of the first item overlap the tail of the previous launch.
 #include <mutex>
 
 #include "kvr_attend.cuh"
@@ -208,9 +209,14 @@ __global__ void __launch_bounds__(kThreads, 1) kvr_attend_kernel(const __grid_co
   // on the stream (its partial buffers, tickets and outputs are reused by this one) must have completed before any
   // global memory is touched.
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  asm volatile("griddepcontrol.wait;" ::: "memory");
   __syncthreads();
   tc_fence_after();
+  // griddepcontrol.wait is executed per role, by the threads that touch global memory an earlier kernel may write: the
+  // scheduler / query warp (the query, the item counter) and the epilogue warps (outputs, partials, tickets).  The
+  // work items and tensor maps were staged before this kernel could start.  With P.early (every segment carries
+  // KVR_SEG_SRC_STABLE: precompiled skills) the TMA producers do NOT wait: the K / V tiles of the CTA's first item
+  // stream in while the previous kernel on the stream drains; otherwise they wait as well.
+  auto dependency_wait = [] { asm volatile("griddepcontrol.wait;" ::: "memory"); };
   const uint32_t tmem = *tmem_slot;
   const uint32_t tm_s0 = tmem, tm_o0 = tmem + 32u;
 
@@ -228,6 +234,7 @@ __global__ void __launch_bounds__(kThreads, 1) kvr_attend_kernel(const __grid_co
   if (warp == 0 || warp == 2) {
     // =========================================================================== TMA PRODUCERS (warp 0: K, warp 2: V)
     if (lane == 0) {
+      if (!P.early) dependency_wait();
       const bool is_k = warp == 0;
       const int NS = is_k ? kKS : kVS;
       const int b_full = is_k ? B_KFULL : B_VFULL, b_empty = is_k ? B_KEMPTY : B_VEMPTY;
@@ -327,12 +334,14 @@ __global__ void __launch_bounds__(kThreads, 1) kvr_attend_kernel(const __grid_co
     int64_t idx = blockIdx.x;
     uint32_t n_pub = 0;
     // lane 0: fetch the next item (or the end marker), publish it, request the draw after it
-    auto publish_next = [&]() -> AttnItem {
+    auto publish_next = [&](bool first) -> AttnItem {
       AttnItem it{};
       it.seg = -1;
       if (idx < P.n_items) it = P.items[idx];
-      idx = (int64_t)gridDim.x + (int64_t)nxt;
-      if (it.seg >= 0 && idx < P.n_items) nxt = atomicAdd(P.sched, 1ull);
+      if (!first) {
+        idx = (int64_t)gridDim.x + (int64_t)nxt;
+        if (it.seg >= 0 && idx < P.n_items) nxt = atomicAdd(P.sched, 1ull);
+      }
       const int slot = n_pub % kIR;
       if (n_pub >= (uint32_t)kIR) mbar_wait(bar(B_IEMPTY + slot), ((n_pub / kIR) - 1u) & 1u, 30);
       ring_w[slot] = it;
@@ -342,10 +351,18 @@ __global__ void __launch_bounds__(kThreads, 1) kvr_attend_kernel(const __grid_co
     };
     AttnItem nx{};
     nx.seg = -1;
-    if (lane == 0) { nxt = atomicAdd(P.sched, 1ull); nx = publish_next(); }
+    // the first item is static (items[blockIdx.x]) and is published BEFORE the dependency wait, so that the producers
+    // can start on it; the item counter (re-armed by the previous launch's last CTA) is only touched after the wait
+    if (lane == 0) nx = publish_next(true);
+    dependency_wait();
+    if (lane == 0) {
+      nxt = atomicAdd(P.sched, 1ull);
+      idx = (int64_t)gridDim.x + (int64_t)nxt;
+      if (idx < P.n_items) nxt = atomicAdd(P.sched, 1ull);
+    }
     for (uint32_t ic = 0;; ++ic) {
       AttnItem it = nx;                    // the item whose Q' is built now; the one after it is published first, so
-      if (lane == 0 && it.seg >= 0) nx = publish_next();   // that the producers can run an item ahead of the query
+      if (lane == 0 && it.seg >= 0) nx = publish_next(false);   // that the producers can run an item ahead of the query
       it.seg = __shfl_sync(0xFFFFFFFFu, it.seg, 0);
       if (it.seg < 0) break;
       it.head = __shfl_sync(0xFFFFFFFFu, it.head, 0);
@@ -499,6 +516,7 @@ __global__ void __launch_bounds__(kThreads, 1) kvr_attend_kernel(const __grid_co
     const int w4 = warp - 8;
     const uint32_t lane_base = (uint32_t)(w4 * 32) << 16;
     const float* const stat = reinterpret_cast<const float*>(smem + kOffStat);
+    dependency_wait();
     for (uint32_t ic = 0;; ++ic) {
       const AttnItem it = take_item(ic, 50);
       if (it.seg < 0) break;

@@ -34,6 +34,7 @@ struct AttnParams {
   const AttnMerge* merges;
   int32_t n_items, n_merges;
   int32_t merge_max_count; // largest group among `merges`
+  int32_t early;           // every segment carries KVR_SEG_SRC_STABLE: the TMA producers need not wait for the previous kernel
   int32_t q_heads, group;  // group = q_heads / kv_heads
   int32_t layer, rotary_dim, rotary_offset, pairing;
   float scale_log2;        // softmax_scale * log2(e)

@@ -170,7 +170,8 @@ class DeviceReadWorkload:
         self.q = self._dev(queries, "q")
         self.o = self._dev(torch.full((w.n_req, w.q_heads, w.head_dim), float("nan"), dtype=torch.float32), "o")
         self.lse = self._dev(torch.full((w.n_req, w.q_heads), float("nan"), dtype=torch.float32), "lse")
-        self.segs = kvr.read_segment_array([kvr.read_segment(k, v, w.src_strides(s), s.len, s.delta, s.request)
+        self.segs = kvr.read_segment_array([kvr.read_segment(k, v, w.src_strides(s), s.len, s.delta, s.request,
+                                                             flags=kvr.KVR_SEG_SRC_STABLE if getattr(s, "src_stable", True) else 0)
                                             for s, (k, v) in zip(w.segments, self.sources)])
 
     _dev = DeviceWorkload._dev

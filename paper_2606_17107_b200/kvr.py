@@ -67,7 +67,7 @@ class kvr_span(C.Structure):
 class kvr_read_segment(C.Structure):
     _fields_ = [("k_src", C.c_void_p), ("v_src", C.c_void_p),
                 ("src_stride_layer", C.c_int64), ("src_stride_head", C.c_int64), ("src_stride_token", C.c_int64),
-                ("len", C.c_int32), ("delta", C.c_int32), ("request", C.c_int32), ("reserved_", C.c_int32)]
+                ("len", C.c_int32), ("delta", C.c_int32), ("request", C.c_int32), ("flags", C.c_int32)]
 
 
 EXPORTS = ["kvr_rotate_on_read_attention", "kvr_attention_bytes_read", "kvr_reposition_inplace", "kvr_inplace_bytes_moved", "kvr_write_span",
@@ -184,9 +184,9 @@ def span_array(spans):
     return (kvr_span * len(spans))(*spans)
 
 
-def read_segment(k_src, v_src, src_strides, len, delta, request):
+def read_segment(k_src, v_src, src_strides, len, delta, request, flags=0):
     sl, sh, st = src_strides
-    return kvr_read_segment(_ptr(k_src), _ptr(v_src), sl, sh, st, len, delta, request, 0)
+    return kvr_read_segment(_ptr(k_src), _ptr(v_src), sl, sh, st, len, delta, request, flags)
 
 
 def read_segment_array(segs):

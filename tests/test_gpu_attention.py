@@ -236,6 +236,8 @@ def test_argument_errors_and_limits():
         k, v = dw.sources[0]
         bad = [kvr.read_segment(k, v, w.src_strides(w.segments[0]), 130, 5, 5)]
         assert call(segs=bad) == kvr.KVR_ERR_INVALID_ARG                # request out of range
+        bad = [kvr.read_segment(k, v, w.src_strides(w.segments[0]), 130, 5, 0, flags=4), dw.segs[1]]
+        assert call(segs=bad) == kvr.KVR_ERR_INVALID_ARG                # unknown flag
         g = torch.cuda.CUDAGraph()
         s = torch.cuda.Stream()
         with torch.cuda.stream(s):
@@ -305,6 +307,8 @@ def test_fuzz_shapes_and_decompositions(case):
     w.layer = int(rng.integers(0, w.layers))
     perm = rng.permutation(len(w.segments))
     w.segments = [w.segments[i] for i in perm]
+    if rng.random() < 0.5:                       # a segment that is not flagged stable: no early loads for the call
+        w.segments[0].src_stable = False
     tuning = dict(layers_per_unit=int(rng.choice([0, 1, 2, 3, 5])), max_ctas=int(rng.choice([0, 0, 1, 3, 17])),
                   hsplit=int(rng.choice([0, 1, 2, 100])))
     run_and_check(w, tuning=tuning)

@@ -22,6 +22,7 @@ class ReadSegmentSpec:
     delta: int           # new_start - old_start of the skill in this request's context
     request: int
     src_row_pad: int = 0
+    src_stable: bool = True   # a precompiled skill: nothing earlier on the stream writes its K / V (kvr.h)
 
 
 @dataclass
