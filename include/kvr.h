@@ -263,7 +263,10 @@ KVR_API kvr_status kvr_write_span(kvr_ctx* ctx, const kvr_paged_dst* dst, const 
  * 16-byte aligned).  Asynchronous on `cuda_stream`; descriptors (TMA tensor maps, work items) are built on the host,
  * staged through context-owned pinned memory and CACHED per distinct segment array (8 entries, least recently used
  * replaced): a decode loop that reads the same skills at every step and layer enqueues nothing but its kernels from
- * the second call on.  Not capturable in a CUDA graph (KVR_ERR_UNSUPPORTED under capture).  One or two kernels per
+ * the second call on.  CUDA graphs: a call whose descriptors are cached (it has been issued once eagerly with the same
+ * segment array and its buffers have not grown since) enqueues nothing but kernels and may be captured and replayed
+ * with other q / o / lse / layer arguments per node; its cache entry is then pinned until kvr_destroy.  Any other call
+ * is refused under capture with KVR_ERR_UNSUPPORTED before anything is enqueued.  One or two kernels per
  * call (the second merges the partial results of (request, kv head) groups that were split over many CTAs).  Reads
  * 2 * kv_heads * head_dim * 2 bytes per token (kvr_attention_bytes_read): K and V of one layer, once.  Outputs are
  * written only by this call's kernels; partial results live in context-owned device memory, so calls on one context

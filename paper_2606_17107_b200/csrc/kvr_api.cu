@@ -174,6 +174,7 @@ struct kvr_ctx {
     unsigned char* host = nullptr; unsigned char* dev = nullptr; size_t cap = 0; cudaEvent_t ev = nullptr; bool pending = false;
     std::vector<unsigned char> key; int32_t n_req = 0, q_heads = 0, tpi_tuning = 0, n_groups = 0;
     size_t n_items = 0, seg_bytes = 0, n_merges = 0; int32_t merge_max = 0; uint64_t last_use = 0;
+    bool pinned = false;          // captured in a CUDA graph: never evicted
   };
   static constexpr int kAttnSlots = 8;
   AttnSlot attn_slots[kAttnSlots];
@@ -182,6 +183,7 @@ struct kvr_ctx {
   size_t attn_part_cap = 0;           // bytes
   unsigned int* attn_tickets = nullptr;
   size_t attn_ticket_cap = 0;         // entries
+  std::vector<void*> attn_retired;    // outgrown buffers a captured graph may still point at
 
   kvr_status cuda_fail(cudaError_t e, const char* what) {
     last_err = std::string(what) + ": " + cudaGetErrorString(e);
@@ -297,6 +299,7 @@ kvr_status kvr_destroy(kvr_ctx* c) {
   }
   if (c->attn_part) cudaFree(c->attn_part);
   if (c->attn_tickets) cudaFree(c->attn_tickets);
+  for (void* p : c->attn_retired) cudaFree(p);
   if (c->aux_dev) cudaFree(c->aux_dev);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->d_inv_freq) cudaFree(c->d_inv_freq);
@@ -680,10 +683,7 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
   KVR_CUDA(c, cudaStreamIsCapturing(stream, &cap));
-  if (cap != cudaStreamCaptureStatusNone) {
-    c->last_err = "rotate-on-read attention stages its descriptors through pinned memory and cannot be captured";
-    return KVR_ERR_UNSUPPORTED;
-  }
+  const bool capturing = cap != cudaStreamCaptureStatusNone;
 
   // ---- descriptors: cached per distinct segment array ----
   const size_t key_bytes = (size_t)n * sizeof(kvr_read_segment);
@@ -693,8 +693,16 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
         std::memcmp(a.key.data(), segs, key_bytes) == 0) { slot_p = &a; break; }
   const bool hit = slot_p != nullptr;
   if (!hit) {
-    slot_p = &c->attn_slots[0];
-    for (auto& a : c->attn_slots) if (a.last_use < slot_p->last_use) slot_p = &a;     // least recently used
+    // CUDA graphs: a call whose descriptors are cached enqueues nothing but kernels and may be captured; its cache
+    // entry is then PINNED (never evicted: every replay reads it).  A call that would have to build and copy its
+    // descriptors is refused under capture -- issue it once eagerly first.
+    if (capturing) {
+      c->last_err = "rotate-on-read attention: descriptors of this segment array are not cached yet; issue the call once outside the capture";
+      return KVR_ERR_UNSUPPORTED;
+    }
+    for (auto& a : c->attn_slots)
+      if (!a.pinned && (!slot_p || a.last_use < slot_p->last_use)) slot_p = &a;      // least recently used, not pinned
+    if (!slot_p) { c->last_err = "rotate-on-read attention: every descriptor cache entry is pinned by a captured graph"; return KVR_ERR_NOMEM; }
   }
   kvr_ctx::AttnSlot& slot = *slot_p;
   slot.last_use = ++c->attn_clock;
@@ -779,7 +787,14 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
   // partial results and tickets (grown on demand; a regrowth waits for the launches that may still use the old buffers)
   const size_t part_bytes = n_items * (size_t)group * (128 + 2) * sizeof(float);
   if (part_bytes > c->attn_part_cap || (size_t)n_groups > c->attn_ticket_cap) {
+    if (capturing) { c->last_err = "rotate-on-read attention: partial buffers must grow; issue the call once outside the capture"; return KVR_ERR_UNSUPPORTED; }
     KVR_CUDA(c, cudaDeviceSynchronize());
+    bool any_pinned = false;
+    for (auto& a : c->attn_slots) any_pinned |= a.pinned;
+    if (any_pinned) {           // a captured graph still points at the old buffers: keep them until kvr_destroy
+      if (part_bytes > c->attn_part_cap && c->attn_part) { c->attn_retired.push_back(c->attn_part); c->attn_part = nullptr; }
+      if ((size_t)n_groups > c->attn_ticket_cap && c->attn_tickets) { c->attn_retired.push_back(c->attn_tickets); c->attn_tickets = nullptr; }
+    }
     if (part_bytes > c->attn_part_cap) {
       if (c->attn_part) cudaFree(c->attn_part);
       c->attn_part = nullptr; c->attn_part_cap = 0;
@@ -789,6 +804,7 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
     }
     if ((size_t)n_groups > c->attn_ticket_cap) {
       if (c->attn_tickets) cudaFree(c->attn_tickets);
+  for (void* p : c->attn_retired) cudaFree(p);
       c->attn_tickets = nullptr; c->attn_ticket_cap = 0;
       size_t cap = std::max<size_t>((size_t)n_groups * 2, 1024);
       KVR_CUDA(c, cudaMalloc(&c->attn_tickets, cap * sizeof(unsigned int)));
@@ -821,8 +837,12 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
   c->launches += 1 + (slot.n_merges ? 1 : 0);
   c->last_path = 3;
   c->last_stream = stream;
-  KVR_CUDA(c, cudaEventRecord(slot.ev, stream));
-  slot.pending = true;
+  if (capturing) {
+    slot.pinned = true;
+  } else if (!slot.pinned) {
+    KVR_CUDA(c, cudaEventRecord(slot.ev, stream));      // the entry may be replaced once this launch has run
+    slot.pending = true;
+  }
   return KVR_OK;
 }
 

@@ -240,11 +240,13 @@ def test_argument_errors_and_limits():
         assert call(segs=bad) == kvr.KVR_ERR_INVALID_ARG                # unknown flag
         g = torch.cuda.CUDAGraph()
         s = torch.cuda.Stream()
+        fresh = kvr.read_segment_array([kvr.read_segment(k, v, w.src_strides(w.segments[0]), 129, 5, 0),
+                                        kvr.read_segment(k, v, w.src_strides(w.segments[0]), 60, 6, 1)])
         with torch.cuda.stream(s):
             g.capture_begin()
-            st = ctx.rotate_on_read_attention(dw.q, 2, 8, 1, w.scale, dw.segs, dw.o, dw.lse, stream=s, check=False)
+            st = ctx.rotate_on_read_attention(dw.q, 2, 8, 1, w.scale, fresh, dw.o, dw.lse, stream=s, check=False)
             g.capture_end()
-        assert st == kvr.KVR_ERR_UNSUPPORTED
+        assert st == kvr.KVR_ERR_UNSUPPORTED                            # descriptors not cached yet: refused under capture
         torch.cuda.synchronize()
     w64 = read_workload("d64", q_heads=4, kv_heads=2, head_dim=64, requests=[[(64, 1)]], seed=2)
     d64 = DeviceReadWorkload(w64, "cuda:0")
@@ -312,3 +314,43 @@ def test_fuzz_shapes_and_decompositions(case):
     tuning = dict(layers_per_unit=int(rng.choice([0, 1, 2, 3, 5])), max_ctas=int(rng.choice([0, 0, 1, 3, 17])),
                   hsplit=int(rng.choice([0, 1, 2, 100])))
     run_and_check(w, tuning=tuning)
+
+
+def test_cuda_graph_of_cached_calls_replays_after_cache_churn():
+    """A decode step as a CUDA graph: the attention calls of three layers (descriptors cached by one eager call each)
+    captured once, replayed after a dozen other calls have churned the descriptor cache and the query has changed; the
+    pinned cache entries and the partial buffers the graph points at must still be the ones it was captured with."""
+    from paper_2606_17107_b200 import kvr
+    from paper_2606_17107_b200.harness import DeviceReadWorkload
+    w = read_workload("graph", q_heads=8, kv_heads=2, layers=3, requests=[[(700, 11), (300, -4)], [(2500, 3000)]], seed=4711)
+    srcs_t, q_t = make_read_sources(w, "cpu"), make_queries(w, "cpu")
+    dw = DeviceReadWorkload(w, "cuda:0", sources=srcs_t, queries=q_t)
+    outs = [(torch.empty_like(dw.o), torch.empty_like(dw.lse)) for _ in range(3)]
+    others = [DeviceReadWorkload(read_workload(f"o{i}", q_heads=8, kv_heads=2, requests=[[(3000 + 100 * i, i)] * 3], seed=i), "cuda:0")
+              for i in range(12)]
+    stream = torch.cuda.Stream()
+    with kvr.Context(dw.model) as ctx:
+        call = lambda l: ctx.rotate_on_read_attention(dw.q, w.n_req, w.q_heads, l, w.scale, dw.segs, outs[l][0], outs[l][1], stream=stream)
+        call(0)                                                  # eager once: descriptors cached, buffers sized
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(stream):
+            graph.capture_begin()
+            for l in range(3):
+                call(l)
+            graph.capture_end()
+        for od in others:                                        # churn the cache (and grow the partial buffers)
+            od.run(ctx, stream=stream)
+        for o_, l_ in outs:
+            o_.fill_(float("nan")); l_.fill_(float("nan"))
+        with torch.cuda.stream(stream):
+            graph.replay()
+        torch.cuda.synchronize()
+        srcs = [(np_bits(k), np_bits(v)) for k, v in srcs_t]
+        for l in range(3):
+            w.layer = l
+            ref = reference(w, srcs, np_bits(q_t), orc.host_threads())
+            o, lse = outs[l][0].cpu().numpy().astype(np.float64), outs[l][1].cpu().numpy().astype(np.float64)
+            for r, R in enumerate(ref):
+                assert (np.abs(o[r] - R["o_model"]) <= 2.0 ** -7 * R["wabsv"] + 2.0 ** -12 * R["vmax"]).all(), (l, r)
+                assert (np.abs(lse[r] - R["lse_model"]) <= 2.0 ** -8).all(), (l, r)
