@@ -285,6 +285,11 @@ KVR_API kvr_status kvr_rotate_on_read_attention(kvr_ctx* ctx, const void* q, int
                                                 float softmax_scale, const kvr_read_segment* segs, int32_t n_segs,
                                                 float* o, float* lse, void* cuda_stream);
 KVR_API uint64_t kvr_attention_bytes_read(const kvr_model_desc* model, const kvr_read_segment* segs, int32_t n_segs);
+/* Host-only validation of a kvr_rotate_on_read_attention call (no CUDA call is made; usable without a GPU): the status
+ * the call returns before it enqueues anything (pointers are only checked for NULL and alignment). */
+KVR_API kvr_status kvr_validate_read(const kvr_model_desc* model, const void* q, int32_t n_req, int32_t q_heads, int32_t layer,
+                                     float softmax_scale, const kvr_read_segment* segs, int32_t n_segs, const float* o,
+                                     const float* lse);
 
 /* Algorithmic bytes of a call: read K, read V, write K, write V = 4 * layers*kv_heads*head_dim*esz * sum(len)
  * (2 * ... for a K-only call, i.e. when segs[0].v_src == NULL).

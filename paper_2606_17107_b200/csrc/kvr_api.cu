@@ -652,20 +652,17 @@ uint64_t kvr_attention_bytes_read(const kvr_model_desc* m, const kvr_read_segmen
   return 2ull * (uint64_t)m->kv_heads * (uint64_t)m->head_dim * (uint64_t)elt_bytes(m->dtype) * tokens;
 }
 
-kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req, int32_t q_heads, int32_t layer,
-                                        float softmax_scale, const kvr_read_segment* segs, int32_t n, float* o, float* lse,
-                                        void* cuda_stream) {
-  if (!c) return KVR_ERR_INVALID_ARG;
-  c->last_err.clear();
-  const kvr_model_desc& m = c->model;
+// Host-only validation of a rotate-on-read call (no CUDA call is made): the status the call itself returns before it
+// enqueues anything.
+kvr_status kvr_validate_read(const kvr_model_desc* mp, const void* q, int32_t n_req, int32_t q_heads, int32_t layer,
+                             float softmax_scale, const kvr_read_segment* segs, int32_t n, const float* o, const float* lse) {
+  kvr_status st = check_model(mp);
+  if (st != KVR_OK) return st;
+  const kvr_model_desc& m = *mp;
   if (!q || !o || !lse || !segs || n <= 0 || n_req <= 0 || q_heads <= 0 || layer < 0 || layer >= m.layers) return KVR_ERR_INVALID_ARG;
   if (q_heads % m.kv_heads != 0 || !(softmax_scale > 0.0f) || !std::isfinite(softmax_scale)) return KVR_ERR_INVALID_ARG;
   if (!aligned16(q) || !aligned16(o) || (reinterpret_cast<uintptr_t>(lse) & 3u)) return KVR_ERR_ALIGNMENT;
-  const int group = q_heads / m.kv_heads;
-  if (m.dtype != KVR_BF16 || m.head_dim != 128 || group > 16) {
-    c->last_err = "rotate-on-read attention: bf16 caches, head_dim 128 and q_heads / kv_heads <= 16 only";
-    return KVR_ERR_UNSUPPORTED;
-  }
+  if (m.dtype != KVR_BF16 || m.head_dim != 128 || q_heads / m.kv_heads > 16) return KVR_ERR_UNSUPPORTED;
   std::vector<int32_t> per_req((size_t)n_req, 0);
   for (int32_t i = 0; i < n; ++i) {
     const kvr_read_segment& s = segs[i];
@@ -677,7 +674,22 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
     per_req[(size_t)s.request] += 1;
   }
   for (int32_t r = 0; r < n_req; ++r)
-    if (per_req[(size_t)r] == 0) { c->last_err = "rotate-on-read attention: a request without segments"; return KVR_ERR_INVALID_ARG; }
+    if (per_req[(size_t)r] == 0) return KVR_ERR_INVALID_ARG;      // every request must own at least one segment
+  return KVR_OK;
+}
+
+kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req, int32_t q_heads, int32_t layer,
+                                        float softmax_scale, const kvr_read_segment* segs, int32_t n, float* o, float* lse,
+                                        void* cuda_stream) {
+  if (!c) return KVR_ERR_INVALID_ARG;
+  c->last_err.clear();
+  const kvr_model_desc& m = c->model;
+  const kvr_status vst = kvr_validate_read(&m, q, n_req, q_heads, layer, softmax_scale, segs, n, o, lse);
+  if (vst != KVR_OK) {
+    if (vst == KVR_ERR_UNSUPPORTED) c->last_err = "rotate-on-read attention: bf16 caches, head_dim 128 and q_heads / kv_heads <= 16 only";
+    return vst;
+  }
+  const int group = q_heads / m.kv_heads;
   if (!tmap_encoder()) { c->last_err = "cuTensorMapEncodeTiled is not available"; return KVR_ERR_UNSUPPORTED; }
   DeviceGuard guard(c->device);
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);

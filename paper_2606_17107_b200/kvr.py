@@ -70,7 +70,7 @@ class kvr_read_segment(C.Structure):
                 ("len", C.c_int32), ("delta", C.c_int32), ("request", C.c_int32), ("flags", C.c_int32)]
 
 
-EXPORTS = ["kvr_rotate_on_read_attention", "kvr_attention_bytes_read", "kvr_reposition_inplace", "kvr_inplace_bytes_moved", "kvr_write_span",
+EXPORTS = ["kvr_rotate_on_read_attention", "kvr_attention_bytes_read", "kvr_validate_read", "kvr_reposition_inplace", "kvr_inplace_bytes_moved", "kvr_write_span",
            "kvr_create", "kvr_destroy", "kvr_set_tuning", "kvr_validate", "kvr_reposition_splice",
            "kvr_reposition_splice_host", "kvr_last_h2d_bytes",
            "kvr_bytes_moved", "kvr_last_device_status", "kvr_launch_count", "kvr_last_launch_info",
@@ -104,6 +104,9 @@ def _load():
     lib.kvr_rotate_on_read_attention.restype = C.c_int
     lib.kvr_rotate_on_read_attention.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_float,
                                                  P(kvr_read_segment), C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.kvr_validate_read.restype = C.c_int
+    lib.kvr_validate_read.argtypes = [P(kvr_model_desc), C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_float,
+                                      P(kvr_read_segment), C.c_int32, C.c_void_p, C.c_void_p]
     lib.kvr_attention_bytes_read.restype = C.c_uint64
     lib.kvr_attention_bytes_read.argtypes = [P(kvr_model_desc), P(kvr_read_segment), C.c_int32]
     lib.kvr_last_h2d_bytes.restype = C.c_uint64
@@ -191,6 +194,11 @@ def read_segment(k_src, v_src, src_strides, len, delta, request, flags=0):
 
 def read_segment_array(segs):
     return (kvr_read_segment * len(segs))(*segs)
+
+
+def kvr_validate_read(model, q, n_req, q_heads, layer, softmax_scale, segs, o, lse):
+    arr = segs if not isinstance(segs, (list, tuple)) else read_segment_array(segs)
+    return lib.kvr_validate_read(C.byref(model), _ptr(q), n_req, q_heads, layer, softmax_scale, arr, len(arr), _ptr(o), _ptr(lse))
 
 
 def kvr_attention_bytes_read(model, segs):

@@ -150,3 +150,32 @@ def test_header_is_valid_c99_and_struct_sizes_match_the_binding(kvr, tmp_path):
     sizes = [int(x) for x in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()]
     assert sizes == [C.sizeof(t) for t in (kvr.kvr_model_desc, kvr.kvr_paged_dst, kvr.kvr_segment, kvr.kvr_tuning,
                                            kvr.kvr_resident_span, kvr.kvr_span)]
+
+
+def test_validate_read_without_a_gpu(kvr):
+    """kvr_validate_read: host-only argument checks of kvr_rotate_on_read_attention (kvr.h), no CUDA call."""
+    inv = [1.0] * 64
+    m, keep = kvr.model_desc(4, 8, 128, 128, kvr.KVR_PAIR_NEOX_HALF, kvr.KVR_BF16, inv)
+    A = 0x10000                                     # any 16-byte aligned, non-NULL address: nothing is dereferenced
+    seg = lambda **kw: kvr.read_segment(kw.get("k", A), kw.get("v", A), kw.get("strides", (8 * 100 * 128, 100 * 128, 128)),
+                                        kw.get("len", 100), kw.get("delta", 7), kw.get("request", 0), kw.get("flags", 0))
+    ok = lambda segs, **kw: kvr.kvr_validate_read(kw.get("model", m), kw.get("q", A), kw.get("n_req", 1), kw.get("q_heads", 32),
+                                                  kw.get("layer", 0), kw.get("scale", 0.088), segs, kw.get("o", A), kw.get("lse", A))
+    assert ok([seg()]) == kvr.KVR_OK
+    assert ok([seg(flags=kvr.KVR_SEG_SRC_STABLE), seg(delta=-5)]) == kvr.KVR_OK
+    assert ok([seg()], layer=4) == kvr.KVR_ERR_INVALID_ARG and ok([seg()], layer=-1) == kvr.KVR_ERR_INVALID_ARG
+    assert ok([seg()], q_heads=12) == kvr.KVR_ERR_INVALID_ARG                 # not a multiple of kv_heads
+    assert ok([seg()], scale=0.0) == kvr.KVR_ERR_INVALID_ARG and ok([seg()], scale=float("inf")) == kvr.KVR_ERR_INVALID_ARG
+    assert ok([seg()], q=None) == kvr.KVR_ERR_INVALID_ARG and ok([seg()], o=None) == kvr.KVR_ERR_INVALID_ARG
+    assert ok([seg()], n_req=2) == kvr.KVR_ERR_INVALID_ARG                    # request 1 owns no segment
+    assert ok([seg(request=1)]) == kvr.KVR_ERR_INVALID_ARG
+    assert ok([seg(len=0)]) == kvr.KVR_ERR_INVALID_ARG and ok([seg(flags=1)]) == kvr.KVR_ERR_INVALID_ARG
+    assert ok([seg(strides=(8 * 100 * 128, 100 * 128, 64))]) == kvr.KVR_ERR_INVALID_ARG      # rows overlap
+    assert ok([seg(k=A + 8)]) == kvr.KVR_ERR_ALIGNMENT and ok([seg()], q=A + 2) == kvr.KVR_ERR_ALIGNMENT
+    assert ok([seg(strides=(8 * 100 * 132, 100 * 132, 132))]) == kvr.KVR_ERR_ALIGNMENT        # 264-byte rows
+    assert ok([seg()], q_heads=256) == kvr.KVR_ERR_UNSUPPORTED                # 32 query heads per kv head
+    m64, keep64 = kvr.model_desc(4, 8, 64, 64, kvr.KVR_PAIR_NEOX_HALF, kvr.KVR_BF16, [1.0] * 32)
+    assert ok([seg(strides=(8 * 100 * 64, 100 * 64, 64))], model=m64) == kvr.KVR_ERR_UNSUPPORTED
+    m8, keep8 = kvr.model_desc(4, 8, 128, 128, kvr.KVR_PAIR_NEOX_HALF, kvr.KVR_FP8_E4M3, inv)
+    assert ok([seg()], model=m8) == kvr.KVR_ERR_UNSUPPORTED
+    assert kvr.kvr_attention_bytes_read(m, [seg(), seg(len=28)]) == 2 * 8 * 128 * 2 * 128
