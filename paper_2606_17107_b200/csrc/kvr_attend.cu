@@ -205,17 +205,16 @@ __global__ void __launch_bounds__(kThreads, 1) kvr_attend_kernel(const __grid_co
   }
   fence_async_smem();
   tc_fence_before();
-  // Programmatic dependent launch: everything above touches only this CTA's shared memory and TMEM; the previous launch
-  // on the stream (its partial buffers, tickets and outputs are reused by this one) must have completed before any
-  // global memory is touched.
+  // Programmatic dependent launch: everything above touches only this CTA's shared memory and TMEM and may overlap
+  // the tail of the previous launch on the stream.  That launch's partial buffers, tickets, item counter and outputs are
+  // reused by this one, and the query may be its product: griddepcontrol.wait is executed per role, by the threads that
+  // touch such memory -- the scheduler / query warp (the query, the item counter) and the epilogue warps (outputs,
+  // partials, tickets).  The work items and tensor maps were staged before this kernel could start.  With P.early (every segment carries
+  // KVR_SEG_SRC_STABLE: precompiled skills) the TMA producers do NOT wait: the K / V tiles of the CTA's first item
+  // stream in while the previous kernel on the stream drains; otherwise they wait as well.
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   __syncthreads();
   tc_fence_after();
-  // griddepcontrol.wait is executed per role, by the threads that touch global memory an earlier kernel may write: the
-  // scheduler / query warp (the query, the item counter) and the epilogue warps (outputs, partials, tickets).  The
-  // work items and tensor maps were staged before this kernel could start.  With P.early (every segment carries
-  // KVR_SEG_SRC_STABLE: precompiled skills) the TMA producers do NOT wait: the K / V tiles of the CTA's first item
-  // stream in while the previous kernel on the stream drains; otherwise they wait as well.
   auto dependency_wait = [] { asm volatile("griddepcontrol.wait;" ::: "memory"); };
   const uint32_t tmem = *tmem_slot;
   const uint32_t tm_s0 = tmem, tm_o0 = tmem + 32u;
