@@ -426,7 +426,7 @@ def measure_case(kvr, timer, ctx_of, w, dw, op, steps, warmup, min_device_s, pea
         "achieved": gbs(med), "best_achieved": gbs(best), "unit": "GB/s", "frac": gbs(med) / peak,
         "best_frac": gbs(best) / peak, "gb_s_of_nominal_8000": gbs(med) / 8000.0,
         "clocks": timer.sampler.summary(), "traffic": traffic_of(w.name, w.layout, op),
-        "kernel": {1: "kvr_generic_kernel", 2: "kvr_ring_kernel"}.get(info["path"], "?"),
+        "kernel": {1: "kvr_generic_kernel", 2: "kvr_ring_kernel", 4: "kvr_window_inplace_kernel"}.get(info["path"], "?"),
         "grid": info["grid"], "block": info["block"], "smem": info["smem"],
         "warmup": warmup, "warmup_ramp_steps": ramp,
     })

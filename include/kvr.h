@@ -301,7 +301,7 @@ KVR_API uint64_t kvr_bytes_moved(const kvr_model_desc* model, const kvr_segment*
 KVR_API kvr_status kvr_last_device_status(kvr_ctx* ctx, int32_t* bad_segment, int32_t* bad_token);
 
 /* Introspection for benchmarks: kernels launched by this context so far; the kernel path the last call took
- * (1 generic, 2 TMA ring, 3 rotate-on-read attention); grid size, CTA size and dynamic shared memory of its main kernel. */
+ * (1 generic, 2 TMA ring, 3 rotate-on-read attention, 4 window in place); grid size, CTA size and dynamic shared memory of its main kernel. */
 KVR_API uint64_t kvr_launch_count(const kvr_ctx* ctx);
 KVR_API kvr_status kvr_last_launch_info(const kvr_ctx* ctx, int32_t* path, int32_t* grid, int32_t* block,
                                         int32_t* smem_bytes);

@@ -571,6 +571,20 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     path = ok ? 2 : 1;
     break;
   }
+  if (path == 1 && tu.path == 0 && window_inplace_supported(P)) {
+    // in place on rows that carry position-free dims besides the rotary window (the MLA [latent | k_pe] row): the window
+    // kernel touches the window alone.  Units of all layers x one chunk, halved while there are fewer than 4 per SM.
+    P.tmajor = 0; P.ct = 0; P.tmaps = nullptr; P.gather = 0;
+    const int cg = chunk_granularity(d->block_size, 16);
+    int64_t chunks_total = 0;
+    for (int32_t i = 0; i < n; ++i)
+      chunks_total += ((int64_t)segs[i].dst_token_start + segs[i].len - 1) / cg - segs[i].dst_token_start / cg + 1;
+    int lpu = tu.layers_per_unit > 0 ? tu.layers_per_unit : m.layers;
+    if (tu.layers_per_unit <= 0)
+      while (lpu > 1 && chunks_total * ((m.layers + lpu - 1) / lpu) < (int64_t)4 * c->sm_count) lpu = (lpu + 1) / 2;
+    decompose(cg, lpu, 1, false);
+    path = 4;
+  }
   if (path == 1) {
     P.tmajor = 0; P.ct = 0; P.tmaps = nullptr; P.gather = 0;
     // generic kernel: chunk table [cg][R/2] float4 must fit 48 KB of static-limit shared memory
@@ -591,10 +605,12 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     RingConfig rc{tu.ctas_per_sm, tu.consumer_warps, tu.stages, tu.v_bulk_store, tu.max_ctas, tu.grab, tu.pdl, tu.warps_per_stage,
                   tu.lanes_over_heads, (use_tmaps && inline_descs) ? &tmaps_inline : nullptr};
     e = launch_ring(P, rc, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
+  } else if (path == 4) {
+    e = launch_window_inplace(P, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
   } else {
     e = launch_generic(P, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
   }
-  if (e != cudaSuccess) return c->cuda_fail(e, path == 2 ? "launch_ring" : "launch_generic");
+  if (e != cudaSuccess) return c->cuda_fail(e, path == 2 ? "launch_ring" : path == 4 ? "launch_window_inplace" : "launch_generic");
   c->launches += 1;
   c->last_path = path;
   c->last_stream = stream;

@@ -16,7 +16,7 @@ KVR_ERR_OUT_OF_RANGE, KVR_ERR_CUDA, KVR_ERR_NOMEM = -4, -5, -6
 KVR_BF16, KVR_FP8_E4M3 = 0, 1
 KVR_PAIR_NEOX_HALF, KVR_PAIR_GPTJ_INTERLEAVED = 0, 1
 KVR_SEG_PRE_ROPE, KVR_SEG_SRC_STABLE = 1, 2
-PATH_AUTO, PATH_GENERIC, PATH_RING, PATH_ATTEND = 0, 1, 2, 3
+PATH_AUTO, PATH_GENERIC, PATH_RING, PATH_ATTEND, PATH_WINDOW = 0, 1, 2, 3, 4
 
 
 class kvr_model_desc(C.Structure):

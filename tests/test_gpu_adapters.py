@@ -97,6 +97,7 @@ def test_mla_inplace_refloat(pairing, path):
         ctx.set_tuning(path=0 if path == "auto" else PATHS[path])
         dw.run_inplace(ctx, dw.inplace_spans(deltas))
         assert ctx.last_device_status()[0] == 0
+        assert ctx.last_launch_info()["path"] == (kvr.PATH_WINDOW if path == "auto" else PATHS[path])
     torch.cuda.synchronize()
     orc.inplace_workload(w, kc, deltas=deltas)
     got = np_bits(dw.k_cache)

@@ -15,6 +15,7 @@ from workloads import config, config_small, make_workload
 pytestmark = pytest.mark.gpu
 
 PATHS = {"generic": 1, "ring": 2}
+WINDOW = 4                      # kvr_last_launch_info path of the window in-place kernel (auto dispatch only)
 
 
 def _random_pool(w, seed):
@@ -43,9 +44,10 @@ def check_inplace(w, path, with_pos_map=False, null_v=False, declined_ok=False, 
     dk, dv = torch_bits(kc.copy()).cuda(), torch_bits(vc.copy()).cuda()
     dw = _PoolOnly(w, dk, None if null_v else dv)
     with kvr.Context(dw.model) as ctx:
-        ctx.set_tuning(path=PATHS[path], **tuning)
+        ctx.set_tuning(path=0 if path == "window" else PATHS[path], **tuning)
         spans = dw.inplace_spans(deltas, with_pos_map=with_pos_map)
-        assert kvr.kvr_inplace_bytes_moved(dw.model, spans) == 2 * w.layers * w.kv_heads * w.head_dim * w.elt_bytes * w.tokens
+        moved_dims = w.rotary_dim if getattr(w, "rotary_offset", 0) else w.head_dim        # kvr.h: only the window moves
+        assert kvr.kvr_inplace_bytes_moved(dw.model, spans) == 2 * w.layers * w.kv_heads * moved_dims * w.elt_bytes * w.tokens
         try:
             dw.run_inplace(ctx, spans)
         except kvr.KvrError as e:
@@ -55,7 +57,7 @@ def check_inplace(w, path, with_pos_map=False, null_v=False, declined_ok=False, 
         st = ctx.last_device_status()
         info = ctx.last_launch_info()
     torch.cuda.synchronize()
-    assert st[0] == 0 and info["path"] == PATHS[path], (st, info)
+    assert st[0] == 0 and info["path"] == (WINDOW if path == "window" else PATHS[path]), (st, info)
     ref = kc.copy()
     orc.inplace_workload(w, ref, deltas=deltas)
     gk = np_bits(dk)
@@ -73,8 +75,9 @@ def _untouched_mask(w, shape):
     """True for every pool element no (segment, token, rotary dim) addresses -- by brute force."""
     from tests.helpers import brute_force_offsets
     m = np.ones(shape, dtype=bool)
+    off = getattr(w, "rotary_offset", 0)               # the rotary window starts at rotary_offset inside the row
     for o in brute_force_offsets(w).values():
-        m[o:o + w.rotary_dim] = False
+        m[o + off:o + off + w.rotary_dim] = False
     return m
 
 
@@ -301,3 +304,54 @@ def test_seam_repair_overwrites_the_first_token_of_a_spliced_chunk():
                 assert np.array_equal(gk[o:o + w.head_dim], nk[l, h, t]) and np.array_equal(gv[o:o + w.head_dim], nv[l, h, t])
     assert np.array_equal(gv[~repaired], vc[~repaired])
     assert k_distance(w, gk[~repaired], kc[~repaired]).max() <= K_TOL["bf16"]
+
+
+@pytest.mark.parametrize("path", ["window", "generic"])
+@pytest.mark.parametrize("layout", ["NHD", "HND"])
+@pytest.mark.parametrize("pairing,D,R,off,dtype", [
+    ("neox", 576, 64, 512, "bf16"),      # the MLA [latent 512 | k_pe 64] row
+    ("gptj", 576, 64, 512, "bf16"),
+    ("neox", 96, 64, 16, "bf16"),        # head_dim 96: 192-byte rows, window in the middle
+    ("gptj", 96, 32, 32, "bf16"),
+    ("neox", 80, 16, 64, "bf16"),        # one lane per row (32-byte window)
+    ("neox", 192, 64, 128, "fp8"),       # fp8 codes rotated as they are (one scale in place)
+    ("gptj", 192, 128, 64, "fp8"),
+    ("neox", 1024, 512, 512, "bf16")])   # 16 lanes per row
+def test_inplace_window_kernel(pairing, D, R, off, dtype, layout, path):
+    """kvr_reposition_inplace on rows that carry position-free dims besides the rotary window (kvr_window.cu): auto
+    dispatch takes the window kernel, which touches the window alone; the generic kernel is the cross-check.  Several
+    heads, padded pool rows, block size 8, ragged chunks, five spans over two sequences, shifts of both signs and 0."""
+    pad = 8 if dtype == "bf16" else 16
+    w = make_workload(name="winip", layers=3, kv_heads=2 if D < 500 else 1, head_dim=D, rotary_dim=R, rotary_offset=off,
+                      pairing=pairing, dtype=dtype, theta=1e4, block_size=8, layout=layout, seed=1234, dst_head_pad=pad,
+                      slack=1.5, seq_segments=[[dict(len=1, dst_token_start=3), dict(len=37, dst_token_start=7),
+                                                dict(len=14, dst_token_start=49)],
+                                               [dict(len=5, dst_token_start=0), dict(len=23, dst_token_start=6)]])
+    check_inplace(w, path)
+
+
+def test_inplace_window_kernel_bad_block_and_many_spans():
+    """A bad block-table entry skips its chunk and raises the sticky status; 40 spans (staged descriptors) in one call."""
+    from paper_2606_17107_b200 import kvr
+    w = make_workload(name="winbad", layers=2, kv_heads=1, head_dim=576, rotary_dim=64, rotary_offset=512, theta=1e4,
+                      block_size=4, seed=2, has_v=False, seq_segments=[[dict(len=10, dst_token_start=2)]])
+    good = int(w.block_table[0, 2])
+    w.block_table[0, 2] = -1
+    kc, _ = _random_pool(w, 5)
+    dk = torch_bits(kc.copy()).cuda()
+    dw = _PoolOnly(w, dk, None)
+    with kvr.Context(dw.model) as ctx:
+        dw.run_inplace(ctx, dw.inplace_spans([9]))
+        st = ctx.last_device_status()
+        assert ctx.last_launch_info()["path"] == WINDOW
+    assert st[0] == kvr.KVR_ERR_OUT_OF_RANGE and st[1] == 0 and st[2] == 6
+    s_l, s_b, _, _ = w.dst_strides()
+    gk = np_bits(dk)
+    for l in range(w.layers):
+        o = l * s_l + good * s_b
+        assert np.array_equal(gk[o:o + s_b], kc[o:o + s_b])
+    assert not np.array_equal(gk, kc)
+    w2 = make_workload(name="winmany", layers=2, kv_heads=1, head_dim=576, rotary_dim=64, rotary_offset=512, theta=1e4,
+                       block_size=16, seed=3, has_v=False,
+                       seq_segments=[[dict(len=11, dst_token_start=13 * i) for i in range(40)]])
+    check_inplace(w2, "window", null_v=True)
