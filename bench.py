@@ -115,6 +115,9 @@ def config_block(w, op, config_index, layout, world):
     return {"workload": w.name, "op": op, "config_index": config_index, "layout": layout,
             "cache_dtype": CACHE_DTYPE[w.dtype], "tokens": w.tokens, "segments": len(w.segments),
             "bytes_per_step": b, "parallelism": f"replicas x{world}",
+            "sources": ("precompiled skills: every segment carries KVR_SEG_SRC_STABLE (kvr.h), so a launch may start reading its "
+                        "sources while the previous launch on the stream drains") if all(getattr(s_, "src_stable", False) for s_ in w.segments)
+                       else "no ordering promise (no early source loads)",
             "l2": (f"inputs larger than L2 ({b // 2} B of sources + as many pool bytes per step vs 126 MB L2); no flush")
                   if b // 2 > 2 * L2_BYTES else
                   (f"working set ({b} B per step) does NOT exceed the 126 MB L2 and is not flushed: a latency-bound "
