@@ -40,7 +40,7 @@ def test_both_arms_describe_the_workload_with_the_same_config_object():
         w = config(c, "NHD", layers=1)
         a = bench.config_block(w, "splice", c, "NHD", 1)
         assert set(a) == {"workload", "op", "config_index", "layout", "cache_dtype", "tokens", "segments",
-                          "bytes_per_step", "parallelism", "l2"}
+                          "bytes_per_step", "parallelism", "sources", "l2"}
         assert a["bytes_per_step"] == 4 * w.layers * w.kv_heads * w.head_dim * w.elt_bytes * w.tokens
     args = bench.parse_args([])
     assert args.config is None and bench.HEADLINE_CONFIG == 4          # the headline is the largest bf16 configuration
