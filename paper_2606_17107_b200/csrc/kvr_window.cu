@@ -18,8 +18,6 @@
 
 namespace kvr {
 
-namespace {
-
 template <int DTYPE, int PAIRING>
 __global__ void __launch_bounds__(256) kvr_window_inplace_kernel(const __grid_constant__ CallParams P, int log_lpr) {
   using G = Geo<DTYPE, PAIRING>;
@@ -96,8 +94,6 @@ __global__ void __launch_bounds__(256) kvr_window_inplace_kernel(const __grid_co
     }
   }
 }
-
-}  // namespace
 
 // rotary windows the kernel takes: rotary_dim * esz = 32 * 2^k bytes (k <= 5), at most 512 pairs, per-segment shifts
 bool window_inplace_supported(const CallParams& P) {
