@@ -561,7 +561,9 @@ __global__ void __launch_bounds__(kThreads, 1) kvr_attend_kernel(const __grid_co
         int* const flag = reinterpret_cast<int*>(smem + kOffMisc + 16);
         if (tid == 0) {
           __threadfence();
-          *flag = (atomicAdd(P.tickets + it.group, 1u) == (unsigned)it.group_count - 1u) ? 1 : 0;
+          const int last = atomicAdd(P.tickets + it.group, 1u) == (unsigned)it.group_count - 1u;
+          if (last) __threadfence();      // acquire: the other items' partials, released before their tickets, are visible
+          *flag = last;
         }
         named_bar_sync(2, 128);
         const bool do_merge = *flag != 0;
