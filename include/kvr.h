@@ -200,6 +200,46 @@ KVR_API kvr_status kvr_reposition_splice_host(kvr_ctx* ctx, const kvr_paged_dst*
                                               int32_t n_segs, void* cuda_stream);
 KVR_API uint64_t kvr_last_h2d_bytes(const kvr_ctx* ctx);
 
+/* ---- The hot path for callers that must not allocate ------------------------------------------------------
+ * kvr_create, and now and then the calls above, reserve device and pinned memory (cudaMalloc / cudaMallocHost).
+ * Some hosts of this library cannot let that happen:
+ *   - a serving engine that sized its KV pool to whatever HBM was left at start-up: a later cudaMalloc of even a
+ *     few KB can fail there, and the engine's memory accounting would not see it if it succeeded;
+ *   - a process in which some thread is recording a CUDA graph in the default (global) capture mode: cudaMalloc
+ *     from ANY thread then fails and invalidates that recording;
+ *   - a latency-critical step that cannot afford the device-wide synchronisation cudaMalloc / cudaFree may imply;
+ *   - a plug-in loaded under an allocator policy ("all device memory comes from the host application's pool") that
+ *     forbids driver allocations outright.
+ * For them: the same reposition + splice as kvr_reposition_splice -- same validation, same kernels, same results
+ * bit for bit -- WITHOUT a context and without a single CUDA allocation (no cudaMalloc, cudaMallocHost, cudaFree,
+ * stream or event creation).  What a context would hold on the device -- the unit scheduler's two counters, the
+ * sticky status word and the model's inv_freq table -- lives in ONE fixed array of KVR_NOALLOC_SCRATCH_BYTES bytes
+ * that is part of the library's device image: every GPU that loads the library carries it until the process exits,
+ * whether or not this call is ever made.
+ * Limits, rejected with KVR_ERR_UNSUPPORTED and a message in `err` before anything is enqueued:
+ *   n_segs <= KVR_NOALLOC_MAX_SEGMENTS (the descriptors then travel in the kernel parameters; split larger calls),
+ *   model->rotary_dim <= KVR_NOALLOC_MAX_ROTARY_DIM (room for its inv_freq in the array).
+ * Arguments: model / dst / segs / n_segs / cuda_stream as for kvr_create + kvr_reposition_splice (library default
+ * tuning); cuda_device = the device that owns every pointer and the stream.  device_status: NULL, or DEVICE int32[4]
+ * that this call zeroes and the kernel then fills if it meets a bad block-table entry ([0] != 0, [1] = segment,
+ * [2] = token; those tokens are skipped) -- read it after the stream has passed the call; with NULL the word stays
+ * in the array and is dropped.  err / err_len: NULL / 0, or a HOST buffer that receives a 0-terminated message
+ * whenever the result is not KVR_OK.
+ * First call on a device: looks up the array's device address (this can make the CUDA runtime load the library's
+ * device code), so make that call outside any stream capture; a one-token splice into a spare block will do.
+ * Every call: enqueues, on cuda_stream, a 64-byte clear of the counters and status word, a copy of inv_freq
+ * (rotary_dim/2 doubles, from pageable host memory: it is consumed before the call returns), and the kernel.
+ * Sharing: all calls on one device use the same array, and each one overwrites what the previous left there.  Calls
+ * on ONE stream are ordered and safe.  Two calls that can overlap on the GPU (different streams without an event
+ * between them, or two host threads' streams) race on the counters and the table and give undefined results; the
+ * host side is serialised by a lock, which does not order the GPU work. */
+#define KVR_NOALLOC_MAX_SEGMENTS 8
+#define KVR_NOALLOC_MAX_ROTARY_DIM 1024
+#define KVR_NOALLOC_SCRATCH_BYTES 4352
+KVR_API kvr_status kvr_reposition_splice_noalloc(const kvr_model_desc* model, int cuda_device, const kvr_paged_dst* dst,
+                                                 const kvr_segment* segs, int32_t n_segs, int32_t* device_status,
+                                                 void* cuda_stream, char* err, int32_t err_len);
+
 /* ---- NEXT-1: in-place reposition of a chunk that is ALREADY RESIDENT in the paged pool -------------------
  * PAPER.md:528 (App. H): "the user-memory chunk is precompiled once in isolation and RoPE-repositioned to float
  * just before the query each turn (an O(L_mem) re-rotation, no re-prefill)"; PAPER.md:167 (sec. 7).

@@ -2,6 +2,7 @@
 // descriptor staging and kernel dispatch.  No arithmetic of the method happens on the host.
 #include <algorithm>
 #include <cmath>
+#include <cstddef>
 #include <cstdio>
 #include <cstring>
 #include <mutex>
@@ -1127,5 +1128,133 @@ const char* kvr_status_string(kvr_status s) {
 const char* kvr_last_cuda_error(const kvr_ctx* c) { return c ? c->last_err.c_str() : ""; }
 
 const char* kvr_version(void) { return "kvr 0.1 (sm_100a)"; }
+
+}  // extern "C"
+
+// ---- reposition + splice for callers that must not allocate (kvr.h: kvr_reposition_splice_noalloc) ----
+// Everything a context keeps in device memory for this path, in one array that belongs to the library's device image
+// (one copy per GPU that loads the library, alive until the process exits).  Layout = NoAllocScratch below.
+namespace {
+
+constexpr int kNoAllocMaxPairs = KVR_NOALLOC_MAX_ROTARY_DIM / 2;
+struct NoAllocScratch {
+  unsigned long long sched[4];      // ring kernel: next unit, finished CTAs (zero when a launch starts)
+  int32_t status[4];                // sticky {flag, segment, token, -} when the caller passes no device_status
+  int32_t pad_[4];
+  double inv_freq[kNoAllocMaxPairs];
+};
+constexpr size_t kNoAllocHeaderBytes = 64;   // sched + status + pad_: what every call clears
+static_assert(offsetof(NoAllocScratch, inv_freq) == kNoAllocHeaderBytes, "header is 64 bytes");
+static_assert(sizeof(NoAllocScratch) <= KVR_NOALLOC_SCRATCH_BYTES, "kvr.h states the size of the array");
+
+// In HOST code this name is only a handle for cudaGetSymbolAddress: it is not a device address and must never be given
+// to a kernel or a cudaMemcpy as one.  noalloc_device_state() asks the runtime for the real address, once per device.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[KVR_NOALLOC_SCRATCH_BYTES];
+
+struct NoAllocDevice {
+  bool ready = false;
+  unsigned char* base = nullptr;    // device address of g_noalloc_scratch on this device
+  kvr_ctx* ctx = nullptr;           // host-only bookkeeping (owns no CUDA resource); its device pointers aim into `base`
+};
+constexpr int kNoAllocMaxDevices = 64;
+NoAllocDevice g_noalloc_dev[kNoAllocMaxDevices];
+std::mutex g_noalloc_mu;
+
+kvr_status noalloc_fail(kvr_status st, char* err, int32_t err_len, const char* fmt, long long a = 0, long long b = 0) {
+  if (err && err_len > 0) std::snprintf(err, (size_t)err_len, fmt, a, b);
+  return st;
+}
+
+// Set-up, once per device, with that device current (the caller holds g_noalloc_mu and a DeviceGuard).
+kvr_status noalloc_device_state(int dev, NoAllocDevice** out, char* err, int32_t err_len) {
+  NoAllocDevice& d = g_noalloc_dev[dev];
+  if (!d.ready) {
+    int major = 0, sms = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) {
+      (void)cudaGetLastError();
+      return noalloc_fail(KVR_ERR_CUDA, err, err_len, "kvr_reposition_splice_noalloc: cannot query device %lld (CUDA error %lld)", dev, (long long)e);
+    }
+    if (major != 10)
+      return noalloc_fail(KVR_ERR_UNSUPPORTED, err, err_len, "kvr_reposition_splice_noalloc: device %lld has compute capability %lld.x; the library is built for sm_100a", dev, major);
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (e != cudaSuccess || !p) {
+      (void)cudaGetLastError();
+      return noalloc_fail(KVR_ERR_CUDA, err, err_len, "kvr_reposition_splice_noalloc: cudaGetSymbolAddress failed on device %lld (CUDA error %lld)", dev, (long long)e);
+    }
+    if (!d.ctx) d.ctx = new (std::nothrow) kvr_ctx();
+    if (!d.ctx) return noalloc_fail(KVR_ERR_NOMEM, err, err_len, "kvr_reposition_splice_noalloc: out of host memory");
+    d.base = static_cast<unsigned char*>(p);
+    d.ctx->device = dev;
+    d.ctx->sm_count = sms;
+    d.ctx->d_sched = reinterpret_cast<unsigned long long*>(d.base + offsetof(NoAllocScratch, sched));
+    d.ctx->d_inv_freq = reinterpret_cast<double*>(d.base + offsetof(NoAllocScratch, inv_freq));
+    d.ready = true;
+  }
+  *out = &d;
+  return KVR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+kvr_status kvr_reposition_splice_noalloc(const kvr_model_desc* model, int cuda_device, const kvr_paged_dst* dst,
+                                         const kvr_segment* segs, int32_t n, int32_t* device_status, void* cuda_stream,
+                                         char* err, int32_t err_len) {
+  if (err && err_len > 0) err[0] = 0;
+  // ---- host-only checks: nothing below this block runs unless the call fits the fixed array ----
+  kvr_status st = check_call(model, dst, segs, n);
+  if (st == KVR_OK && n > 0) st = check_deltas(segs, n);
+  if (st != KVR_OK) return noalloc_fail(st, err, err_len, "kvr_reposition_splice_noalloc: invalid arguments (see kvr_validate)");
+  if (n > KVR_NOALLOC_MAX_SEGMENTS)
+    return noalloc_fail(KVR_ERR_UNSUPPORTED, err, err_len,
+                        "kvr_reposition_splice_noalloc: %lld segments, but a call without allocations carries at most %lld "
+                        "(KVR_NOALLOC_MAX_SEGMENTS); split the call", n, KVR_NOALLOC_MAX_SEGMENTS);
+  if (model->rotary_dim > KVR_NOALLOC_MAX_ROTARY_DIM)
+    return noalloc_fail(KVR_ERR_UNSUPPORTED, err, err_len,
+                        "kvr_reposition_splice_noalloc: rotary_dim %lld, but the fixed device array has room for %lld "
+                        "(KVR_NOALLOC_MAX_ROTARY_DIM)", model->rotary_dim, KVR_NOALLOC_MAX_ROTARY_DIM);
+  if (device_status && (reinterpret_cast<uintptr_t>(device_status) & 3u))
+    return noalloc_fail(KVR_ERR_ALIGNMENT, err, err_len, "kvr_reposition_splice_noalloc: device_status is not 4-byte aligned");
+  if (cuda_device < 0 || cuda_device >= kNoAllocMaxDevices)
+    return noalloc_fail(KVR_ERR_INVALID_ARG, err, err_len, "kvr_reposition_splice_noalloc: cuda_device %lld out of range", cuda_device);
+  if (n == 0) return KVR_OK;
+
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);      // orders the HOST side only; GPU work of overlapping calls races (kvr.h)
+  int count = 0;
+  if (cudaGetDeviceCount(&count) != cudaSuccess || cuda_device >= count) {
+    (void)cudaGetLastError();
+    return noalloc_fail(KVR_ERR_CUDA, err, err_len, "kvr_reposition_splice_noalloc: no CUDA device %lld (there is no CPU fallback)", cuda_device);
+  }
+  DeviceGuard guard(cuda_device);
+  NoAllocDevice* d = nullptr;
+  if ((st = noalloc_device_state(cuda_device, &d, err, err_len)) != KVR_OK) return st;
+  kvr_ctx* c = d->ctx;
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  c->last_err.clear();
+  c->model = *model;                       // inv_freq stays the caller's HOST pointer: only the copy below reads it
+  c->tuning = kvr_tuning{};
+  c->d_status = device_status ? device_status : reinterpret_cast<int32_t*>(d->base + offsetof(NoAllocScratch, status));
+
+  // The array keeps whatever the last call left: the counters and the status word must be zero when the kernel starts.
+  cudaError_t e = cudaMemsetAsync(d->base, 0, kNoAllocHeaderBytes, stream);
+  if (e == cudaSuccess && device_status) e = cudaMemsetAsync(device_status, 0, 4 * sizeof(int32_t), stream);
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(c->d_inv_freq, model->inv_freq, (size_t)(model->rotary_dim / 2) * sizeof(double),
+                        cudaMemcpyHostToDevice, stream);
+  if (e != cudaSuccess) {
+    (void)cudaGetLastError();
+    return noalloc_fail(KVR_ERR_CUDA, err, err_len, "kvr_reposition_splice_noalloc: staging the scratch array failed (CUDA error %lld)", (long long)e);
+  }
+  // n <= kInlineSegs: enqueue_layers builds the descriptors in c->inline_scratch (host) and passes them in the kernel
+  // parameters; it touches no staging slot and allocates nothing.
+  static_assert(KVR_NOALLOC_MAX_SEGMENTS <= kInlineSegs, "descriptors must fit the kernel parameters");
+  st = enqueue_layers(c, dst, segs, n, stream, 0, model->layers, false);
+  if (st != KVR_OK && err && err_len > 0) std::snprintf(err, (size_t)err_len, "kvr_reposition_splice_noalloc: %s", c->last_err.c_str());
+  return st;
+}
 
 }  // extern "C"

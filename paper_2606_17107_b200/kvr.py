@@ -16,6 +16,7 @@ KVR_ERR_OUT_OF_RANGE, KVR_ERR_CUDA, KVR_ERR_NOMEM = -4, -5, -6
 KVR_BF16, KVR_FP8_E4M3 = 0, 1
 KVR_PAIR_NEOX_HALF, KVR_PAIR_GPTJ_INTERLEAVED = 0, 1
 KVR_SEG_PRE_ROPE, KVR_SEG_SRC_STABLE = 1, 2
+KVR_NOALLOC_MAX_SEGMENTS, KVR_NOALLOC_MAX_ROTARY_DIM, KVR_NOALLOC_SCRATCH_BYTES = 8, 1024, 4352
 PATH_AUTO, PATH_GENERIC, PATH_RING, PATH_ATTEND, PATH_WINDOW = 0, 1, 2, 3, 4
 
 
@@ -72,6 +73,7 @@ class kvr_read_segment(C.Structure):
 
 EXPORTS = ["kvr_rotate_on_read_attention", "kvr_attention_bytes_read", "kvr_validate_read", "kvr_reposition_inplace", "kvr_inplace_bytes_moved", "kvr_write_span",
            "kvr_create", "kvr_destroy", "kvr_set_tuning", "kvr_validate", "kvr_reposition_splice",
+           "kvr_reposition_splice_noalloc",
            "kvr_reposition_splice_host", "kvr_last_h2d_bytes",
            "kvr_bytes_moved", "kvr_last_device_status", "kvr_launch_count", "kvr_last_launch_info",
            "kvr_status_string", "kvr_last_cuda_error", "kvr_version"]
@@ -93,6 +95,9 @@ def _load():
     lib.kvr_validate.argtypes = [P(kvr_model_desc), P(kvr_paged_dst), P(kvr_segment), C.c_int32]
     lib.kvr_reposition_splice.restype = C.c_int
     lib.kvr_reposition_splice.argtypes = [C.c_void_p, P(kvr_paged_dst), P(kvr_segment), C.c_int32, C.c_void_p]
+    lib.kvr_reposition_splice_noalloc.restype = C.c_int
+    lib.kvr_reposition_splice_noalloc.argtypes = [P(kvr_model_desc), C.c_int, P(kvr_paged_dst), P(kvr_segment), C.c_int32,
+                                                  C.c_void_p, C.c_void_p, C.c_char_p, C.c_int32]
     lib.kvr_reposition_splice_host.restype = C.c_int
     lib.kvr_reposition_splice_host.argtypes = lib.kvr_reposition_splice.argtypes
     lib.kvr_reposition_inplace.restype = C.c_int
@@ -223,6 +228,24 @@ def kvr_validate(model, dst, segs):
 def kvr_bytes_moved(model, segs):
     arr = segs if not isinstance(segs, (list, tuple)) else segment_array(segs)
     return int(lib.kvr_bytes_moved(C.byref(model), arr, len(arr)))
+
+
+def kvr_reposition_splice_noalloc(model, dst, segs, device=0, device_status=None, stream=None, check=True):
+    """kvr_reposition_splice_noalloc (kvr.h): the reposition + splice for hosts that cannot let this library allocate
+    CUDA memory (an engine that gave all free HBM to its KV pool, a process with a graph capture in flight on another
+    thread, a plug-in under a no-driver-allocations policy).  No Context: the scheduler counters, status word and
+    inv_freq table sit in a fixed 4352-byte array inside the library's device image, shared by every call on the device,
+    so calls must not overlap on the GPU.  At most 8 segments and rotary_dim <= 1024 per call (KvrError otherwise).
+    device_status: optional device int32[4] that receives {flag, segment, token, -} for a bad block-table entry.
+    Make the first call on a device outside any stream capture."""
+    arr = segs if not isinstance(segs, (list, tuple)) else segment_array(segs)
+    s = None if stream is None else (stream if isinstance(stream, int) else stream.cuda_stream)
+    msg = C.create_string_buffer(256)
+    st = lib.kvr_reposition_splice_noalloc(C.byref(model), device, C.byref(dst), arr, len(arr), _ptr(device_status), s,
+                                           msg, len(msg))
+    if check and st != KVR_OK:
+        raise KvrError(st, msg.value.decode())
+    return st
 
 
 def kvr_version():
