@@ -78,7 +78,11 @@ int kvr_oracle_rotate_on_read_attention(
     const int h = g / group;
     double* x = (double*)malloc((size_t)total * sizeof(double));   /* every score of this head */
     double* kp = (double*)malloc((size_t)head_dim * sizeof(double));
-    if (!x || !kp) { fail = 1; free(x); free(kp); continue; }
+    if (!x || !kp) {
+#pragma omp atomic write
+      fail = 1;
+      free(x); free(kp); continue;
+    }
     /* scores: rotate the key, then the dot product */
     int64_t n = 0;
     for (int s = 0; s < n_segs; ++s)

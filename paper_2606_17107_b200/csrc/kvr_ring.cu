@@ -794,7 +794,7 @@ bool ring_supported(const CallParams& P, const SegDev* segs, const RingConfig& c
   if (ring_window_mode(P)) {
     if (rowB < 32 || rowB > 4096 || rowB % 16) w = "window mode: head_dim*esz must be a multiple of 16 in [32, 4096] bytes";
     else if (rotB % 32 || rotB > 1024 || ((rotB / 32) & (rotB / 32 - 1))) w = "window mode: rotary_dim*esz must be 32 * a power of two, <= 1024";
-    else if (P.inplace) w = "window mode: in-place calls take the generic kernel (it touches only the rotary window)";
+    else if (P.inplace) w = "window mode: in-place calls take kvr_window_inplace_kernel (it touches only the rotary window)";
   }
   else if (rowB < 32 || rowB > 1024 || (rowB & (rowB - 1))) w = "head_dim*esz must be a power of two in [32, 1024] bytes";
   else if (P.pairing == 0 && (P.rotary_dim * E) % 32) w = "NeoX pairing needs rotary_dim*esz % 32 == 0";
