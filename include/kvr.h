@@ -310,7 +310,10 @@ KVR_API kvr_status kvr_write_span(kvr_ctx* ctx, const kvr_paged_dst* dst, const 
  * call (the second merges the partial results of (request, kv head) groups that were split over many CTAs).  Reads
  * 2 * kv_heads * head_dim * 2 bytes per token (kvr_attention_bytes_read): K and V of one layer, once.  Outputs are
  * written only by this call's kernels; partial results live in context-owned device memory, so calls on one context
- * must be issued to one stream at a time (as for every other call). */
+ * must be issued to one stream at a time (as for every other call).  Changing streams between calls: an eager call
+ * that finds its descriptors cached but was issued on another stream than the previous one first waits (on the
+ * device) for that stream's call; a CAPTURED call cannot do so, so capture on the stream of the eager call or
+ * synchronise that stream before the capture begins. */
 typedef struct {
   const void* k_src;
   const void* v_src;
@@ -326,7 +329,9 @@ KVR_API kvr_status kvr_rotate_on_read_attention(kvr_ctx* ctx, const void* q, int
                                                 float* o, float* lse, void* cuda_stream);
 KVR_API uint64_t kvr_attention_bytes_read(const kvr_model_desc* model, const kvr_read_segment* segs, int32_t n_segs);
 /* Host-only validation of a kvr_rotate_on_read_attention call (no CUDA call is made; usable without a GPU): the status
- * the call returns before it enqueues anything (pointers are only checked for NULL and alignment). */
+ * the call returns before it enqueues anything (pointers are only checked for NULL and alignment; what a TMA tensor
+ * map cannot describe -- a zero layer stride with layers > 1, a stride of 2^40 bytes or more -- is
+ * KVR_ERR_UNSUPPORTED; n_req > n_segs is KVR_ERR_INVALID_ARG since every request must own a segment). */
 KVR_API kvr_status kvr_validate_read(const kvr_model_desc* model, const void* q, int32_t n_req, int32_t q_heads, int32_t layer,
                                      float softmax_scale, const kvr_read_segment* segs, int32_t n_segs, const float* o,
                                      const float* lse);

@@ -176,6 +176,7 @@ struct kvr_ctx {
     std::vector<unsigned char> key; int32_t n_req = 0, q_heads = 0, tpi_tuning = 0, n_groups = 0;
     size_t n_items = 0, seg_bytes = 0, n_merges = 0; int32_t merge_max = 0; uint64_t last_use = 0;
     bool pinned = false;          // captured in a CUDA graph: never evicted
+    cudaStream_t last_stream = nullptr;   // stream of the last eager call on this entry (`ev` was recorded there)
   };
   static constexpr int kAttnSlots = 8;
   AttnSlot attn_slots[kAttnSlots];
@@ -680,7 +681,9 @@ kvr_status kvr_validate_read(const kvr_model_desc* mp, const void* q, int32_t n_
   if (q_heads % m.kv_heads != 0 || !(softmax_scale > 0.0f) || !std::isfinite(softmax_scale)) return KVR_ERR_INVALID_ARG;
   if (!aligned16(q) || !aligned16(o) || (reinterpret_cast<uintptr_t>(lse) & 3u)) return KVR_ERR_ALIGNMENT;
   if (m.dtype != KVR_BF16 || m.head_dim != 128 || q_heads / m.kv_heads > 16) return KVR_ERR_UNSUPPORTED;
-  std::vector<int32_t> per_req((size_t)n_req, 0);
+  if (n_req > n) return KVR_ERR_INVALID_ARG;      // every request must own a segment (also bounds the vector below)
+  std::vector<int32_t> per_req;
+  try { per_req.assign((size_t)n_req, 0); } catch (const std::bad_alloc&) { return KVR_ERR_NOMEM; }
   for (int32_t i = 0; i < n; ++i) {
     const kvr_read_segment& s = segs[i];
     if (!s.k_src || !s.v_src || s.len <= 0 || s.request < 0 || s.request >= n_req || (s.flags & ~KVR_SEG_SRC_STABLE)) return KVR_ERR_INVALID_ARG;
@@ -688,6 +691,11 @@ kvr_status kvr_validate_read(const kvr_model_desc* mp, const void* q, int32_t n_
     if ((s.src_stride_head < m.head_dim && m.kv_heads > 1)) return KVR_ERR_INVALID_ARG;
     if (!aligned16(s.k_src) || !aligned16(s.v_src)) return KVR_ERR_ALIGNMENT;
     if ((s.src_stride_layer * 2) % 16 || (s.src_stride_head * 2) % 16 || (s.src_stride_token * 2) % 16) return KVR_ERR_ALIGNMENT;
+    // what a TMA tensor map can describe (encode_attn_map): a dimension of extent > 1 needs a non-zero stride, strides
+    // stay below 2^40 bytes
+    if ((s.src_stride_layer == 0 && m.layers > 1) || (s.src_stride_head == 0 && m.kv_heads > 1)) return KVR_ERR_UNSUPPORTED;
+    const int64_t lim = (int64_t)1 << 39;           // elements of 2 bytes
+    if (s.src_stride_layer >= lim || s.src_stride_head >= lim || s.src_stride_token >= lim) return KVR_ERR_UNSUPPORTED;
     per_req[(size_t)s.request] += 1;
   }
   for (int32_t r = 0; r < n_req; ++r)
@@ -695,9 +703,25 @@ kvr_status kvr_validate_read(const kvr_model_desc* mp, const void* q, int32_t n_
   return KVR_OK;
 }
 
+static kvr_status attend_call(kvr_ctx* c, const void* q, int32_t n_req, int32_t q_heads, int32_t layer,
+                              float softmax_scale, const kvr_read_segment* segs, int32_t n, float* o, float* lse,
+                              void* cuda_stream);
+
+// The C ABI never throws: the host-side decomposition builds std::vectors sized by the caller's numbers.
 kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req, int32_t q_heads, int32_t layer,
                                         float softmax_scale, const kvr_read_segment* segs, int32_t n, float* o, float* lse,
                                         void* cuda_stream) {
+  try {
+    return attend_call(c, q, n_req, q_heads, layer, softmax_scale, segs, n, o, lse, cuda_stream);
+  } catch (const std::bad_alloc&) {
+    if (c) c->last_err = "rotate-on-read attention: out of host memory while building the work items";
+    return KVR_ERR_NOMEM;
+  }
+}
+
+static kvr_status attend_call(kvr_ctx* c, const void* q, int32_t n_req, int32_t q_heads, int32_t layer,
+                              float softmax_scale, const kvr_read_segment* segs, int32_t n, float* o, float* lse,
+                              void* cuda_stream) {
   if (!c) return KVR_ERR_INVALID_ARG;
   c->last_err.clear();
   const kvr_model_desc& m = c->model;
@@ -811,6 +835,11 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
     slot.n_req = n_req; slot.q_heads = q_heads; slot.tpi_tuning = c->tuning.layers_per_unit + 1000 * c->tuning.hsplit;
     slot.key.assign(reinterpret_cast<const unsigned char*>(segs), reinterpret_cast<const unsigned char*>(segs) + key_bytes);
   }
+  if (hit && slot.pending && stream != slot.last_stream) {
+    // The descriptors were copied in on another stream: order this stream behind that copy.  Under capture an event
+    // recorded outside the capture cannot be waited on, so the caller must have synchronised that stream (kvr.h).
+    if (!capturing) KVR_CUDA(c, cudaStreamWaitEvent(stream, slot.ev, 0));
+  }
   const size_t n_items = slot.n_items, seg_bytes = slot.seg_bytes;
   const int32_t n_groups = slot.n_groups;
   // partial results and tickets (grown on demand; a regrowth waits for the launches that may still use the old buffers)
@@ -833,7 +862,6 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
     }
     if ((size_t)n_groups > c->attn_ticket_cap) {
       if (c->attn_tickets) cudaFree(c->attn_tickets);
-  for (void* p : c->attn_retired) cudaFree(p);
       c->attn_tickets = nullptr; c->attn_ticket_cap = 0;
       size_t cap = std::max<size_t>((size_t)n_groups * 2, 1024);
       KVR_CUDA(c, cudaMalloc(&c->attn_tickets, cap * sizeof(unsigned int)));
@@ -871,6 +899,7 @@ kvr_status kvr_rotate_on_read_attention(kvr_ctx* c, const void* q, int32_t n_req
   } else if (!slot.pinned) {
     KVR_CUDA(c, cudaEventRecord(slot.ev, stream));      // the entry may be replaced once this launch has run
     slot.pending = true;
+    slot.last_stream = stream;
   }
   return KVR_OK;
 }
