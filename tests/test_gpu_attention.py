@@ -6,7 +6,8 @@ Two comparisons per case, both element by element:
      derives from the kernel's arithmetic contract: the counter-rotated query is rounded once to bf16, so score j is off
      by at most E_j = scale * sum_d |q'_d - bf16(q'_d)| * |k_jd| (computed here exactly, per query head), the softmax
      weights are rounded to bf16 (relative 2^-9 each, numerator and denominator alike), everything else is fp32:
-         |o - o_ref|   <= (expm1(2 max_j E_j) + 2^-8 + 2^-12) * max_j |v_jd|
+         |o - o_ref|[g, d] <= first-order term + kappa(E) sum_j w_j |v_jd - o_d| + 2^-7 sum_j w_j |v_jd| + 2^-12 max_j |v_jd|
+                              (reference() below and DESIGN.md section 3: per element, a few per cent of |o|, not of max |v|)
          |lse - lse_ref| <= max_j E_j + 2^-8
  (2) against the same definition evaluated with the bf16-rounded counter-rotated query (numpy fp64; "both sides take
      the rounding decision in the same precision"): what is left is the bf16 rounding of the weights and fp32
@@ -51,7 +52,13 @@ def counter_rotate(q, delta, inv_freq, R, pairing, offset):
 
 
 def reference(w, srcs, q_bits, n_threads):
-    """Per request: oracle (o, lse), the bf16-query model (o, lse, sum_j w_j |v_j|), E = max_j E_j and max_j |v_jd|."""
+    """Per request: oracle (o, lse); the bf16-query model (o, lse, sum_j w_j |v_j|); E = max_j E_j, max_j |v_jd|; and
+    tol_ref[g, d], the per-element bound on |o_kernel - o_oracle| that DESIGN.md section 3 derives:
+        scale * sum_s sum_c u^(s)_c |C^(s)_cd|  +  kappa(E) * sum_j w_j |v_jd - o_d|  +  2^-7 sum_j w_j |v_jd|  +  2^-12 max_j |v_jd|
+    with w, o the ORACLE's weights and output, u^(s) = |q'^(s) - bf16(q'^(s))| the rounding error of the query counter-
+    rotated for segment s, C^(s)_cd = sum_{j in s} w_j k_jc (v_jd - o_d)  (first order in the score error: the softmax
+    weights sum to one, so only the covariance of keys and values under w is seen), and
+    kappa(E) = e^E (2 (e^E - 1 - E)(1 + E) + 2 E^2) the bound on everything beyond first order."""
     D, G = w.head_dim, w.q_heads // w.kv_heads
     out = []
     for r in range(w.n_req):
@@ -61,24 +68,40 @@ def reference(w, srcs, q_bits, n_threads):
             scale=w.scale, rotary_offset=w.rotary_offset, n_threads=n_threads,
             segments=[(srcs[i][0][w.layer][:, :, :D], srcs[i][1][w.layer][:, :, :D], s.delta) for i, s in segs])
         qv = bf16_val(q_bits[r])                                       # [Hq, D]
-        xs, vs, E = [], [], np.zeros(w.q_heads)
-        for i, s in segs:
-            k = bf16_val(srcs[i][0][w.layer][:, :, :D])                 # [Hkv, L, D]
-            v = bf16_val(srcs[i][1][w.layer][:, :, :D])
-            qp = counter_rotate(qv, s.delta, w.inv_freq, w.rotary_dim, w.pairing, w.rotary_offset)
-            qb = bf16_round(qp)
-            kk = np.repeat(k, G, axis=0)                                # [Hq, L, D]
-            xs.append(w.scale * np.einsum("gd,gld->gl", qb, kk))
-            E = np.maximum(E, w.scale * np.einsum("gd,gld->gl", np.abs(qp - qb), np.abs(kk)).max(axis=1))
-            vs.append(np.repeat(v, G, axis=0))
-        x, v = np.concatenate(xs, axis=1), np.concatenate(vs, axis=1)   # [Hq, T], [Hq, T, D]
-        m = x.max(axis=1, keepdims=True)
-        p = np.exp(x - m)
-        z = p.sum(axis=1, keepdims=True)
-        wgt = p / z
-        out.append(dict(o_ref=o_ref, lse_ref=lse_ref, o_model=np.einsum("gt,gtd->gd", wgt, v),
-                        lse_model=(m + np.log(z))[:, 0], wabsv=np.einsum("gt,gtd->gd", wgt, np.abs(v)),
-                        vmax=np.abs(v).max(axis=1), E=E))
+        ks = [bf16_val(srcs[i][0][w.layer][:, :, :D]) for i, s in segs]   # per segment [Hkv, L, D]
+        vs = [bf16_val(srcs[i][1][w.layer][:, :, :D]) for i, s in segs]
+        qps = [counter_rotate(qv, s.delta, w.inv_freq, w.rotary_dim, w.pairing, w.rotary_offset) for i, s in segs]
+        qbs = [bf16_round(qp) for qp in qps]
+        cuts = np.cumsum([0] + [s.len for i, s in segs])
+        R = dict(o_ref=o_ref, lse_ref=lse_ref, o_model=np.zeros((w.q_heads, D)), lse_model=np.zeros(w.q_heads),
+                 wabsv=np.zeros((w.q_heads, D)), vmax=np.zeros((w.q_heads, D)), E=np.zeros(w.q_heads),
+                 tol_ref=np.zeros((w.q_heads, D)), tol_first_order=np.zeros((w.q_heads, D)))
+        for g in range(w.q_heads):
+            h = g // G
+            v = np.concatenate([v_[h] for v_ in vs], axis=0)                                      # [T, D]
+            x_b = np.concatenate([w.scale * (k[h] @ qb[g]) for k, qb in zip(ks, qbs)])            # bf16-query scores
+            x = np.concatenate([w.scale * (k[h] @ qp[g]) for k, qp in zip(ks, qps)])              # exact scores
+            E = max(float((w.scale * (np.abs(k[h]) @ np.abs(qp[g] - qb[g]))).max()) for k, qp, qb in zip(ks, qps, qbs))
+            # the bf16-query model
+            m = x_b.max(); p = np.exp(x_b - m); z = p.sum(); wb = p / z
+            R["o_model"][g] = wb @ v
+            R["lse_model"][g] = m + np.log(z)
+            R["wabsv"][g] = wb @ np.abs(v)
+            R["vmax"][g] = np.abs(v).max(axis=0)
+            R["E"][g] = E
+            # the oracle-side bound (weights and output of the definition itself)
+            p = np.exp(x - x.max()); wt = p / p.sum()
+            o = wt @ v
+            dv = v - o
+            first = np.zeros(D)
+            for si, (k, qp, qb) in enumerate(zip(ks, qps, qbs)):
+                a, b = cuts[si], cuts[si + 1]
+                C = (k[h] * wt[a:b, None]).T @ dv[a:b]                                             # [D(c), D(d)]
+                first += w.scale * (np.abs(qp[g] - qb[g]) @ np.abs(C))
+            kappa = np.exp(E) * (2 * (np.expm1(E) - E) * (1 + E) + 2 * E * E)
+            R["tol_first_order"][g] = first + kappa * (wt @ np.abs(dv))
+            R["tol_ref"][g] = R["tol_first_order"][g] + 2.0 ** -7 * (wt @ np.abs(v)) + 2.0 ** -12 * R["vmax"][g]
+        out.append(R)
     return out
 
 
@@ -106,9 +129,8 @@ def run_and_check(w, tuning=None, n_threads=None, layer=None):
     ref = reference(w, srcs, np_bits(q_t), n_threads or orc.host_threads())
     worst = 0.0
     for r, R in enumerate(ref):
-        E = R["E"][:, None]
-        tol_o = (np.expm1(2 * E) + 2.0 ** -8 + 2.0 ** -12) * R["vmax"]
-        assert (np.abs(o[r] - R["o_ref"]) <= tol_o).all(), (r, float(np.abs(o[r] - R["o_ref"]).max()), float(tol_o.min()))
+        tol_o = R["tol_ref"]
+        assert (np.abs(o[r] - R["o_ref"]) <= tol_o).all(), (r, float((np.abs(o[r] - R["o_ref"]) / tol_o).max()))
         assert (np.abs(lse[r] - R["lse_ref"]) <= R["E"] + 2.0 ** -8).all(), (r, float(np.abs(lse[r] - R["lse_ref"]).max()))
         tol_m = 2.0 ** -7 * R["wabsv"] + 2.0 ** -12 * R["vmax"]
         d = np.abs(o[r] - R["o_model"])
@@ -257,9 +279,10 @@ def test_argument_errors_and_limits():
 
 
 @pytest.mark.parametrize("name", ["attend-compose4", "attend-32k-x8", "attend-serving"])
-def test_full_size_sampled_requests(name):
-    """BASELINE-sized calls in the launch configuration bench.py times: the whole call runs on the GPU; the oracle
-    checks a sample of requests completely (every query head and dim of them)."""
+def test_full_size_every_request(name):
+    """BASELINE-sized calls in the launch configuration bench.py times: the whole call runs on the GPU and EVERY request
+    of it (all query heads and dims) is checked against the oracle and against the bf16-query model, at the tolerances of
+    the small cases."""
     from paper_2606_17107_b200 import kvr
     from paper_2606_17107_b200.harness import DeviceReadWorkload
     w = attention_config(name)
@@ -270,16 +293,22 @@ def test_full_size_sampled_requests(name):
         assert ctx.last_launch_info()["grid"] == torch.cuda.get_device_properties(0).multi_processor_count
     o, lse = dw.o.cpu().numpy().astype(np.float64), dw.lse.cpu().numpy().astype(np.float64)
     assert np.isfinite(o).all() and np.isfinite(lse).all()
-    sample = sorted({0, w.n_req // 2, w.n_req - 1})[: (1 if name == "attend-32k-x8" else 3)]
-    for r in sample:
+    q_bits = np_bits(dw.q)
+    for r in range(w.n_req):
         idx = [i for i, s in enumerate(w.segments) if s.request == r]
         sub = read_workload("sub", q_heads=w.q_heads, kv_heads=w.kv_heads, layers=w.layers, layer=w.layer,
                             requests=[[(w.segments[i].len, w.segments[i].delta) for i in idx]], seed=0, inv_freq=w.inv_freq)
-        srcs = [(np_bits(dw.sources[i][0]), np_bits(dw.sources[i][1])) for i in idx]
-        R = reference(sub, srcs, np_bits(dw.q[r:r + 1]), orc.host_threads())[0]
+        # only this request's layer of its sources comes to the host (the other layers stay zero: reference() reads one)
+        srcs = []
+        for i in idx:
+            k, v = dw.sources[i]
+            kh, vh = np.zeros(tuple(k.shape), np.uint16), np.zeros(tuple(v.shape), np.uint16)
+            kh[w.layer], vh[w.layer] = np_bits(k[w.layer]), np_bits(v[w.layer])
+            srcs.append((kh, vh))
+        R = reference(sub, srcs, q_bits[r:r + 1], orc.host_threads())[0]
         assert (np.abs(o[r] - R["o_model"]) <= 2.0 ** -7 * R["wabsv"] + 2.0 ** -12 * R["vmax"]).all(), r
         assert (np.abs(lse[r] - R["lse_model"]) <= 2.0 ** -8).all(), r
-        assert (np.abs(o[r] - R["o_ref"]) <= (np.expm1(2 * R["E"][:, None]) + 2.0 ** -8 + 2.0 ** -12) * R["vmax"]).all(), r
+        assert (np.abs(o[r] - R["o_ref"]) <= R["tol_ref"]).all(), (r, float((np.abs(o[r] - R["o_ref"]) / R["tol_ref"]).max()))
         assert (np.abs(lse[r] - R["lse_ref"]) <= R["E"] + 2.0 ** -8).all(), r
 
 
@@ -354,3 +383,47 @@ def test_cuda_graph_of_cached_calls_replays_after_cache_churn():
             for r, R in enumerate(ref):
                 assert (np.abs(o[r] - R["o_model"]) <= 2.0 ** -7 * R["wabsv"] + 2.0 ** -12 * R["vmax"]).all(), (l, r)
                 assert (np.abs(lse[r] - R["lse_model"]) <= 2.0 ** -8).all(), (l, r)
+
+
+def test_cuda_graph_survives_growth_of_tickets_and_partials():
+    """After a graph has pinned its cache entry, a call with more than 1024 (request, kv head) groups AND a larger
+    partial buffer makes both context buffers grow in one call.  The outgrown buffers are what the graph still points
+    at: they must stay allocated until kvr_destroy (freeing them at regrowth handed a later replay freed memory, and
+    kvr_destroy then freed them a second time).  Replay twice after the growth and check the outputs."""
+    from paper_2606_17107_b200 import kvr
+    from paper_2606_17107_b200.harness import DeviceReadWorkload
+    w = read_workload("graph-grow", q_heads=8, kv_heads=2, layers=2, requests=[[(900, 5), (200, -3)], [(1500, 777)]], seed=99)
+    srcs_t, q_t = make_read_sources(w, "cpu"), make_queries(w, "cpu")
+    dw = DeviceReadWorkload(w, "cuda:0", sources=srcs_t, queries=q_t)
+    outs = [(torch.empty_like(dw.o), torch.empty_like(dw.lse)) for _ in range(2)]
+    big = DeviceReadWorkload(read_workload("many-groups", q_heads=8, kv_heads=2, requests=[[(8, i)] for i in range(640)], seed=5),
+                             "cuda:0")                          # 1280 groups > the 1024-ticket floor; 1280 items x 4 x 130 floats > 1 MB
+    stream = torch.cuda.Stream()
+    with kvr.Context(dw.model) as ctx:
+        call = lambda l: ctx.rotate_on_read_attention(dw.q, w.n_req, w.q_heads, l, w.scale, dw.segs, outs[l][0], outs[l][1], stream=stream)
+        call(0)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(stream):
+            graph.capture_begin()
+            for l in range(2):
+                call(l)
+            graph.capture_end()
+        big.run(ctx, stream=stream)                              # tickets and partials both outgrown in this call
+        torch.cuda.synchronize()
+        assert torch.isfinite(big.o).all() and torch.isfinite(big.lse).all()
+        srcs = [(np_bits(k), np_bits(v)) for k, v in srcs_t]
+        for rep in range(2):
+            for o_, l_ in outs:
+                o_.fill_(float("nan")); l_.fill_(float("nan"))
+            with torch.cuda.stream(stream):
+                graph.replay()
+            big.run(ctx, stream=stream)                          # the new buffers in use right behind the replay
+            torch.cuda.synchronize()
+            for l in range(2):
+                w.layer = l
+                ref = reference(w, srcs, np_bits(q_t), orc.host_threads())
+                o, lse = outs[l][0].cpu().numpy().astype(np.float64), outs[l][1].cpu().numpy().astype(np.float64)
+                for r, R in enumerate(ref):
+                    assert (np.abs(o[r] - R["o_model"]) <= 2.0 ** -7 * R["wabsv"] + 2.0 ** -12 * R["vmax"]).all(), (rep, l, r)
+                    assert (np.abs(lse[r] - R["lse_model"]) <= 2.0 ** -8).all(), (rep, l, r)

@@ -214,3 +214,23 @@ def test_bytes_read_and_argument_checks():
     k = np.zeros((3, 2, 8), np.uint16)
     with pytest.raises(ValueError):                                            # 4 query heads over 3 kv heads
         orc.rotate_on_read_attention(q=q, kv_heads=3, rotary_dim=8, pairing=0, inv_freq=np.ones(4), scale=1.0, segments=[(k, k, 0)])
+
+
+def test_the_gpu_tests_bound_on_o_is_small_and_holds_for_the_bf16_query_model():
+    """The per-element bound the GPU tests hold |o_kernel - o_oracle| to (tests/test_gpu_attention.py reference(),
+    DESIGN.md section 3) must (a) be small against the output -- median(tol) <= 0.2 median(|o|) on the serving workload;
+    an earlier bound, (expm1(2E) + 2^-8) max|v|, was larger than the output and decided nothing -- and (b) hold for the one
+    deviation that can be evaluated without a GPU: the definition evaluated with the counter-rotated query rounded to
+    bf16 stays within the first-order + remainder part of the bound (no 2^-7 slack for the kernel's bf16 weights)."""
+    from tests.test_gpu_attention import reference
+    from tests.helpers import np_bits
+    from workloads import attention_config, make_queries, make_read_sources
+    w = attention_config("attend-serving", shrink=16)
+    srcs_t, q_t = make_read_sources(w, "cpu"), make_queries(w, "cpu")
+    ref = reference(w, [(np_bits(k), np_bits(v)) for k, v in srcs_t], np_bits(q_t), orc.host_threads())
+    tol = np.concatenate([R["tol_ref"].ravel() for R in ref])
+    mag = np.concatenate([np.abs(R["o_ref"]).ravel() for R in ref])
+    assert np.median(tol) <= 0.2 * np.median(mag), (np.median(tol), np.median(mag))
+    for R in ref:
+        assert (np.abs(R["o_model"] - R["o_ref"]) <= R["tol_first_order"] + 1e-12).all()
+        assert (np.abs(R["lse_model"] - R["lse_ref"]) <= R["E"] + 1e-12).all()
