@@ -89,6 +89,7 @@ def parse_args(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-next", action="store_true", help="skip the short NEXT-row cases of the default run")
     ap.add_argument("--layers", type=int, default=None,
                     help="profiling aid: keep only the first N layers of the configuration (same kernel, tiles and "
                          "per-layer access pattern, less memory for ncu to save and restore); never a bench number")
@@ -366,6 +367,23 @@ class Timer:
         self.rep.barrier()
         return ev0.elapsed_time(ev1) * 1e-3
 
+    def single_calls(self, run_step, n=15):
+        """`n` ISOLATED steps: the device is idle when each one starts (synchronize on both sides), so nothing of the
+        previous call's tail overlaps its ramp (no programmatic dependent launch, no early source loads).  This is the
+        figure for the paper's use -- one transplant per request on the TTFT path, one re-float per turn
+        (PAPER.md:528).  CUDA events around one launch add a few microseconds.  Returns the per-call seconds."""
+        import torch
+        out = []
+        for _ in range(n):
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(self.device)
+            ev0.record(self.stream)
+            run_step()
+            ev1.record(self.stream)
+            torch.cuda.synchronize(self.device)
+            out.append(ev0.elapsed_time(ev1) * 1e-3)
+        return out
+
     def blocks(self, run_step, steps, est_step_s, min_device_s, max_blocks=2000):
         """Blocks of `steps` steps back to back (one event between blocks, no host sync inside) until the device has
         been timed for >= min_device_s.  Returns the per-block seconds."""
@@ -411,6 +429,7 @@ def measure_case(kvr, timer, ctx_of, w, dw, op, steps, warmup, min_device_s, pea
             exact_s = timer.exact_block(run_step, steps) if headline else None
             launches_exact = ctx.launch_count() - launches0
             blk = timer.blocks(run_step, steps, est, min_device_s)
+            single = timer.single_calls(run_step)
         out["remeasured"] = attempt > 0
         if not timer.sampler.bad():
             break
@@ -428,12 +447,80 @@ def measure_case(kvr, timer, ctx_of, w, dw, op, steps, warmup, min_device_s, pea
         "tokens_per_s": w.tokens / med,
         "achieved": gbs(med), "best_achieved": gbs(best), "unit": "GB/s", "frac": gbs(med) / peak,
         "best_frac": gbs(best) / peak, "gb_s_of_nominal_8000": gbs(med) / 8000.0,
+        "single_call_us": _median(single) * 1e6, "single_call_achieved": gbs(_median(single)),
+        "single_call_best_us": min(single) * 1e6, "single_call_calls": len(single),
         "clocks": timer.sampler.summary(), "traffic": traffic_of(w.name, w.layout, op),
         "kernel": {1: "kvr_generic_kernel", 2: "kvr_ring_kernel", 4: "kvr_window_inplace_kernel"}.get(info["path"], "?"),
         "grid": info["grid"], "block": info["block"], "smem": info["smem"],
         "warmup": warmup, "warmup_ramp_steps": ramp,
     })
     return out, exact_s, launches_exact, ctx
+
+
+def measure_attend(kvr, timer, w, device, peak, steps, warmup, min_device_s, tune=None):
+    """Times kvr_rotate_on_read_attention on `w` (one layer per step; source sets rotated so no call finds its keys in
+    L2).  Returns (entry, exact seconds of `steps` steps, launches in them, the device workloads)."""
+    from paper_2606_17107_b200.harness import DeviceReadWorkload
+    sets = max(1, min(8, int(-(-3 * L2_BYTES // max(1, w.bytes_read())))))
+    dws = [DeviceReadWorkload(w, device) for _ in range(sets)]
+    ctx = kvr.Context(dws[0].model, device=device.index)
+    if tune:
+        ctx.set_tuning(**tune)
+    state = {"i": 0}
+
+    def run_step():
+        dws[state["i"] % sets].run(ctx, stream=timer.stream)
+        state["i"] += 1
+    ramp, est = timer.warm(run_step, warmup)
+    timer.sampler.reset()
+    l0 = ctx.launch_count()
+    with timer.sampler:
+        exact_s = timer.exact_block(run_step, steps)
+        launches = ctx.launch_count() - l0
+        blk = timer.blocks(run_step, steps, est, min_device_s)
+        single = timer.single_calls(run_step)
+    per = [b / steps for b in blk]
+    med, best, worst = _median(per), min(per), max(per)
+    info = ctx.last_launch_info()
+    b = dws[0].bytes_read()
+    ctx.close()
+    entry = {"workload": w.name, "op": "attend", "bytes_per_step": int(b), "ms_per_step": med * 1e3,
+             "achieved": b / med / 1e9, "best_achieved": b / best / 1e9, "unit": "GB/s", "frac": b / med / 1e9 / peak,
+             "spread": (worst - best) / med, "blocks": len(blk), "steps_per_block": steps,
+             "single_call_us": _median(single) * 1e6, "single_call_achieved": b / _median(single) / 1e9,
+             "tokens_per_s": w.tokens / med, "clocks": timer.sampler.summary(), "source_sets": sets,
+             "kernel": "kvr_attend_kernel", "grid": info["grid"], "block": info["block"], "smem": info["smem"],
+             "warmup": warmup, "warmup_ramp_steps": ramp}
+    return entry, exact_s, launches, dws
+
+
+NEXT_ROWS = [("inplace", "config", 2), ("span", "config", 1), ("splice", "adapter", "mla-dsv2-lite"),
+             ("splice", "adapter", "compose-qwen3-8b"), ("attend", "read", "attend-serving")]
+
+
+def next_rows(kvr, timer, ctx_of, peak, device, min_device_s=0.1):
+    """One short timed case per SURVEY.md 8(f) row (in place, span overwrite, the MLA adapter, the compose workload,
+    rotate-on-read attention) so that the default run's line carries them: median GB/s of back-to-back calls, fraction of
+    the measured peak, GB/s of an isolated call, clocks.  No oracle leg here (parity is the tests' business)."""
+    import torch
+    from paper_2606_17107_b200.harness import DeviceWorkload
+    from workloads import adapter_config, attention_config, config
+    keep = ("workload", "layout", "op", "bytes_per_step", "ms_per_step", "achieved", "best_achieved", "frac", "unit",
+            "single_call_us", "single_call_achieved", "kernel", "grid", "clocks", "blocks", "steps_per_block")
+    rows = []
+    for op, kind, which in NEXT_ROWS:
+        if kind == "read":
+            entry, _, _, dws = measure_attend(kvr, timer, attention_config(which), device, peak, 20, 3, min_device_s)
+            del dws
+        else:
+            w = config(which, "NHD") if kind == "config" else adapter_config(which, "NHD")
+            dw = DeviceWorkload(w, device)
+            entry, _, _, ctx = measure_case(kvr, timer, ctx_of, w, dw, op, 20, 3, min_device_s, peak, headline=False)
+            ctx.close()
+            del dw
+        rows.append({k: entry[k] for k in keep if k in entry})
+        torch.cuda.empty_cache()
+    return rows
 
 
 def run_kvr(args):
@@ -535,8 +622,25 @@ def run_kvr(args):
         e2e_seconds = time.perf_counter() - t0
         rep.barrier()
         e_agg = aggregate_throughput(rep, tokens * e2e_steps, e2e_seconds)
+        # the ceiling of this leg: a plain pinned-host -> device cudaMemcpyAsync of one source tensor, timed alone
+        hk = max((k for k, _ in dw.host_sources), key=lambda t: t.numel())
+        scratch = torch.empty(hk.shape, dtype=hk.dtype, device=device)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            scratch.copy_(hk, non_blocking=True)
+            ev0.record(stream)
+            for _ in range(3):
+                scratch.copy_(hk, non_blocking=True)
+            ev1.record(stream)
+        torch.cuda.synchronize(device)
+        h2d_peak = 3 * hk.numel() * hk.element_size() / (ev0.elapsed_time(ev1) * 1e-3) / 1e9
+        del scratch
+        e2e_ms = e_agg["seconds"] / e2e_steps * 1e3
         e2e = {"value": e_agg["per_second"], "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": 16,
-               "steps": e2e_steps, "ms_per_step": e_agg["seconds"] / e2e_steps * 1e3,
+               "steps": e2e_steps, "ms_per_step": e2e_ms,
+               "h2d_gbs": h2d / (e2e_ms * 1e-3) / 1e9, "h2d_peak_gbs": h2d_peak,
+               "h2d_frac": h2d / (e2e_ms * 1e-3) / 1e9 / h2d_peak,
+               "h2d_peak_source": f"pinned cudaMemcpyAsync of one {hk.numel() * hk.element_size()} B source tensor, 3 copies, CUDA events",
                "api": "kvr_reposition_splice_host (pinned host K/V sources -> staged H2D overlapped with the kernel) "
                       "+ kvr_last_device_status"}
         dw.host_sources = dw.host_segs = None
@@ -548,6 +652,10 @@ def run_kvr(args):
         cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
                "single_thread_value": getattr(_oracle_sample, "single_thread_value", None),
                "single_thread_sample": "layer 0 of every segment, one thread, scaled linearly to all layers"}
+
+    nxt = None
+    if sweep and rep.world == 1 and args.op == "splice" and not args.workload and not args.no_next:
+        nxt = next_rows(kvr, timer, ctx_of, peak, device)
 
     for c_ in ctxs:
         c_.close()
@@ -583,9 +691,29 @@ def run_kvr(args):
                                                      "blocks", "steps_per_block", "device_s", "remeasured")}
         if latency is not None:
             line["latency"] = latency
+        if nxt is not None:
+            line["next"] = nxt
+        # LAST key, short on purpose: whoever keeps only the tail of this line still sees every case
+        line["per_config_summary"] = summary_of(per_config, nxt)
         print(json.dumps(line), flush=True)
     rep.close()
     return 0
+
+
+def summary_of(per_config, nxt):
+    """Short on purpose (about 600 bytes) and ordered so that configs[1..4] come last: per case
+    [GB/s back to back, fraction of the measured peak, GB/s of an isolated call, median SM MHz, bad clocks]."""
+    def row(e):
+        return [round(e["achieved"]), round(e["frac"], 3), round(e["single_call_achieved"]),
+                round(e["clocks"].get("sm_mhz") or 0), int(any(r in ClockSampler.BAD for r in e["clocks"].get("reasons", [])))]
+    out = {"_": "GB/s,frac,isolated GB/s,MHz,badclk"}
+    for e in nxt or []:
+        name = e["workload"].split("-")[0] if e["workload"].startswith("cfg") else e["workload"]
+        out[name if e["op"] in ("splice", "attend") else f'{e["op"]}:{name}'] = row(e)
+    for e in per_config:
+        name = f'cfg{e["config_index"]}' if e.get("config_index") is not None else e["workload"]
+        out[f'{name}:{e["layout"]}' + ("" if e["op"] == "splice" else ":" + e["op"])] = row(e)
+    return out
 
 
 def run_attend(args):
