@@ -179,3 +179,9 @@ def test_validate_read_without_a_gpu(kvr):
     m8, keep8 = kvr.model_desc(4, 8, 128, 128, kvr.KVR_PAIR_NEOX_HALF, kvr.KVR_FP8_E4M3, inv)
     assert ok([seg()], model=m8) == kvr.KVR_ERR_UNSUPPORTED
     assert kvr.kvr_attention_bytes_read(m, [seg(), seg(len=28)]) == 2 * 8 * 128 * 2 * 128
+    # what a TMA tensor map cannot describe is refused here, before the call would touch its descriptor cache
+    assert ok([seg(strides=(0, 100 * 128, 128))]) == kvr.KVR_ERR_UNSUPPORTED                  # 4 layers on a zero stride
+    assert ok([seg(strides=(1 << 39, 100 * 128, 128))]) == kvr.KVR_ERR_UNSUPPORTED            # 2^40 bytes
+    m1, keep1 = kvr.model_desc(1, 8, 128, 128, kvr.KVR_PAIR_NEOX_HALF, kvr.KVR_BF16, inv)
+    assert ok([seg(strides=(0, 100 * 128, 128))], model=m1) == kvr.KVR_OK                     # one layer never uses its stride
+    assert ok([seg()], n_req=1 << 30) == kvr.KVR_ERR_INVALID_ARG                              # more requests than segments
