@@ -450,7 +450,7 @@ def measure_case(kvr, timer, ctx_of, w, dw, op, steps, warmup, min_device_s, pea
         "single_call_us": _median(single) * 1e6, "single_call_achieved": gbs(_median(single)),
         "single_call_best_us": min(single) * 1e6, "single_call_calls": len(single),
         "clocks": timer.sampler.summary(), "traffic": traffic_of(w.name, w.layout, op),
-        "kernel": {1: "kvr_generic_kernel", 2: "kvr_ring_kernel", 4: "kvr_window_inplace_kernel"}.get(info["path"], "?"),
+        "kernel": {1: "kvr_generic_kernel", 2: "kvr_ring_kernel", 4: "kvr_window_inplace_kernel", 5: "kvr_generic_vec_kernel"}.get(info["path"], "?"),
         "grid": info["grid"], "block": info["block"], "smem": info["smem"],
         "warmup": warmup, "warmup_ramp_steps": ramp,
     })

@@ -139,7 +139,7 @@ typedef struct {
 
 /* Optional tuning knobs (0 = library default).  Never changes results, only the launch shape. */
 typedef struct {
-  int32_t path;            /* 0 auto, 1 force the generic kernel, 2 force the TMA-ring kernel */
+  int32_t path;            /* 0 auto, 1 force the scalar generic kernel, 2 force the TMA-ring kernel, 5 force the generic kernel with 16-byte accesses */
   int32_t ctas_per_sm;     /* persistent CTAs per SM for the ring kernel                       */
   int32_t consumer_warps;  /* consumer warps per CTA                                           */
   int32_t stages;          /* ring depth (tiles in flight per CTA)                             */
@@ -346,7 +346,7 @@ KVR_API uint64_t kvr_bytes_moved(const kvr_model_desc* model, const kvr_segment*
 KVR_API kvr_status kvr_last_device_status(kvr_ctx* ctx, int32_t* bad_segment, int32_t* bad_token);
 
 /* Introspection for benchmarks: kernels launched by this context so far; the kernel path the last call took
- * (1 generic, 2 TMA ring, 3 rotate-on-read attention, 4 window in place); grid size, CTA size and dynamic shared memory of its main kernel. */
+ * (1 generic, 2 TMA ring, 3 rotate-on-read attention, 4 window in place, 5 generic with 16-byte accesses); grid size, CTA size and dynamic shared memory of its main kernel. */
 KVR_API uint64_t kvr_launch_count(const kvr_ctx* ctx);
 KVR_API kvr_status kvr_last_launch_info(const kvr_ctx* ctx, int32_t* path, int32_t* grid, int32_t* block,
                                         int32_t* smem_bytes);

@@ -8,7 +8,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libkvr.so")
-SOURCES = ["kvr_api.cu", "kvr_generic.cu", "kvr_ring.cu", "kvr_attend.cu", "kvr_window.cu"]
+SOURCES = ["kvr_api.cu", "kvr_generic.cu", "kvr_generic_vec.cu", "kvr_ring.cu", "kvr_attend.cu", "kvr_window.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC,-fvisibility=hidden,-Wall", "-shared", "-cudart", "static", "--threads", "4"]
 

@@ -587,12 +587,17 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     decompose(cg, lpu, 1, false);
     path = 4;
   }
-  if (path == 1) {
+  if (path == 1 || path == 5) {
     P.tmajor = 0; P.ct = 0; P.tmaps = nullptr; P.gather = 0;
-    // generic kernel: chunk table [cg][R/2] float4 must fit 48 KB of static-limit shared memory
+    // generic kernels: chunk table [cg][R/2] float4 must fit 48 KB of static-limit shared memory
     int limit = (int)(47 * 1024 / ((m.rotary_dim / 2) * 16 + 4));
     if (limit < 1) return KVR_ERR_UNSUPPORTED;
     decompose(chunk_granularity(d->block_size, limit < 16 ? limit : 16), tu.layers_per_unit, 1, false);
+    // Auto dispatch prefers the 16-byte-access form where the rotary window splits into whole vectors; tuning.path = 1
+    // keeps the scalar kernel (the on-device cross-check), tuning.path = 5 insists on the vector one.
+    const bool vec_ok = generic_vec_supported(P);
+    if (path == 5 && !vec_ok) { c->last_err = "vectorised generic kernel: rotary_dim * esz must be a multiple of 32 (NeoX) or 16 (GPT-J) bytes"; return KVR_ERR_UNSUPPORTED; }
+    if (path == 1 && tu.path == 0 && vec_ok) path = 5;
   }
 
   if (inline_descs) {
@@ -609,10 +614,12 @@ static kvr_status enqueue_layers(kvr_ctx* c, const kvr_paged_dst* d, const kvr_s
     e = launch_ring(P, rc, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
   } else if (path == 4) {
     e = launch_window_inplace(P, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
+  } else if (path == 5) {
+    e = launch_generic_vec(P, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
   } else {
     e = launch_generic(P, c->sm_count, stream, &c->last_grid, &c->last_block, &c->last_smem);
   }
-  if (e != cudaSuccess) return c->cuda_fail(e, path == 2 ? "launch_ring" : path == 4 ? "launch_window_inplace" : "launch_generic");
+  if (e != cudaSuccess) return c->cuda_fail(e, path == 2 ? "launch_ring" : path == 4 ? "launch_window_inplace" : path == 5 ? "launch_generic_vec" : "launch_generic");
   c->launches += 1;
   c->last_path = path;
   c->last_stream = stream;

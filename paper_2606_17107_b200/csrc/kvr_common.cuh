@@ -185,6 +185,10 @@ __device__ __forceinline__ uint32_t f32x2_to_e4m3x2_sat(float lo, float hi) {
 // launch entry points implemented in the .cu files
 cudaError_t launch_generic(const CallParams& P, int sm_count, cudaStream_t stream, int* grid, int* block, int* smem);
 
+// the same kernel with 16-byte accesses, for shapes whose rotary window splits into whole vectors (kvr_generic_vec.cu)
+bool generic_vec_supported(const CallParams& P);
+cudaError_t launch_generic_vec(const CallParams& P, int sm_count, cudaStream_t stream, int* grid, int* block, int* smem);
+
 // in-place re-float of a rotary window inside a longer row (kvr_window.cu)
 bool window_inplace_supported(const CallParams& P);
 cudaError_t launch_window_inplace(const CallParams& P, int sm_count, cudaStream_t stream, int* grid, int* block, int* smem);

@@ -17,7 +17,7 @@ KVR_BF16, KVR_FP8_E4M3 = 0, 1
 KVR_PAIR_NEOX_HALF, KVR_PAIR_GPTJ_INTERLEAVED = 0, 1
 KVR_SEG_PRE_ROPE, KVR_SEG_SRC_STABLE = 1, 2
 KVR_NOALLOC_MAX_SEGMENTS, KVR_NOALLOC_MAX_ROTARY_DIM, KVR_NOALLOC_SCRATCH_BYTES = 8, 1024, 4352
-PATH_AUTO, PATH_GENERIC, PATH_RING, PATH_ATTEND, PATH_WINDOW = 0, 1, 2, 3, 4
+PATH_AUTO, PATH_GENERIC, PATH_RING, PATH_ATTEND, PATH_WINDOW, PATH_GENERIC_VEC = 0, 1, 2, 3, 4, 5
 
 
 class kvr_model_desc(C.Structure):

@@ -13,7 +13,7 @@ from workloads import ADAPTERS, SENTINEL_BF16, adapter_config, adapter_small, ma
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 @pytest.mark.parametrize("layout", ["NHD", "HND"])
 @pytest.mark.parametrize("name", ADAPTERS)
 def test_adapter_small(name, layout, path):
@@ -41,7 +41,7 @@ def _mla(pairing, dtype="bf16", layout="NHD", scales_differ=False, D=576, off=51
                                         dict(len=131, dst_token_start=6, new_start=161)]])
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 @pytest.mark.parametrize("pairing,dtype,scales_differ,pad", [("gptj", "bf16", False, 0), ("neox", "bf16", False, 8),
                                                              ("gptj", "fp8", False, 0), ("neox", "fp8", True, 16),
                                                              ("gptj", "fp8", True, 0)])
@@ -58,7 +58,7 @@ def test_mla_ring_wraps(tuning):
     check_parity(adapter_small("mla-dsv2-lite"), "ring", **tuning)
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 @pytest.mark.parametrize("layout", ["NHD", "HND"])
 @pytest.mark.parametrize("pairing,D,R,off,dtype,has_v", [
     ("neox", 96, 64, 0, "bf16", True),      # head_dim 96 (192-byte rows): window mode with a V tensor
@@ -80,7 +80,7 @@ def test_rows_that_are_not_a_power_of_two(pairing, D, R, off, dtype, has_v, layo
     check_parity(w, path)
 
 
-@pytest.mark.parametrize("path", ["auto", "generic"])
+@pytest.mark.parametrize("path", ["auto", "generic", "generic_vec"])
 @pytest.mark.parametrize("pairing", ["neox", "gptj"])
 def test_mla_inplace_refloat(pairing, path):
     """kvr_reposition_inplace on a resident [latent | k_pe] chunk: only the k_pe window changes; v_cache is NULL."""
@@ -181,7 +181,7 @@ def _compose(dtype="bf16", layout="NHD", pairing="neox", with_map=False, D=128, 
                        dict(len=40, dst_token_start=135, new_start=135, pre_rope=True)]])
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 @pytest.mark.parametrize("dtype,layout,pairing,with_map,heads", [("bf16", "NHD", "neox", False, 4), ("bf16", "HND", "gptj", True, 8),
                                                               ("fp8", "NHD", "neox", True, 8), ("bf16", "NHD", "neox", True, 2)])
 def test_compose_skill_seam_and_fresh_suffix_in_one_call(dtype, layout, pairing, with_map, heads, path):

@@ -14,7 +14,7 @@ from workloads import config, config_small, make_workload
 
 pytestmark = pytest.mark.gpu
 
-PATHS = {"generic": 1, "ring": 2}
+PATHS = {"generic": 1, "ring": 2, "generic_vec": 5}
 WINDOW = 4                      # kvr_last_launch_info path of the window in-place kernel (auto dispatch only)
 
 
@@ -103,7 +103,7 @@ class _PoolOnly:
         return getattr(self._dw, name)
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 @pytest.mark.parametrize("layout", ["NHD", "HND"])
 @pytest.mark.parametrize("c", [0, 1, 2, 3, 4])
 def test_inplace_small_configs(c, layout, path):
@@ -115,7 +115,7 @@ def test_inplace_small_configs(c, layout, path):
         assert np.mean(d == 0) > 0.95
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 @pytest.mark.parametrize("layout", ["NHD", "HND"])
 def test_inplace_with_position_map_and_without_v(layout, path):
     w = config_small(1, layout)
@@ -131,7 +131,7 @@ def test_inplace_ring_wraps(c, tuning):
     check_inplace(w, "ring", **tuning)
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 @pytest.mark.parametrize("layout", ["NHD", "HND"])
 @pytest.mark.parametrize("pairing,D,R,dtype", [("neox", 32, 32, "bf16"), ("gptj", 32, 16, "bf16"),
                                                ("neox", 64, 64, "fp8"), ("gptj", 64, 32, "fp8"),
@@ -147,7 +147,7 @@ def test_inplace_edge_cases(layout, pairing, D, R, dtype, path):
     check_inplace(w, path)
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 def test_inplace_bad_block_sets_status_and_skips(path):
     from paper_2606_17107_b200 import kvr
     w = make_workload(name="bad", layers=2, kv_heads=2, head_dim=64, theta=1e4, block_size=4, seed=2,
@@ -250,7 +250,7 @@ def test_inplace_full_size_every_layer(c, layout):
 
 
 # ------------------------------------------------------------------ NEXT-2: span overwrite
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 @pytest.mark.parametrize("layout", ["NHD", "HND"])
 @pytest.mark.parametrize("c", [0, 3, 4])
 def test_write_span_is_a_byte_exact_scatter(c, layout, path):
@@ -306,7 +306,7 @@ def test_seam_repair_overwrites_the_first_token_of_a_spliced_chunk():
     assert k_distance(w, gk[~repaired], kc[~repaired]).max() <= K_TOL["bf16"]
 
 
-@pytest.mark.parametrize("path", ["window", "generic"])
+@pytest.mark.parametrize("path", ["window", "generic", "generic_vec"])
 @pytest.mark.parametrize("layout", ["NHD", "HND"])
 @pytest.mark.parametrize("pairing,D,R,off,dtype", [
     ("neox", 576, 64, 512, "bf16"),      # the MLA [latent 512 | k_pe 64] row

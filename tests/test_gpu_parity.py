@@ -10,12 +10,13 @@ from workloads import (SENTINEL_BF16, config, config_small, make_workload, pos_m
 
 pytestmark = pytest.mark.gpu
 
-PATHS = {"generic": 1, "ring": 2}
+PATHS = {"generic": 1, "ring": 2, "generic_vec": 5}
 GUARD = 1 << 16      # canary bytes before and after every device buffer of a parity run (harness.DeviceWorkload)
 
 
 class RingDeclined(Exception):
-    """The forced ring kernel refused a shape outside its domain (the generic kernel covers it)."""
+    """The forced ring kernel (or the forced 16-byte-access generic kernel) refused a shape outside its domain (the
+    scalar generic kernel covers it)."""
 
 
 def _gpu(w, srcs, tuning):
@@ -28,7 +29,7 @@ def _gpu(w, srcs, tuning):
         try:
             dw.run(ctx)
         except kvr.KvrError as e:
-            if e.status == kvr.KVR_ERR_UNSUPPORTED and tuning.get("path") == PATHS["ring"]:
+            if e.status == kvr.KVR_ERR_UNSUPPORTED and tuning.get("path") in (PATHS["ring"], PATHS["generic_vec"]):
                 raise RingDeclined(str(e)) from e
             raise
         st, seg, tok = ctx.last_device_status()
@@ -67,7 +68,7 @@ def test_auto_dispatch_takes_the_ring_kernel_on_every_baseline_config(c, layout)
     assert status[0] == 0 and info["path"] == PATHS["ring"], info
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 @pytest.mark.parametrize("layout", ["NHD", "HND"])
 @pytest.mark.parametrize("c", [0, 1, 2, 3, 4])
 def test_small_configs(c, layout, path):
@@ -90,7 +91,7 @@ def test_ring_wraps_many_times_per_cta(c, tuning):
     check_parity(w, "ring", **tuning)
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 @pytest.mark.parametrize("layout", ["NHD", "HND"])
 @pytest.mark.parametrize("pairing,D,R,dtype", [("neox", 32, 32, "bf16"), ("gptj", 32, 16, "bf16"),
                                                ("neox", 64, 32, "bf16"), ("gptj", 16, 16, "bf16"),
@@ -112,7 +113,7 @@ def test_edge_cases(layout, pairing, D, R, dtype, path):
     check_parity(w, path)
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 @pytest.mark.parametrize("bs", [1, 8, 16, 24, 32, 128])
 def test_block_sizes_and_ragged(bs, path):
     w = make_workload(name="bs", layers=2, kv_heads=2, head_dim=128, theta=1e6, block_size=bs, seed=5,
@@ -121,7 +122,7 @@ def test_block_sizes_and_ragged(bs, path):
     check_parity(w, path)
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 def test_pos_map_with_zero_delta_tokens(path):
     pm = pos_map_with_gaps(301, 500, 0.3, 64, 5)
     pm[:5] = np.arange(5)                               # Delta_t = 0 for the first five tokens
@@ -131,7 +132,7 @@ def test_pos_map_with_zero_delta_tokens(path):
     check_parity(w, path)
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 def test_many_small_segments(path):
     """Block-granular memory (S <= 16 independently precompiled blocks), each with its own Delta."""
     rng = np.random.default_rng(8)
@@ -146,7 +147,7 @@ def test_many_small_segments(path):
     check_parity(w, path)
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 def test_delta_zero_is_byte_copy(path):
     w = make_workload(name="d0", layers=1, kv_heads=2, head_dim=64, theta=1e4, block_size=4, seed=1,
                       seq_segments=[[dict(len=9, dst_token_start=2, new_start=0)]])
@@ -158,7 +159,7 @@ def test_delta_zero_is_byte_copy(path):
     assert np.array_equal(gk, kc) and np.array_equal(gv, vc)          # bit-exact, payloads included
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 def test_unallocated_block_sets_sticky_status_and_skips(path):
     w = make_workload(name="bad", layers=2, kv_heads=2, head_dim=64, theta=1e4, block_size=4, seed=2,
                       seq_segments=[[dict(len=10, dst_token_start=2, new_start=2)],
@@ -400,7 +401,7 @@ def test_gather_mode_ragged_blocks(bs, heads, D, dtype):
     check_parity(w, "ring", transpose_load=1, tile_bytes=2048, max_ctas=2, stages=3)
 
 
-@pytest.mark.parametrize("path", ["generic", "ring"])
+@pytest.mark.parametrize("path", ["generic", "generic_vec", "ring"])
 def test_thousands_of_tiny_segments(path):
     """2600 segments in one call: descriptor staging grows past its initial capacity and the ring kernel's producer
     searches the segments' unit prefix sums in global memory (more than fit its shared-memory copy)."""
@@ -512,7 +513,7 @@ def test_auto_dispatch_falls_back_when_the_ring_layout_cannot_fit(dtype):
                       seq_segments=[[dict(len=70, dst_token_start=5, new_start=300, pos_map=pm)]])
     srcs, kc, vc = materialize_cpu(w)
     gk, gv, status, info = _gpu(w, srcs, dict(path=0))
-    assert status[0] == 0 and info["path"] == PATHS["generic"], info
+    assert status[0] == 0 and info["path"] == PATHS["generic_vec"], info     # the generic kernel with 16-byte accesses
     run_oracle(w, srcs, kc, vc)
     assert np.array_equal(gv, vc) and k_distance(w, gk, kc).max() <= K_TOL[w.dtype]
     with pytest.raises(RingDeclined):
