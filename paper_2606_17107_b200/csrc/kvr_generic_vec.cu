@@ -99,10 +99,23 @@ __device__ __forceinline__ void requant_vec(uint4& A, const RowScale& sc) {
   A = make_uint4(a[0], a[1], a[2], a[3]);
 }
 
-constexpr int kUnroll = 4;   // vectors (NeoX: pair-vectors) a thread has in flight per iteration
+// Launch shape, measured on B200 over configs[1] / [3] fp8 / [4] forced through this kernel (GB/s): 2 items in flight per
+// thread with >= 4 CTAs per SM (<= 64 registers) 2895 / 2761 / 3855; 4 items, 2 CTAs 2650 / 2601 / 3291; 1 item, 6 CTAs
+// 2719 / 2585 / 3141; 4 items, 3 CTAs 2314 / 1907 / 3368: more resident warps beat more loads per warp.
+#ifndef KVR_GVEC_UNROLL
+#define KVR_GVEC_UNROLL 2
+#endif
+#ifndef KVR_GVEC_COPY_UNROLL
+#define KVR_GVEC_COPY_UNROLL KVR_GVEC_UNROLL
+#endif
+#ifndef KVR_GVEC_MIN_CTAS
+#define KVR_GVEC_MIN_CTAS 4
+#endif
+constexpr int kUnroll = KVR_GVEC_UNROLL;            // rotary items (NeoX: pair-vectors) a thread has in flight per iteration
+constexpr int kCopyUnroll = KVR_GVEC_COPY_UNROLL;   // plain 16-byte copies (pass-through dims, V) in flight per iteration
 
 template <int DTYPE, int PAIRING>
-__global__ void __launch_bounds__(256) kvr_generic_vec_kernel(const __grid_constant__ CallParams P) {
+__global__ void __launch_bounds__(256, KVR_GVEC_MIN_CTAS) kvr_generic_vec_kernel(const __grid_constant__ CallParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float4* tab = reinterpret_cast<float4*>(smem_raw);                 // [cg][R/2]
   int32_t* is_copy = reinterpret_cast<int32_t*>(tab + (size_t)P.cg * (P.rotary_dim / 2));  // [cg]
@@ -201,11 +214,11 @@ __global__ void __launch_bounds__(256) kvr_generic_vec_kernel(const __grid_const
     // ---- K pass-through vectors ([0, rotary_offset) and [rotary_offset + R, D)) and all V vectors: copies ----
     const int per_row = npass + (P.no_v ? 0 : nvec);
     const int64_t n_copy = (int64_t)rows * per_row;
-    for (int64_t base = threadIdx.x; base < n_copy; base += (int64_t)blockDim.x * kUnroll) {
-      uint4 A[kUnroll];
-      uint8_t* dp[kUnroll];
+    for (int64_t base = threadIdx.x; base < n_copy; base += (int64_t)blockDim.x * kCopyUnroll) {
+      uint4 A[kCopyUnroll];
+      uint8_t* dp[kCopyUnroll];
 #pragma unroll
-      for (int u = 0; u < kUnroll; ++u) {
+      for (int u = 0; u < kCopyUnroll; ++u) {
         const int64_t idx = base + (int64_t)u * blockDim.x;
         dp[u] = nullptr;
         if (idx >= n_copy) continue;
@@ -229,7 +242,7 @@ __global__ void __launch_bounds__(256) kvr_generic_vec_kernel(const __grid_const
         }
       }
 #pragma unroll
-      for (int u = 0; u < kUnroll; ++u)
+      for (int u = 0; u < kCopyUnroll; ++u)
         if (dp[u]) st16(dp[u], A[u]);
     }
   }
